@@ -1,0 +1,158 @@
+/* include/muca.h -- C ABI of libmuca_b200: the data-parallel hot path of parallel
+ * multicanonical (MUCA) simulation of the 2D Ising model (arXiv 1707.00919),
+ * hand-written CUDA for sm_100a (NVIDIA B200).
+ *
+ * What the library computes (citations: /root/reference/PAPER.md line numbers,
+ * "R<n>" = reading listed in DESIGN.md section 3):
+ *   - W independent walkers, each on its own L x L periodic Ising lattice
+ *     ("p independent walkers", Eq. (5)),
+ *   - single-spin-flip Metropolis updates accepted with
+ *     min(1, exp[omega(E') - omega(E)]), omega = ln W,
+ *     sites visited in typewriter order (R3), uniform deviates from the
+ *     counter-based Philox4x32-10 generator keyed by (seed; site, sweep,
+ *     iteration, walker) (R4),
+ *   - one shared histogram H(E) of the energies met after every attempted flip
+ *     of the measured sweeps (thermalisation sweeps are not
+ *     recorded),
+ *   - the weight recursion W(n+1)(E) = W(n)(E) / H(n)(E)  (Eq. (4), R8).
+ *
+ * Conventions
+ *   N = L*L spins, n_bins = N + 1 energy slots, slot j = (E + 2N)/4, E = -2N + 4j
+ *   (energies spaced by 4 on [-2N, 2N]; slots 1 and N-1 are unreachable).
+ *   Spins are +1 / -1; packed on the device with bit 1 <-> spin -1.
+ *
+ * General rules
+ *   - every call returns MUCA_OK (0) or a negative muca_status; no exceptions cross
+ *     the boundary; muca_last_error() returns a NUL-terminated description of the
+ *     last failure on that context (owned by the context, valid until the next call);
+ *   - "host" pointers are ordinary host memory owned by the caller, sized exactly as
+ *     stated; "device" pointers are CUDA device memory of the current device;
+ *   - the context owns all device state except a workspace handed to muca_create_in();
+ *   - calls on one context must not run concurrently; different contexts are independent;
+ *   - there is no CPU fallback: without a CUDA device every compute entry point
+ *     fails with MUCA_ECUDA.
+ */
+#ifndef MUCA_H_
+#define MUCA_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct muca_ctx muca_ctx;
+
+typedef enum muca_status {
+    MUCA_OK = 0,
+    MUCA_EINVAL = -1, /* bad argument (L, n_walkers, n_bins, negative sweeps, NULL, wrong size) */
+    MUCA_ECUDA = -2,  /* a CUDA runtime call or kernel failed; see muca_last_error()            */
+    MUCA_ERANGE = -3, /* iteration counter exhausted (0xFFFFFFFF is reserved for init, R5)      */
+    MUCA_ENOMEM = -4  /* workspace too small / allocation failed                                */
+} muca_status;
+
+/* Sweep-kernel variants (muca_set_option(ctx, MUCA_OPT_KERNEL, ...)).
+ * AUTO picks RESIDENT when the packed lattices of one block plus the tables fit in
+ * shared memory (L <= 64) and STREAMED otherwise (L = 128). */
+enum { MUCA_KERNEL_AUTO = 0, MUCA_KERNEL_RESIDENT = 1, MUCA_KERNEL_STREAMED = 2 };
+enum {
+    MUCA_OPT_KERNEL = 1,          /* one of MUCA_KERNEL_*                                        */
+    MUCA_OPT_THREADS_PER_BLOCK = 2, /* walkers (= threads) per block; 0 = library default         */
+    MUCA_OPT_MAX_SWEEPS_PER_LAUNCH = 3 /* split an iteration into launches of at most this many sweeps;
+                                          0 = only as needed to keep a block's uint32 bins from overflowing */
+};
+
+/* Device workspace needed by muca_create_in() for (L, n_walkers); 0 on bad arguments. */
+size_t muca_workspace_bytes(int L, int n_walkers);
+
+/* Create a context and initialise the walkers on the device (R1, R2, R5):
+ *   spin of site i = y*L + x of GLOBAL walker g = walker_offset + w is
+ *   1 - 2*bit(i & 31) of word ((i >> 5) & 3) of Philox4x32-10(ctr = (i >> 7, 0, 0xFFFFFFFF, g),
+ *   key = (seed & 0xFFFFFFFF, seed >> 32)); energies are computed from scratch (Eq. (5));
+ *   omega == 0; iteration counter n = 0.
+ * L must be one of 8, 16, 32, 64, 128 (R13); n_walkers >= 1.
+ * muca_create      : the library allocates its own device memory and uses the legacy default stream.
+ * muca_create_in   : device memory and stream are the caller's (e.g. a torch tensor and torch's
+ *                    current stream): d_workspace must hold muca_workspace_bytes() bytes, be
+ *                    256-byte aligned and outlive the context; cuda_stream is a cudaStream_t
+ *                    (NULL = default stream).  walker_offset shards walkers over several
+ *                    contexts/GPUs with results independent of the split (R16).
+ * On failure *out is NULL and the status is returned. */
+int muca_create(muca_ctx** out, int L, int n_walkers, uint64_t seed);
+int muca_create_in(muca_ctx** out, int L, int n_walkers, uint64_t seed, uint32_t walker_offset,
+                   void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+void muca_destroy(muca_ctx* ctx);
+
+/* Tuning knobs (see the enums above). Returns MUCA_EINVAL for unknown options/values. */
+int muca_set_option(muca_ctx* ctx, int option, int value);
+
+/* omega(E_j) = ln W(E_j), j = 0..n_bins-1, host double[n_bins], n_bins must equal L*L+1.
+ * set: copies the table into the context; does not touch spins or the iteration counter.
+ * (the log-weights are the only state shared by the walkers.) */
+int muca_set_log_weights(muca_ctx* ctx, const double* logw, int n_bins);
+int muca_get_log_weights(muca_ctx* ctx, double* logw_out, int n_bins);
+
+/* One MUCA iteration with the current fixed weights (Fig. 1):
+ *   1. acceptance thresholds from omega, in double, on the host (R6, R7, R12):
+ *        for slot j, a antiparallel neighbours, j' = j + 2 - a:
+ *        a == 2 -> t = 0xFFFFFFFF;  j' outside [0, N] -> t = 0;
+ *        d = omega[j'] - omega[j];  T = 2^32 if d >= 0 else floor(exp(d) * 2^32) clamped to [1, 2^32];
+ *        t = T - 1;  a move is accepted iff the Philox word r <= t;
+ *   2. therm_sweeps + sweeps typewriter sweeps of every walker on the device; the deviate of site i
+ *      in sweep s of iteration n of global walker g is word (i & 3) of
+ *      Philox4x32-10(ctr = (i >> 2, s, n, g), key);
+ *   3. H[j] += 1 after every attempt (accepted or not) of the last `sweeps` sweeps, j the slot after
+ *      the decision; per-block shared-memory histograms are merged into one uint64 histogram;
+ *   4. n <- n + 1.
+ * H_out: host uint64[n_bins] (may be NULL: H stays in the context for muca_update_weights /
+ * muca_get_histogram).  sum(H) = n_walkers * sweeps * N.  therm_sweeps, sweeps >= 0.
+ * Synchronises the context's stream before returning. */
+int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_out, int n_bins);
+
+/* Histogram of the last muca_run_iteration (host uint64[n_bins]). */
+int muca_get_histogram(muca_ctx* ctx, uint64_t* H_out, int n_bins);
+
+/* Eq. (4), R8: omega[j] -= ln(H[j]) for every j with H[j] > 0 (raw counts,
+ * natural log, host double); unvisited slots keep their omega.
+ * muca_update_weights      uses the H of the last muca_run_iteration on this context;
+ * muca_update_weights_with uses a caller-supplied total histogram (host uint64[n_bins]) --
+ *                          H summed over all shards when walkers are split over GPUs. */
+int muca_update_weights(muca_ctx* ctx);
+int muca_update_weights_with(muca_ctx* ctx, const uint64_t* H_total, int n_bins);
+
+/* Per-walker energies E (host int32[n_walkers]) as tracked incrementally by the sweeps. */
+int muca_get_energies(muca_ctx* ctx, int32_t* E_out, int n_walkers);
+
+/* Spin configurations, host int8[n = n_walkers*L*L], out[w*N + y*L + x] = +1 / -1.
+ * set: replaces the configurations and recomputes the energies from scratch on the device. */
+int muca_get_spins(muca_ctx* ctx, int8_t* spins_out, size_t n);
+int muca_set_spins(muca_ctx* ctx, const int8_t* spins, size_t n);
+
+/* Same as muca_get_spins but into DEVICE memory int8[n] (no host copy); asynchronous on the
+ * context's stream. */
+int muca_unpack_spins_device(muca_ctx* ctx, void* d_spins_out, size_t n);
+
+/* Debug / diagnostics.
+ * thresholds: host uint32[n = n_bins*5], out[j*5 + a] as defined under muca_run_iteration, from the
+ *             current omega.
+ * iteration : the counter n that the next muca_run_iteration will use in the Philox counter.
+ * last_sweep_ms: device time (CUDA events on the context's stream) of the sweep kernel launch(es)
+ *             of the last muca_run_iteration, in milliseconds; *launches = number of kernel launches. */
+int muca_get_thresholds(muca_ctx* ctx, uint32_t* out, size_t n);
+int muca_get_iteration(muca_ctx* ctx, uint32_t* n_out);
+int muca_set_iteration(muca_ctx* ctx, uint32_t n);
+int muca_last_sweep_ms(muca_ctx* ctx, double* ms_out, int* launches_out);
+const char* muca_last_error(const muca_ctx* ctx);
+
+/* Test hook: Philox4x32-10 evaluated ON THE DEVICE for n (ctr, key) pairs.
+ * ctr: host uint32[4n], key: host uint32[2n], out: host uint32[4n]. */
+int muca_debug_philox(const uint32_t* ctr, const uint32_t* key, uint32_t* out, int n);
+
+/* Library version string. */
+const char* muca_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MUCA_H_ */

@@ -1,0 +1,473 @@
+// paper_1707_00919_b200/csrc/muca.cu -- host side of libmuca_b200 (C ABI declared in include/muca.h).
+// Context, threshold-table build (double, host libm: DESIGN.md R12), weight update (Eq. (4)), launch logic.
+// There is NO CPU fallback: every compute entry point needs a CUDA device and fails with MUCA_ECUDA otherwise.
+#include "../../include/muca.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "muca_device.cuh"
+
+using namespace muca;
+
+struct muca_ctx {
+    int L = 0, N = 0, W = 0, n_bins = 0;
+    uint64_t seed = 0;
+    uint32_t walker_offset = 0;
+    uint32_t iteration = 0;
+    cudaStream_t stream = nullptr;
+    bool own_workspace = false;
+    void* d_workspace = nullptr;
+    // carved from the workspace
+    uint32_t* d_spins = nullptr;
+    int32_t* d_E = nullptr;
+    uint32_t* d_table = nullptr;
+    unsigned long long* d_H = nullptr;
+    // host state
+    std::vector<double> logw;       // omega, n_bins
+    std::vector<uint64_t> H;        // last histogram
+    uint32_t* h_table = nullptr;    // pinned, n_bins*8
+    unsigned long long* h_H = nullptr;  // pinned, n_bins
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    double last_sweep_ms = 0.0;
+    int last_launches = 0;
+    int opt_kernel = MUCA_KERNEL_AUTO;
+    int opt_tpb = 0;
+    int opt_max_sweeps = 0;
+    char err[512] = {0};
+};
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+
+bool valid_L(int L) { return L == 8 || L == 16 || L == 32 || L == 64 || L == 128; }
+
+struct Carve { size_t spins, E, table, H, total; };
+Carve carve(int L, int W) {
+    const size_t N = (size_t)L * L, bins = N + 1;
+    Carve c;
+    size_t off = 0;
+    c.spins = off; off += align_up((size_t)W * (N / 8));
+    c.E = off;     off += align_up((size_t)W * 4);
+    c.table = off; off += align_up(bins * 8 * 4);
+    c.H = off;     off += align_up(bins * 8);
+    c.total = off;
+    return c;
+}
+
+int fail(muca_ctx* c, int code, const char* fmt, ...) {
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(c->err, sizeof(c->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+#define CU(call)                                                                                     \
+    do {                                                                                             \
+        cudaError_t e_ = (call);                                                                     \
+        if (e_ != cudaSuccess)                                                                       \
+            return fail(ctx, MUCA_ECUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_),     \
+                        __FILE__, __LINE__);                                                         \
+    } while (0)
+
+// Acceptance thresholds thresh[j][a], a = 0..4 (include/muca.h, muca_run_iteration step 1, R6/R7/R9).
+void build_thresholds5(const std::vector<double>& omega, std::vector<uint32_t>& t5) {
+    const int bins = (int)omega.size();
+    t5.assign((size_t)bins * 5, 0u);
+    const double two32 = 4294967296.0;
+    for (int j = 0; j < bins; ++j)
+        for (int a = 0; a < 5; ++a) {
+            uint32_t t = 0u;
+            const int jn = j + 2 - a;
+            if (a == 2) t = 0xFFFFFFFFu;
+            else if (jn >= 0 && jn < bins) {
+                const double d = omega[jn] - omega[j];
+                if (d >= 0.0) t = 0xFFFFFFFFu;
+                else {
+                    double T = std::floor(std::ldexp(std::exp(d), 32));
+                    if (T < 1.0) T = 1.0;
+                    if (T > two32) T = two32;
+                    t = (uint32_t)((uint64_t)T - 1u);
+                }
+            }
+            t5[(size_t)j * 5 + a] = t;
+        }
+}
+
+// Device format T8[j][f], f = 4*hi + 2*lo + g, a = (lo + 2*hi) + g  (muca_device.cuh).
+void expand_table8(const std::vector<uint32_t>& t5, int bins, uint32_t* t8) {
+    for (int j = 0; j < bins; ++j)
+        for (int f = 0; f < 8; ++f) {
+            const int a = (f >> 1) + (f & 1);
+            t8[(size_t)j * 8 + f] = t5[(size_t)j * 5 + a];
+        }
+}
+
+template <int L, int MODE>
+int launch_sweep_t(muca_ctx* ctx, const SweepParams& prm, int tpb) {
+    const size_t smem = sweep_smem_bytes<L, MODE>(tpb);
+    static size_t configured = 0;
+    if (smem > configured) {
+        CU(cudaFuncSetAttribute(sweep_kernel<L, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured = smem;
+    }
+    const int grid = (prm.W + tpb - 1) / tpb;
+    sweep_kernel<L, MODE><<<grid, tpb, smem, ctx->stream>>>(prm);
+    CU(cudaGetLastError());
+    return MUCA_OK;
+}
+
+struct Plan { int mode; int tpb; };
+
+Plan make_plan(const muca_ctx* c) {
+    Plan p;
+    const int L = c->L;
+    int kern = c->opt_kernel;
+    if (kern == MUCA_KERNEL_AUTO) kern = L <= 64 ? MUCA_KERNEL_RESIDENT : MUCA_KERNEL_STREAMED;
+    if (kern == MUCA_KERNEL_STREAMED && L < 32) kern = MUCA_KERNEL_RESIDENT;
+    if (kern == MUCA_KERNEL_RESIDENT) p.mode = L <= 32 ? MODE_TBL_SMEM : MODE_TBL_L1;
+    else p.mode = MODE_STREAMED;
+    int tpb = c->opt_tpb;
+    if (tpb <= 0) {
+        if (p.mode == MODE_TBL_SMEM) tpb = 32;
+        else if (p.mode == MODE_TBL_L1) tpb = L == 64 ? 64 : 32;
+        else tpb = 32;
+    }
+    p.tpb = tpb;
+    return p;
+}
+
+size_t plan_smem(int L, const Plan& p) {
+    switch (L) {
+        case 8: return sweep_smem_bytes<8, MODE_TBL_SMEM>(p.tpb);
+        case 16: return sweep_smem_bytes<16, MODE_TBL_SMEM>(p.tpb);
+        case 32: return p.mode == MODE_TBL_SMEM ? sweep_smem_bytes<32, MODE_TBL_SMEM>(p.tpb)
+                        : p.mode == MODE_TBL_L1 ? sweep_smem_bytes<32, MODE_TBL_L1>(p.tpb)
+                                                : sweep_smem_bytes<32, MODE_STREAMED>(p.tpb);
+        case 64: return p.mode == MODE_STREAMED ? sweep_smem_bytes<64, MODE_STREAMED>(p.tpb)
+                                                : sweep_smem_bytes<64, MODE_TBL_L1>(p.tpb);
+        default: return p.mode == MODE_STREAMED ? sweep_smem_bytes<128, MODE_STREAMED>(p.tpb)
+                                                : sweep_smem_bytes<128, MODE_TBL_L1>(p.tpb);
+    }
+}
+
+int launch_sweep(muca_ctx* ctx, const SweepParams& prm, const Plan& p) {
+    switch (ctx->L) {
+        case 8: return launch_sweep_t<8, MODE_TBL_SMEM>(ctx, prm, p.tpb);
+        case 16: return launch_sweep_t<16, MODE_TBL_SMEM>(ctx, prm, p.tpb);
+        case 32:
+            if (p.mode == MODE_TBL_SMEM) return launch_sweep_t<32, MODE_TBL_SMEM>(ctx, prm, p.tpb);
+            if (p.mode == MODE_TBL_L1) return launch_sweep_t<32, MODE_TBL_L1>(ctx, prm, p.tpb);
+            return launch_sweep_t<32, MODE_STREAMED>(ctx, prm, p.tpb);
+        case 64:
+            if (p.mode == MODE_STREAMED) return launch_sweep_t<64, MODE_STREAMED>(ctx, prm, p.tpb);
+            return launch_sweep_t<64, MODE_TBL_L1>(ctx, prm, p.tpb);
+        case 128:
+            if (p.mode == MODE_STREAMED) return launch_sweep_t<128, MODE_STREAMED>(ctx, prm, p.tpb);
+            return launch_sweep_t<128, MODE_TBL_L1>(ctx, prm, p.tpb);
+    }
+    return fail(ctx, MUCA_EINVAL, "unsupported L=%d", ctx->L);
+}
+
+int create_common(muca_ctx** out, int L, int W, uint64_t seed, uint32_t walker_offset, void* d_ws, size_t ws_bytes,
+                  void* stream, bool own) {
+    if (!out) return MUCA_EINVAL;
+    *out = nullptr;
+    if (!valid_L(L) || W < 1 || (uint64_t)walker_offset + (uint64_t)W > 0xFFFFFFFFull) {
+        if (own && d_ws) cudaFree(d_ws);
+        return MUCA_EINVAL;
+    }
+    muca_ctx* ctx = new (std::nothrow) muca_ctx;
+    if (!ctx) return MUCA_ENOMEM;
+    ctx->L = L; ctx->N = L * L; ctx->W = W; ctx->n_bins = ctx->N + 1;
+    ctx->seed = seed; ctx->walker_offset = walker_offset;
+    ctx->stream = (cudaStream_t)stream;
+    ctx->own_workspace = own;
+    ctx->d_workspace = d_ws;
+    const Carve c = carve(L, W);
+    auto bail = [&](int code) { muca_destroy(ctx); return code; };
+    if (!d_ws || ws_bytes < c.total || ((uintptr_t)d_ws % ALIGN) != 0) return bail(MUCA_ENOMEM);
+    char* base = (char*)d_ws;
+    ctx->d_spins = (uint32_t*)(base + c.spins);
+    ctx->d_E = (int32_t*)(base + c.E);
+    ctx->d_table = (uint32_t*)(base + c.table);
+    ctx->d_H = (unsigned long long*)(base + c.H);
+    ctx->logw.assign(ctx->n_bins, 0.0);   // R2: omega == 0
+    ctx->H.assign(ctx->n_bins, 0);
+    if (cudaMallocHost((void**)&ctx->h_table, (size_t)ctx->n_bins * 8 * 4) != cudaSuccess ||
+        cudaMallocHost((void**)&ctx->h_H, (size_t)ctx->n_bins * 8) != cudaSuccess ||
+        cudaEventCreate(&ctx->ev0) != cudaSuccess || cudaEventCreate(&ctx->ev1) != cudaSuccess)
+        return bail(MUCA_ECUDA);
+    const int tpb = 128;
+    init_kernel<<<(W + tpb - 1) / tpb, tpb, 0, ctx->stream>>>(ctx->d_spins, ctx->d_E, L, W, walker_offset,
+                                                             (uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32));
+    if (cudaGetLastError() != cudaSuccess) return bail(MUCA_ECUDA);
+    if (cudaMemsetAsync(ctx->d_H, 0, (size_t)ctx->n_bins * 8, ctx->stream) != cudaSuccess) return bail(MUCA_ECUDA);
+    *out = ctx;
+    return MUCA_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* muca_version(void) { return "muca_b200 0.1 (sm_100a)"; }
+
+size_t muca_workspace_bytes(int L, int n_walkers) {
+    if (!valid_L(L) || n_walkers < 1) return 0;
+    return carve(L, n_walkers).total;
+}
+
+int muca_create(muca_ctx** out, int L, int n_walkers, uint64_t seed) {
+    if (!out) return MUCA_EINVAL;
+    *out = nullptr;
+    if (!valid_L(L) || n_walkers < 1) return MUCA_EINVAL;
+    const size_t bytes = carve(L, n_walkers).total;
+    void* ws = nullptr;
+    if (cudaMalloc(&ws, bytes) != cudaSuccess) return MUCA_ECUDA;
+    return create_common(out, L, n_walkers, seed, 0u, ws, bytes, nullptr, true);
+}
+
+int muca_create_in(muca_ctx** out, int L, int n_walkers, uint64_t seed, uint32_t walker_offset, void* d_workspace,
+                   size_t workspace_bytes, void* cuda_stream) {
+    return create_common(out, L, n_walkers, seed, walker_offset, d_workspace, workspace_bytes, cuda_stream, false);
+}
+
+void muca_destroy(muca_ctx* ctx) {
+    if (!ctx) return;
+    if (ctx->stream || ctx->d_workspace) cudaStreamSynchronize(ctx->stream);
+    if (ctx->h_table) cudaFreeHost(ctx->h_table);
+    if (ctx->h_H) cudaFreeHost(ctx->h_H);
+    if (ctx->ev0) cudaEventDestroy(ctx->ev0);
+    if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+    if (ctx->own_workspace && ctx->d_workspace) cudaFree(ctx->d_workspace);
+    delete ctx;
+}
+
+int muca_set_option(muca_ctx* ctx, int option, int value) {
+    if (!ctx) return MUCA_EINVAL;
+    if (option == MUCA_OPT_KERNEL) {
+        if (value < MUCA_KERNEL_AUTO || value > MUCA_KERNEL_STREAMED) return fail(ctx, MUCA_EINVAL, "bad kernel %d", value);
+        ctx->opt_kernel = value;
+        return MUCA_OK;
+    }
+    if (option == MUCA_OPT_THREADS_PER_BLOCK) {
+        if (value < 0 || value > 1024 || (value % 32) != 0) return fail(ctx, MUCA_EINVAL, "threads per block must be a multiple of 32 in [0, 1024]");
+        ctx->opt_tpb = value;
+        return MUCA_OK;
+    }
+    if (option == MUCA_OPT_MAX_SWEEPS_PER_LAUNCH) {
+        if (value < 0) return fail(ctx, MUCA_EINVAL, "max sweeps per launch must be >= 0");
+        ctx->opt_max_sweeps = value;
+        return MUCA_OK;
+    }
+    return fail(ctx, MUCA_EINVAL, "unknown option %d", option);
+}
+
+int muca_set_log_weights(muca_ctx* ctx, const double* logw, int n_bins) {
+    if (!ctx) return MUCA_EINVAL;
+    if (!logw || n_bins != ctx->n_bins) return fail(ctx, MUCA_EINVAL, "set_log_weights: n_bins must be %d", ctx->n_bins);
+    std::memcpy(ctx->logw.data(), logw, sizeof(double) * n_bins);
+    return MUCA_OK;
+}
+
+int muca_get_log_weights(muca_ctx* ctx, double* out, int n_bins) {
+    if (!ctx) return MUCA_EINVAL;
+    if (!out || n_bins != ctx->n_bins) return fail(ctx, MUCA_EINVAL, "get_log_weights: n_bins must be %d", ctx->n_bins);
+    std::memcpy(out, ctx->logw.data(), sizeof(double) * n_bins);
+    return MUCA_OK;
+}
+
+int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_out, int n_bins) {
+    if (!ctx) return MUCA_EINVAL;
+    if (n_bins != ctx->n_bins || therm_sweeps < 0 || sweeps < 0)
+        return fail(ctx, MUCA_EINVAL, "run_iteration: n_bins must be %d, sweeps >= 0", ctx->n_bins);
+    if (ctx->iteration == 0xFFFFFFFFu) return fail(ctx, MUCA_ERANGE, "iteration counter exhausted");
+    const Plan plan = make_plan(ctx);
+    {
+        int dev = 0, max_smem = 0;
+        CU(cudaGetDevice(&dev));
+        CU(cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+        if (plan_smem(ctx->L, plan) > (size_t)max_smem)
+            return fail(ctx, MUCA_EINVAL, "kernel variant needs %zu B of shared memory per block, device allows %d",
+                        plan_smem(ctx->L, plan), max_smem);
+    }
+    // a1: thresholds from omega (host, double)
+    std::vector<uint32_t> t5;
+    build_thresholds5(ctx->logw, t5);
+    expand_table8(t5, ctx->n_bins, ctx->h_table);
+    CU(cudaMemcpyAsync(ctx->d_table, ctx->h_table, (size_t)ctx->n_bins * 8 * 4, cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaMemsetAsync(ctx->d_H, 0, (size_t)ctx->n_bins * 8, ctx->stream));
+
+    // a2-a4: sweeps.  A block's uint32 bins must not overflow: tpb * measured sweeps * N < 2^32 per launch.
+    const uint64_t total = (uint64_t)therm_sweeps + (uint64_t)sweeps;
+    if (total > 0xFFFFFFFFull) return fail(ctx, MUCA_EINVAL, "too many sweeps");
+    uint64_t max_meas = 0xFFFFFFFFull / ((uint64_t)plan.tpb * (uint64_t)ctx->N);
+    if (max_meas < 1) max_meas = 1;
+    const uint64_t max_any = ctx->opt_max_sweeps > 0 ? (uint64_t)ctx->opt_max_sweeps : total + 1;
+    SweepParams prm;
+    prm.spins = ctx->d_spins; prm.E = ctx->d_E; prm.table = ctx->d_table; prm.H = ctx->d_H;
+    prm.W = ctx->W; prm.walker_offset = ctx->walker_offset;
+    prm.key0 = (uint32_t)(ctx->seed & 0xFFFFFFFFull); prm.key1 = (uint32_t)(ctx->seed >> 32);
+    prm.iteration = ctx->iteration; prm.therm = (uint32_t)therm_sweeps;
+    int launches = 0;
+    CU(cudaEventRecord(ctx->ev0, ctx->stream));
+    uint64_t s = 0;
+    while (s < total) {
+        uint64_t e = total;
+        const uint64_t meas_begin = s > (uint64_t)therm_sweeps ? s : (uint64_t)therm_sweeps;
+        if (e > meas_begin + max_meas) e = meas_begin + max_meas;
+        if (e > s + max_any) e = s + max_any;
+        prm.sweep_begin = (uint32_t)s; prm.sweep_end = (uint32_t)e;
+        const int rc = launch_sweep(ctx, prm, plan);
+        if (rc != MUCA_OK) return rc;
+        ++launches;
+        s = e;
+    }
+    CU(cudaEventRecord(ctx->ev1, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->h_H, ctx->d_H, (size_t)ctx->n_bins * 8, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
+    ctx->last_sweep_ms = ms;
+    ctx->last_launches = launches;
+    for (int j = 0; j < ctx->n_bins; ++j) ctx->H[j] = (uint64_t)ctx->h_H[j];
+    if (H_out) std::memcpy(H_out, ctx->H.data(), sizeof(uint64_t) * ctx->n_bins);
+    ctx->iteration += 1;
+    return MUCA_OK;
+}
+
+int muca_get_histogram(muca_ctx* ctx, uint64_t* H_out, int n_bins) {
+    if (!ctx) return MUCA_EINVAL;
+    if (!H_out || n_bins != ctx->n_bins) return fail(ctx, MUCA_EINVAL, "get_histogram: n_bins must be %d", ctx->n_bins);
+    std::memcpy(H_out, ctx->H.data(), sizeof(uint64_t) * n_bins);
+    return MUCA_OK;
+}
+
+int muca_update_weights_with(muca_ctx* ctx, const uint64_t* H_total, int n_bins) {
+    if (!ctx) return MUCA_EINVAL;
+    if (!H_total || n_bins != ctx->n_bins) return fail(ctx, MUCA_EINVAL, "update_weights: n_bins must be %d", ctx->n_bins);
+    // Eq. (4): omega <- omega - ln H on visited slots (R8: raw counts)
+    for (int j = 0; j < n_bins; ++j)
+        if (H_total[j] != 0) ctx->logw[j] -= std::log((double)H_total[j]);
+    return MUCA_OK;
+}
+
+int muca_update_weights(muca_ctx* ctx) {
+    if (!ctx) return MUCA_EINVAL;
+    return muca_update_weights_with(ctx, ctx->H.data(), ctx->n_bins);
+}
+
+int muca_get_energies(muca_ctx* ctx, int32_t* E_out, int n_walkers) {
+    if (!ctx) return MUCA_EINVAL;
+    if (!E_out || n_walkers != ctx->W) return fail(ctx, MUCA_EINVAL, "get_energies: n_walkers must be %d", ctx->W);
+    CU(cudaMemcpyAsync(E_out, ctx->d_E, sizeof(int32_t) * (size_t)ctx->W, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return MUCA_OK;
+}
+
+int muca_unpack_spins_device(muca_ctx* ctx, void* d_out, size_t n) {
+    if (!ctx) return MUCA_EINVAL;
+    if (!d_out || n != (size_t)ctx->W * ctx->N) return fail(ctx, MUCA_EINVAL, "unpack: n must be %zu", (size_t)ctx->W * ctx->N);
+    if (((uintptr_t)d_out % 16) != 0) return fail(ctx, MUCA_EINVAL, "unpack: device buffer must be 16-byte aligned");
+    const size_t threads = (size_t)ctx->W * (ctx->N / 32);
+    const int tpb = 256;
+    unpack_kernel<<<(unsigned)((threads + tpb - 1) / tpb), tpb, 0, ctx->stream>>>(ctx->d_spins, (int8_t*)d_out, ctx->L, ctx->W);
+    CU(cudaGetLastError());
+    return MUCA_OK;
+}
+
+int muca_get_spins(muca_ctx* ctx, int8_t* out, size_t n) {
+    if (!ctx) return MUCA_EINVAL;
+    if (!out || n != (size_t)ctx->W * ctx->N) return fail(ctx, MUCA_EINVAL, "get_spins: n must be %zu", (size_t)ctx->W * ctx->N);
+    void* d_tmp = nullptr;
+    CU(cudaMalloc(&d_tmp, n));
+    int rc = muca_unpack_spins_device(ctx, d_tmp, n);
+    if (rc == MUCA_OK) {
+        cudaError_t e = cudaMemcpyAsync(out, d_tmp, n, cudaMemcpyDeviceToHost, ctx->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+        if (e != cudaSuccess) rc = fail(ctx, MUCA_ECUDA, "get_spins copy failed: %s", cudaGetErrorString(e));
+    }
+    cudaFree(d_tmp);
+    return rc;
+}
+
+int muca_set_spins(muca_ctx* ctx, const int8_t* spins, size_t n) {
+    if (!ctx) return MUCA_EINVAL;
+    if (!spins || n != (size_t)ctx->W * ctx->N) return fail(ctx, MUCA_EINVAL, "set_spins: n must be %zu", (size_t)ctx->W * ctx->N);
+    void* d_tmp = nullptr;
+    CU(cudaMalloc(&d_tmp, n));
+    int rc = MUCA_OK;
+    cudaError_t e = cudaMemcpyAsync(d_tmp, spins, n, cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) {
+        const size_t threads = (size_t)ctx->W * (ctx->N / 32);
+        const int tpb = 256;
+        pack_kernel<<<(unsigned)((threads + tpb - 1) / tpb), tpb, 0, ctx->stream>>>((const int8_t*)d_tmp, ctx->d_spins, ctx->L, ctx->W);
+        energy_kernel<<<(ctx->W + 127) / 128, 128, 0, ctx->stream>>>(ctx->d_spins, ctx->d_E, ctx->L, ctx->W);
+        e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    }
+    if (e != cudaSuccess) rc = fail(ctx, MUCA_ECUDA, "set_spins failed: %s", cudaGetErrorString(e));
+    cudaFree(d_tmp);
+    return rc;
+}
+
+int muca_get_thresholds(muca_ctx* ctx, uint32_t* out, size_t n) {
+    if (!ctx) return MUCA_EINVAL;
+    if (!out || n != (size_t)ctx->n_bins * 5) return fail(ctx, MUCA_EINVAL, "get_thresholds: n must be %zu", (size_t)ctx->n_bins * 5);
+    std::vector<uint32_t> t5;
+    build_thresholds5(ctx->logw, t5);
+    std::memcpy(out, t5.data(), sizeof(uint32_t) * n);
+    return MUCA_OK;
+}
+
+int muca_get_iteration(muca_ctx* ctx, uint32_t* n_out) {
+    if (!ctx || !n_out) return MUCA_EINVAL;
+    *n_out = ctx->iteration;
+    return MUCA_OK;
+}
+
+int muca_set_iteration(muca_ctx* ctx, uint32_t n) {
+    if (!ctx) return MUCA_EINVAL;
+    ctx->iteration = n;
+    return MUCA_OK;
+}
+
+int muca_last_sweep_ms(muca_ctx* ctx, double* ms_out, int* launches_out) {
+    if (!ctx) return MUCA_EINVAL;
+    if (ms_out) *ms_out = ctx->last_sweep_ms;
+    if (launches_out) *launches_out = ctx->last_launches;
+    return MUCA_OK;
+}
+
+const char* muca_last_error(const muca_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+int muca_debug_philox(const uint32_t* ctr, const uint32_t* key, uint32_t* out, int n) {
+    if (!ctr || !key || !out || n < 1) return MUCA_EINVAL;
+    uint32_t *d_c = nullptr, *d_k = nullptr, *d_o = nullptr;
+    int rc = MUCA_OK;
+    if (cudaMalloc((void**)&d_c, 16 * (size_t)n) != cudaSuccess || cudaMalloc((void**)&d_k, 8 * (size_t)n) != cudaSuccess ||
+        cudaMalloc((void**)&d_o, 16 * (size_t)n) != cudaSuccess)
+        rc = MUCA_ECUDA;
+    if (rc == MUCA_OK && (cudaMemcpy(d_c, ctr, 16 * (size_t)n, cudaMemcpyHostToDevice) != cudaSuccess ||
+                          cudaMemcpy(d_k, key, 8 * (size_t)n, cudaMemcpyHostToDevice) != cudaSuccess))
+        rc = MUCA_ECUDA;
+    if (rc == MUCA_OK) {
+        philox_debug_kernel<<<(n + 127) / 128, 128>>>(d_c, d_k, d_o, n);
+        if (cudaGetLastError() != cudaSuccess || cudaMemcpy(out, d_o, 16 * (size_t)n, cudaMemcpyDeviceToHost) != cudaSuccess)
+            rc = MUCA_ECUDA;
+    }
+    cudaFree(d_c); cudaFree(d_k); cudaFree(d_o);
+    return rc;
+}
+
+}  // extern "C"

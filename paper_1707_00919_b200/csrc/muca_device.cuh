@@ -1,0 +1,463 @@
+// paper_1707_00919_b200/csrc/muca_device.cuh
+// Device code of libmuca_b200 (sm_100a): Philox4x32-10, the packed-lattice layout helpers, the
+// init / energy / pack / unpack kernels and the Metropolis sweep kernel (the hot path).
+// Citations: "PAPER.md:<line>" = /root/reference/PAPER.md, "R<n>" = DESIGN.md section 3.
+// Shares nothing with oracle/ (which is byte-per-spin, modulo arithmetic, no bit tricks).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace muca {
+
+// ------------------------------------------------------------------------------------------------
+// Philox4x32-10 ("counter-based RNG Philox", Ref. [41]; R4: 4x32, 10 rounds).
+// One round: (c0,c1,c2,c3) -> (hi(M1*c2)^c1^k0, lo(M1*c2), hi(M0*c0)^c3^k1, lo(M0*c0)); keys bumped by the
+// Weyl constants after every round.  In the sweep kernel only c3 (the walker id) differs between the
+// lanes of a warp, so ptxas moves the key schedule and the first round onto the uniform datapath.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              uint32_t k0, uint32_t k1, uint32_t (&out)[4]) {
+#pragma unroll
+    for (int round = 0; round < 10; ++round) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+        const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Packed lattice layout in HBM.  Spin bit 1 <-> spin -1.  "Typewriter word" t of a
+// walker holds sites 32t .. 32t+31 (site i = y*L + x at bit i & 31).
+//   L <  32 : word t of walker w at spins[t*W + w]                       (walker-interleaved words)
+//   L >= 32 : row y = WPR = L/32 consecutive words; row y of walker w at spins[(y*W + w)*WPR .. +WPR)
+//             (walker-interleaved ROWS: one 4/8/16-byte vector per thread, coalesced across the warp).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ size_t word_index(int L, int W, int w, int t) {
+    if (L < 32) return (size_t)t * W + w;
+    const int wpr = L >> 5;
+    const int y = t / wpr, k = t - y * wpr;
+    return ((size_t)y * W + w) * wpr + k;
+}
+
+// Row y of walker w as up to 4 words (bits 0..L-1 of the row, low word first); generic-L helper for the
+// one-off kernels.
+__device__ __forceinline__ void load_row(const uint32_t* spins, int L, int W, int w, int y,
+                                         uint32_t (&row)[4]) {
+    row[0] = row[1] = row[2] = row[3] = 0u;
+    if (L < 32) {
+        const int bit0 = y * L;
+        const uint32_t word = spins[word_index(L, W, w, bit0 >> 5)];
+        row[0] = (word >> (bit0 & 31)) & ((1u << L) - 1u);
+    } else {
+        const int wpr = L >> 5;
+        for (int k = 0; k < wpr; ++k) row[k] = spins[word_index(L, W, w, y * wpr + k)];
+    }
+}
+
+// Number of antiparallel bonds A of walker w; E = 2A - 2N (Eq. (5): every bond once,
+// -1 if parallel, +1 if antiparallel), slot j = (E + 2N)/4 = A/2.
+__device__ int antiparallel_bonds(const uint32_t* spins, int L, int W, int w) {
+    int A = 0;
+    uint32_t first[4], cur[4], nxt[4];
+    load_row(spins, L, W, w, 0, first);
+    for (int k = 0; k < 4; ++k) cur[k] = first[k];
+    const int wpr = L < 32 ? 1 : (L >> 5);
+    for (int y = 0; y < L; ++y) {
+        if (y + 1 < L) load_row(spins, L, W, w, y + 1, nxt);
+        else for (int k = 0; k < 4; ++k) nxt[k] = first[k];
+        for (int k = 0; k < wpr; ++k) {
+            uint32_t right;  // right neighbour of every site of word k (periodic in the row)
+            if (L < 32) right = (cur[0] >> 1) | ((cur[0] & 1u) << (L - 1));
+            else right = (cur[k] >> 1) | (cur[(k + 1) % wpr] << 31);
+            A += __popc(cur[k] ^ right) + __popc(cur[k] ^ nxt[k]);
+        }
+        for (int k = 0; k < 4; ++k) cur[k] = nxt[k];
+    }
+    return A;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a0 -- initial configuration (R1, R5): typewriter word t = 4q + m of global walker g is word m of
+// Philox(ctr = (q, 0, 0xFFFFFFFF, g), key).  One thread per walker.
+// ------------------------------------------------------------------------------------------------
+__global__ void init_kernel(uint32_t* spins, int32_t* E, int L, int W,
+                            uint32_t walker_offset, uint32_t key0, uint32_t key1) {
+    const int w = blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= W) return;
+    const int N = L * L, n_words = N >> 5;
+    for (int q = 0; 4 * q < n_words; ++q) {
+        uint32_t r[4];
+        philox4x32_10((uint32_t)q, 0u, 0xFFFFFFFFu, walker_offset + (uint32_t)w, key0, key1, r);
+        for (int m = 0; m < 4 && 4 * q + m < n_words; ++m) spins[word_index(L, W, w, 4 * q + m)] = r[m];
+    }
+    E[w] = 2 * antiparallel_bonds(spins, L, W, w) - 2 * N;
+}
+
+__global__ void energy_kernel(const uint32_t* __restrict__ spins, int32_t* __restrict__ E, int L, int W) {
+    const int w = blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= W) return;
+    E[w] = 2 * antiparallel_bonds(spins, L, W, w) - 2 * L * L;
+}
+
+// a6 -- read-back: one thread per (walker, typewriter word) writes 32 int8 spins, out[w*N + i] = 1 - 2*bit.
+__global__ void unpack_kernel(const uint32_t* __restrict__ spins, int8_t* __restrict__ out, int L, int W) {
+    const int n_words = (L * L) >> 5;
+    const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (size_t)W * n_words) return;
+    const int w = (int)(idx / n_words), t = (int)(idx - (size_t)w * n_words);
+    const uint32_t word = spins[word_index(L, W, w, t)];
+    uint4* dst = reinterpret_cast<uint4*>(out + idx * 32);  // 32-byte aligned: idx*32
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        uint32_t v[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const uint32_t nib = (word >> (16 * h + 4 * q)) & 0xFu;
+            // byte b = +1 (0x01) if bit clear, -1 (0xFF) if set
+            uint32_t bytes = 0x01010101u;
+#pragma unroll
+            for (int b = 0; b < 4; ++b)
+                if (nib & (1u << b)) bytes |= 0xFFu << (8 * b);
+            v[q] = bytes;
+        }
+        dst[h] = make_uint4(v[0], v[1], v[2], v[3]);
+    }
+}
+
+// inverse of unpack_kernel (muca_set_spins): in[w*N + i] < 0  <->  bit set.
+__global__ void pack_kernel(const int8_t* __restrict__ in, uint32_t* __restrict__ spins, int L, int W) {
+    const int n_words = (L * L) >> 5;
+    const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (size_t)W * n_words) return;
+    const int w = (int)(idx / n_words), t = (int)(idx - (size_t)w * n_words);
+    const int8_t* src = in + idx * 32;
+    uint32_t word = 0u;
+    for (int b = 0; b < 32; ++b) word |= (src[b] < 0 ? 1u : 0u) << b;
+    spins[word_index(L, W, w, t)] = word;
+}
+
+__global__ void philox_debug_kernel(const uint32_t* __restrict__ ctr, const uint32_t* __restrict__ key,
+                                    uint32_t* __restrict__ out, int n) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    uint32_t r[4];
+    philox4x32_10(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3], key[2 * i], key[2 * i + 1], r);
+    for (int m = 0; m < 4; ++m) out[4 * i + m] = r[m];
+}
+
+// ------------------------------------------------------------------------------------------------
+// a2/a3/a4 -- the sweep kernel.
+//
+// Device threshold table "T8" (built on the host from omega, muca.cu): row j holds 8 words indexed by
+//   f = 4*hi + 2*lo + g,   n3 = lo + 2*hi = antiparallel count over {up, down, right},  g = [left antiparallel],
+//   T8[j][f] = thresh[j][a = n3 + g]     (PAPER.md:109 acceptance, R6/R7 integer form).
+// The left neighbour is the site visited just before (typewriter order, R3), so g = hl ^ D where hl is the
+// static bit (old left value) and D says whether the previous site flipped: the lookup address is
+// (row + 4*f_static) ^ (D << 2) -- one XOR on the serial chain instead of a recount.
+//
+// Variants (template MODE):
+//   0  TBL_SMEM   table AND histogram interleaved in shared memory (row stride 40 B: 8 thresholds, 1 bin, pad),
+//                 lattices resident in shared memory                     (L <= 32)
+//   1  TBL_L1     table read from global through L1 (32 B rows), histogram + lattices in shared memory (L = 64)
+//   2  STREAMED   table through L1, histogram in shared memory, lattice rows streamed from HBM with a
+//                 three-row register window and one-row-ahead prefetch    (L = 128; any L >= 32)
+// ------------------------------------------------------------------------------------------------
+struct SweepParams {
+    uint32_t* spins;            // packed lattices (layout above)
+    int32_t* E;                 // per-walker energy
+    const uint32_t* table;      // T8, (N+1)*8 words, global
+    unsigned long long* H;      // global histogram, N+1 bins
+    int W;                      // walkers in this context
+    uint32_t walker_offset;     // global id of walker 0 (R16)
+    uint32_t key0, key1;        // Philox key = seed split low/high (R4)
+    uint32_t iteration;         // n (R4: ctr.z)
+    uint32_t sweep_begin;       // first sweep index of this launch (ctr.y)
+    uint32_t sweep_end;         // one past the last
+    uint32_t therm;             // sweeps with index < therm are not recorded
+};
+
+enum { MODE_TBL_SMEM = 0, MODE_TBL_L1 = 1, MODE_STREAMED = 2 };
+
+template <int L>
+struct Geo {
+    static constexpr int N = L * L;
+    static constexpr int BINS = N + 1;
+    static constexpr int WPR = L >= 32 ? L / 32 : 1;   // words per row
+    static constexpr int BITS = L >= 32 ? 32 : L;      // valid bits per row word
+    static constexpr uint32_t MASK = L >= 32 ? 0xFFFFFFFFu : ((1u << (L & 31)) - 1u);
+};
+
+constexpr int ROW_SMEM_WORDS = 10;  // MODE 0 row: 8 thresholds + 1 histogram bin + 1 pad (stride 40 B, multiple of 8)
+constexpr int ROW_L1_WORDS = 8;     // MODE 1/2 row: 8 thresholds (32 B)
+
+// One typewriter pass over row y of one walker.  up/dn: rows above/below (current values), cur: the row,
+// updated in place.  o: byte offset of the walker's energy row in the table (= j * row stride), updated.
+template <int L, int MODE, bool MEAS>
+__device__ __forceinline__ void process_row(const uint32_t (&up)[Geo<L>::WPR], uint32_t (&cur)[Geo<L>::WPR],
+                                            const uint32_t (&dn)[Geo<L>::WPR], uint32_t& o,
+                                            const uint32_t ctr0_row, const uint32_t sweep, const uint32_t iteration,
+                                            const uint32_t walker, const uint32_t key0, const uint32_t key1,
+                                            const char* __restrict__ tbl_smem, const char* __restrict__ tbl_glob,
+                                            uint32_t* __restrict__ hist) {
+    using G = Geo<L>;
+    constexpr int WPR = G::WPR, BITS = G::BITS;
+    constexpr int RS = (MODE == MODE_TBL_SMEM ? ROW_SMEM_WORDS : ROW_L1_WORDS) * 4;  // row stride in bytes
+
+    // static bit planes from the values at row start
+    uint32_t lo[WPR], hi[WPR], hl[WPR];
+    uint32_t vuL = 0, vdL = 0, hrL = 0;
+#pragma unroll
+    for (int k = 0; k < WPR; ++k) {
+        const uint32_t c = cur[k];
+        uint32_t rw, lw;
+        if constexpr (L >= 32) {
+            rw = (c >> 1) | (cur[(k + 1) % WPR] << 31);          // right neighbours (old; last site patched below)
+            lw = (c << 1) | (cur[(k + WPR - 1) % WPR] >> 31);    // left neighbours (old)
+        } else {
+            rw = (c >> 1) | ((c & 1u) << (BITS - 1));
+            lw = ((c << 1) | (c >> (BITS - 1))) & G::MASK;
+        }
+        const uint32_t vu = c ^ up[k], vd = c ^ dn[k], hr = c ^ rw;
+        hl[k] = c ^ lw;
+        lo[k] = vu ^ vd ^ hr;
+        hi[k] = (vu & vd) | (vu & hr) | (vd & hr);
+        if (k == WPR - 1) { vuL = vu; vdL = vd; hrL = hr; }
+    }
+
+    bool D = false;  // did the previous site of this row flip?  (site 0: left neighbour is site L-1, not yet visited)
+#pragma unroll
+    for (int k = 0; k < WPR; ++k) {
+        uint32_t c = cur[k];
+#pragma unroll
+        for (int g4 = 0; g4 < BITS / 4; ++g4) {
+            uint32_t r[4];
+            philox4x32_10(ctr0_row + (uint32_t)(k * 8 + g4), sweep, iteration, walker, key0, key1, r);
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                const int x = g4 * 4 + b;
+                const uint32_t f = (((hi[k] >> x) & 1u) << 2) | (((lo[k] >> x) & 1u) << 1) | ((hl[k] >> x) & 1u);
+                const uint32_t fw = f ^ (D ? 1u : 0u);
+                uint32_t t;
+                if (MODE == MODE_TBL_SMEM) t = *reinterpret_cast<const uint32_t*>(tbl_smem + o + 4u * fw);
+                else t = __ldg(reinterpret_cast<const uint32_t*>(tbl_glob + o + 4u * fw));
+                D = r[b] <= t;                                              // R6/R7: accept iff r <= t
+                const int a = (int)(fw >> 1) + (int)(fw & 1u);              // antiparallel neighbours
+                if (D) {
+                    o += (uint32_t)(RS * (2 - a));                          // j <- j + 2 - a  (dE = 8 - 4a)
+                    c ^= 1u << x;
+                }
+                if (MEAS) {                                                 // H[j]++ after EVERY attempt
+                    if (MODE == MODE_TBL_SMEM)
+                        atomicAdd(reinterpret_cast<uint32_t*>(const_cast<char*>(tbl_smem) + o + 32u), 1u);
+                    else
+                        atomicAdd(hist + (o >> 5), 1u);
+                }
+                if (k == 0 && x == 0) {
+                    // the right neighbour of the LAST site of the row is site 0, which has just been decided
+                    if (D) {
+                        hrL ^= 1u << (BITS - 1);
+                        lo[WPR - 1] = vuL ^ vdL ^ hrL;
+                        hi[WPR - 1] = (vuL & vdL) | (vuL & hrL) | (vdL & hrL);
+                    }
+                }
+            }
+        }
+        cur[k] = c;
+    }
+}
+
+template <int WPR> struct RowVec;
+template <> struct RowVec<1> { using type = uint32_t; };
+template <> struct RowVec<2> { using type = uint2; };
+template <> struct RowVec<4> { using type = uint4; };
+
+template <int WPR>
+__device__ __forceinline__ void ld_row(const uint32_t* p, uint32_t (&r)[WPR]) {
+    const typename RowVec<WPR>::type v = *reinterpret_cast<const typename RowVec<WPR>::type*>(p);
+    const uint32_t* s = reinterpret_cast<const uint32_t*>(&v);
+#pragma unroll
+    for (int k = 0; k < WPR; ++k) r[k] = s[k];
+}
+template <int WPR>
+__device__ __forceinline__ void st_row(uint32_t* p, const uint32_t (&r)[WPR]) {
+    typename RowVec<WPR>::type v;
+    uint32_t* s = reinterpret_cast<uint32_t*>(&v);
+#pragma unroll
+    for (int k = 0; k < WPR; ++k) s[k] = r[k];
+    *reinterpret_cast<typename RowVec<WPR>::type*>(p) = v;
+}
+
+// shared-memory footprint of one block (bytes)
+template <int L, int MODE>
+__host__ __device__ constexpr size_t sweep_smem_bytes(int tpb) {
+    using G = Geo<L>;
+    const size_t tbl = MODE == MODE_TBL_SMEM ? (size_t)G::BINS * ROW_SMEM_WORDS * 4 : (size_t)G::BINS * 4;
+    const size_t tbl_al = (tbl + 15) & ~(size_t)15;
+    const size_t lat = MODE == MODE_STREAMED ? 0 : (size_t)L * G::WPR * 4 * tpb;
+    return tbl_al + lat;
+}
+
+template <int L, int MODE, bool MEAS>
+__device__ __forceinline__ void resident_sweeps(uint32_t* __restrict__ lat, const int tpb, uint32_t& o,
+                                                const uint32_t s0, const uint32_t s1, const SweepParams& prm,
+                                                const uint32_t walker, const char* tbl_smem, const char* tbl_glob,
+                                                uint32_t* hist) {
+    using G = Geo<L>;
+    constexpr int WPR = G::WPR;
+#pragma unroll 1
+    for (uint32_t s = s0; s < s1; ++s) {
+#pragma unroll 1
+        for (int y = 0; y < L; ++y) {
+            const int ym = (y + L - 1) & (L - 1), yp = (y + 1) & (L - 1);
+            uint32_t up[WPR], cur[WPR], dn[WPR];
+#pragma unroll
+            for (int k = 0; k < WPR; ++k) {
+                up[k] = lat[(ym * WPR + k) * tpb];
+                cur[k] = lat[(y * WPR + k) * tpb];
+                dn[k] = lat[(yp * WPR + k) * tpb];
+            }
+            process_row<L, MODE, MEAS>(up, cur, dn, o, (uint32_t)(y * (L / 4)), s, prm.iteration, walker, prm.key0,
+                                       prm.key1, tbl_smem, tbl_glob, hist);
+#pragma unroll
+            for (int k = 0; k < WPR; ++k) lat[(y * WPR + k) * tpb] = cur[k];
+        }
+    }
+}
+
+template <int L, bool MEAS>
+__device__ __forceinline__ void streamed_sweeps(uint32_t* __restrict__ rows, const size_t row_stride, uint32_t& o,
+                                                const uint32_t s0, const uint32_t s1, const SweepParams& prm,
+                                                const uint32_t walker, const char* tbl_glob, uint32_t* hist) {
+    using G = Geo<L>;
+    constexpr int WPR = G::WPR;
+#pragma unroll 1
+    for (uint32_t s = s0; s < s1; ++s) {
+        uint32_t first[WPR] = {}, up[WPR], cur[WPR], dn[WPR], pre[WPR] = {};
+        ld_row<WPR>(rows + (size_t)(L - 1) * row_stride, up);   // row L-1, value of the previous sweep
+        ld_row<WPR>(rows, cur);
+        ld_row<WPR>(rows + row_stride, dn);
+#pragma unroll 1
+        for (int y = 0; y < L; ++y) {
+            if (y + 2 < L) ld_row<WPR>(rows + (size_t)(y + 2) * row_stride, pre);   // prefetch one row ahead
+            if (y == L - 1) {
+#pragma unroll
+                for (int k = 0; k < WPR; ++k) dn[k] = first[k];                     // row 0, already updated
+            }
+            process_row<L, MODE_STREAMED, MEAS>(up, cur, dn, o, (uint32_t)(y * (L / 4)), s, prm.iteration, walker,
+                                                prm.key0, prm.key1, nullptr, tbl_glob, hist);
+            st_row<WPR>(rows + (size_t)y * row_stride, cur);
+#pragma unroll
+            for (int k = 0; k < WPR; ++k) {
+                if (y == 0) first[k] = cur[k];
+                up[k] = cur[k];
+                cur[k] = dn[k];
+                dn[k] = pre[k];
+            }
+        }
+    }
+}
+
+template <int L, int MODE>
+__global__ void sweep_kernel(const SweepParams prm) {
+    using G = Geo<L>;
+    constexpr int WPR = G::WPR, N = G::N, BINS = G::BINS;
+    constexpr int RSW = MODE == MODE_TBL_SMEM ? ROW_SMEM_WORDS : ROW_L1_WORDS;
+    extern __shared__ __align__(16) uint32_t smem[];
+    const int tid = threadIdx.x, tpb = blockDim.x;
+    const int w = blockIdx.x * tpb + tid;
+    const bool active = w < prm.W;
+
+    // ---- shared memory: [table+bins | bins] [lattices]
+    constexpr size_t TBL_WORDS = MODE == MODE_TBL_SMEM ? (size_t)BINS * ROW_SMEM_WORDS : (size_t)BINS;
+    constexpr size_t TBL_WORDS_AL = (TBL_WORDS + 3) & ~(size_t)3;
+    uint32_t* const tbl_s = smem;
+    uint32_t* const lat = smem + TBL_WORDS_AL + tid;   // this thread's column: lat[r * tpb]
+    if (MODE == MODE_TBL_SMEM) {
+        for (int idx = tid; idx < BINS * ROW_SMEM_WORDS; idx += tpb) {
+            const int j = idx / ROW_SMEM_WORDS, e = idx - j * ROW_SMEM_WORDS;
+            tbl_s[idx] = e < 8 ? prm.table[j * 8 + e] : 0u;   // e == 8: histogram bin, e == 9: pad
+        }
+    } else {
+        for (int idx = tid; idx < BINS; idx += tpb) tbl_s[idx] = 0u;
+    }
+
+    // ---- lattice into shared memory (unpacked to one word per row for L < 32)
+    if (MODE != MODE_STREAMED) {
+        if (active) {
+            if (L >= 32) {
+                for (int y = 0; y < L; ++y) {
+                    uint32_t r[WPR];
+                    ld_row<WPR>(prm.spins + ((size_t)y * prm.W + w) * WPR, r);
+#pragma unroll
+                    for (int k = 0; k < WPR; ++k) lat[(y * WPR + k) * tpb] = r[k];
+                }
+            } else {
+                constexpr int RPW = 32 / G::BITS;  // rows per packed word
+                for (int t = 0; t < N / 32; ++t) {
+                    const uint32_t word = prm.spins[(size_t)t * prm.W + w];
+#pragma unroll
+                    for (int q = 0; q < RPW; ++q) lat[(t * RPW + q) * tpb] = (word >> (q * G::BITS)) & G::MASK;
+                }
+            }
+        }
+    }
+    __syncthreads();
+
+    if (active) {
+        const int E = prm.E[w];
+        uint32_t o = (uint32_t)((E + 2 * N) >> 2) * (uint32_t)(RSW * 4);   // slot j = (E + 2N)/4
+        const uint32_t walker = prm.walker_offset + (uint32_t)w;
+        const char* tbl_smem = reinterpret_cast<const char*>(tbl_s);
+        const char* tbl_glob = reinterpret_cast<const char*>(prm.table);
+        const uint32_t s_th = prm.therm < prm.sweep_begin ? prm.sweep_begin
+                              : (prm.therm > prm.sweep_end ? prm.sweep_end : prm.therm);
+        if (MODE == MODE_STREAMED) {
+            uint32_t* rows = prm.spins + (size_t)w * WPR;
+            const size_t row_stride = (size_t)prm.W * WPR;
+            streamed_sweeps<L, false>(rows, row_stride, o, prm.sweep_begin, s_th, prm, walker, tbl_glob, tbl_s);
+            streamed_sweeps<L, true>(rows, row_stride, o, s_th, prm.sweep_end, prm, walker, tbl_glob, tbl_s);
+        } else {
+            resident_sweeps<L, MODE, false>(lat, tpb, o, prm.sweep_begin, s_th, prm, walker, tbl_smem, tbl_glob, tbl_s);
+            resident_sweeps<L, MODE, true>(lat, tpb, o, s_th, prm.sweep_end, prm, walker, tbl_smem, tbl_glob, tbl_s);
+        }
+        prm.E[w] = (int)(o / (uint32_t)(RSW * 4)) * 4 - 2 * N;
+
+        if (MODE != MODE_STREAMED) {
+            if (L >= 32) {
+                for (int y = 0; y < L; ++y) {
+                    uint32_t r[WPR];
+#pragma unroll
+                    for (int k = 0; k < WPR; ++k) r[k] = lat[(y * WPR + k) * tpb];
+                    st_row<WPR>(prm.spins + ((size_t)y * prm.W + w) * WPR, r);
+                }
+            } else {
+                constexpr int RPW = 32 / G::BITS;
+                for (int t = 0; t < N / 32; ++t) {
+                    uint32_t word = 0u;
+#pragma unroll
+                    for (int q = 0; q < RPW; ++q) word |= lat[(t * RPW + q) * tpb] << (q * G::BITS);
+                    prm.spins[(size_t)t * prm.W + w] = word;
+                }
+            }
+        }
+    }
+    __syncthreads();
+
+    // ---- a4: merge the block's bins into the global uint64 histogram
+    if (prm.sweep_end > prm.therm) {
+        for (int j = tid; j < BINS; j += tpb) {
+            const uint32_t v = MODE == MODE_TBL_SMEM ? tbl_s[j * ROW_SMEM_WORDS + 8] : tbl_s[j];
+            if (v) atomicAdd(prm.H + j, (unsigned long long)v);
+        }
+    }
+}
+
+}  // namespace muca

@@ -1,0 +1,231 @@
+"""GPU parity: libmuca_b200 (CUDA, through the C ABI) against the CPU oracle, element by element.
+
+Bars (BASELINE.json north_star): bit-exact H, per-walker E, final spins, thresholds; omega within 1e-12
+absolute.  All inputs are seeded and synthetic (paper_1707_00919_b200/workloads.py).
+"""
+import numpy as np
+import pytest
+
+import muca_oracle as mo
+import paper_1707_00919_b200 as mb
+from paper_1707_00919_b200 import binding as B
+from paper_1707_00919_b200.workloads import CONFIGS, EXTRA_SEEDS, PRIMARY_SEED
+
+pytestmark = pytest.mark.gpu
+LOGW_TOL = 1e-12   # north_star: "double log-weights must agree within 1e-12 absolute"
+
+
+def energy_numpy(spins):
+    """E = -sum_<ij> s_i s_j on the periodic lattice, written with numpy rolls (independent of both sides)."""
+    s = spins.astype(np.int32)
+    return -(s * np.roll(s, -1, axis=2)).sum(axis=(1, 2)) - (s * np.roll(s, -1, axis=1)).sum(axis=(1, 2))
+
+
+def compare_state(g, o, tag=""):
+    Eg, Eo = g.get_energies(), o.get_energies()
+    assert np.array_equal(Eg, Eo), f"{tag}: energies differ at walkers {np.nonzero(Eg != Eo)[0][:8]}"
+    sg, so = g.get_spins(), o.get_spins()
+    assert sg.shape == so.shape
+    if not np.array_equal(sg, so):
+        bad = np.nonzero((sg != so).reshape(sg.shape[0], -1).any(axis=1))[0]
+        raise AssertionError(f"{tag}: spins differ for walkers {bad[:8]} ({bad.size} of {sg.shape[0]})")
+    assert np.array_equal(energy_numpy(sg), Eg), f"{tag}: tracked E != recomputed E"
+
+
+def run_pair(L, W, seed, iterations, therm, sweeps, offset=0, options=(), threads=None, check_every=True):
+    """Free-running pair: both sides apply their own Eq. (4) update each iteration."""
+    threads = threads or mo.max_threads()
+    g = mb.Muca(L, W, seed, walker_offset=offset)
+    for k, v in options:
+        g.set_option(k, v)
+    o = mo.Oracle(L, W, seed, walker_offset=offset)
+    try:
+        compare_state(g, o, "init")
+        N = L * L
+        for it in range(iterations):
+            assert np.array_equal(g.get_thresholds(), mo.thresholds(o.get_log_weights())), f"it{it}: thresholds"
+            Hg = g.run_iteration(therm, sweeps)
+            Ho = o.run_iteration(therm, sweeps, n_threads=threads)
+            assert Hg.dtype == np.uint64 and int(Hg.sum()) == W * sweeps * N
+            assert np.array_equal(Hg, Ho), f"it{it}: H differs in slots {np.nonzero(Hg != Ho)[0][:8]}"
+            assert Hg[1] == 0 and Hg[N - 1] == 0                       # unreachable slots
+            if check_every or it == iterations - 1:
+                compare_state(g, o, f"it{it}")
+            g.update_weights()
+            o.update_weights()
+            assert np.max(np.abs(g.get_log_weights() - o.get_log_weights())) <= LOGW_TOL
+            assert g.iteration == o.iteration == it + 1
+    finally:
+        g.close()
+        o.close()
+
+
+# ---------------------------------------------------------------------------------------------------
+def test_device_philox_matches_oracle_philox():
+    rng = np.random.default_rng(1)
+    ctr = rng.integers(0, 2 ** 32, size=(4096, 4), dtype=np.uint64).astype(np.uint32)
+    key = rng.integers(0, 2 ** 32, size=(4096, 2), dtype=np.uint64).astype(np.uint32)
+    ctr[:4] = [[0, 0, 0, 0], [0xFFFFFFFF] * 4, [255, 549, 14, 16383], [3, 0, 0xFFFFFFFF, 77]]
+    got = mb.debug_philox(ctr, key)
+    for i in list(range(64)) + [1000, 4095]:
+        assert np.array_equal(got[i], mo.philox4x32_10(ctr[i], key[i])), i
+
+
+@pytest.mark.parametrize("L", [8, 16, 32, 64, 128])
+@pytest.mark.parametrize("W,offset", [(1, 0), (37, 5), (160, 1000)])
+def test_init_matches_oracle(L, W, offset):
+    for seed in (PRIMARY_SEED,) + EXTRA_SEEDS[1:]:
+        g, o = mb.Muca(L, W, seed, walker_offset=offset), mo.Oracle(L, W, seed, walker_offset=offset)
+        compare_state(g, o, f"L{L} W{W}")
+        assert np.all(g.get_log_weights() == 0.0) and g.iteration == 0
+        g.close(); o.close()
+
+
+def test_thresholds_bit_exact_for_rough_weights():
+    rng = np.random.default_rng(3)
+    g = mb.Muca(16, 32, 1)
+    logw = np.cumsum(rng.normal(0, 2.0, g.n_bins))
+    logw[40] = logw[38]
+    logw[100] = logw[98] - 40.0
+    g.set_log_weights(logw)
+    assert np.array_equal(g.get_log_weights(), logw)
+    assert np.array_equal(g.get_thresholds(), mo.thresholds(logw))
+    g.close()
+
+
+# config 1 in full, all three seeds
+@pytest.mark.parametrize("seed", (PRIMARY_SEED,) + EXTRA_SEEDS)
+def test_config1_L8_full(seed):
+    c = CONFIGS[0]
+    run_pair(c.L, c.n_walkers, seed, c.iterations, c.therm_sweeps, c.sweeps)
+
+
+# config 2 in full (2.8e9 attempts on the oracle: tens of seconds on a few cores)
+def test_config2_L16_full():
+    c = CONFIGS[1]
+    run_pair(c.L, c.n_walkers, c.seed, c.iterations, c.therm_sweeps, c.sweeps, check_every=False)
+
+
+# configs 3-5 at reduced walker count / sweeps, several tiles and a ragged tail, default launch configuration
+@pytest.mark.parametrize("L,W,iters,therm,sweeps", [
+    (32, 32 * 5 + 7, 6, 5, 40),
+    (64, 64 * 2 + 19, 4, 3, 12),
+    (128, 32 * 2 + 9, 3, 2, 5),
+])
+def test_configs345_reduced(L, W, iters, therm, sweeps):
+    for seed in (PRIMARY_SEED, EXTRA_SEEDS[1]):
+        run_pair(L, W, seed, iters, therm, sweeps, offset=11)
+
+
+# every kernel variant / block size must give the same chains
+@pytest.mark.parametrize("L,kernel,tpb", [
+    (8, B.MUCA_KERNEL_RESIDENT, 64), (16, B.MUCA_KERNEL_RESIDENT, 128),
+    (32, B.MUCA_KERNEL_RESIDENT, 64), (32, B.MUCA_KERNEL_RESIDENT, 128), (32, B.MUCA_KERNEL_STREAMED, 32),
+    (32, B.MUCA_KERNEL_STREAMED, 96),
+    (64, B.MUCA_KERNEL_RESIDENT, 32), (64, B.MUCA_KERNEL_RESIDENT, 224), (64, B.MUCA_KERNEL_STREAMED, 64),
+    (128, B.MUCA_KERNEL_RESIDENT, 32), (128, B.MUCA_KERNEL_STREAMED, 64),
+])
+def test_kernel_variants(L, kernel, tpb):
+    W = 2 * tpb + 13
+    sweeps = {8: 30, 16: 20, 32: 10, 64: 5, 128: 3}[L]
+    run_pair(L, W, PRIMARY_SEED, 3, 2, sweeps,
+             options=((B.MUCA_OPT_KERNEL, kernel), (B.MUCA_OPT_THREADS_PER_BLOCK, tpb)))
+
+
+def test_split_launches_give_the_same_iteration():
+    # an iteration split into several launches (the uint32-bin overflow guard) is the same Markov chain
+    run_pair(32, 70, PRIMARY_SEED, 3, 3, 9, options=((B.MUCA_OPT_MAX_SWEEPS_PER_LAUNCH, 2),))
+    run_pair(128, 40, PRIMARY_SEED, 2, 1, 4, options=((B.MUCA_OPT_MAX_SWEEPS_PER_LAUNCH, 1),))
+
+
+def test_edge_cases_zero_sweeps_and_single_walker():
+    g, o = mb.Muca(16, 1, 5), mo.Oracle(16, 1, 5)
+    H = g.run_iteration(0, 0)
+    assert H.sum() == 0 and g.iteration == 1
+    o.run_iteration(0, 0)
+    compare_state(g, o)
+    g.update_weights()
+    assert np.all(g.get_log_weights() == 0.0)                 # H == 0 everywhere: omega unchanged (R8)
+    Hg, Ho = g.run_iteration(3, 0), o.run_iteration(3, 0)     # thermalisation only: nothing recorded
+    assert Hg.sum() == 0 and np.array_equal(Hg, Ho)
+    compare_state(g, o)
+    Hg, Ho = g.run_iteration(0, 4), o.run_iteration(0, 4)
+    assert np.array_equal(Hg, Ho) and Hg.sum() == 4 * 256
+    compare_state(g, o)
+    g.close(); o.close()
+
+
+@pytest.mark.parametrize("L", [8, 32, 64])
+def test_degenerate_configurations_and_canonical_weights(L):
+    # ground states (slot 0), antiferromagnetic ceiling (slot N), stripes; omega = -beta*E exercises genuine
+    # rejections at the edges of the table (moves to unreachable / out-of-range slots never occur)
+    N, W = L * L, 48
+    yy, xx = np.mgrid[0:L, 0:L]
+    pats = [np.ones((L, L)), -np.ones((L, L)), 1 - 2 * ((xx + yy) % 2), 1 - 2 * (yy % 2), 1 - 2 * (xx % 2)]
+    spins = np.stack([pats[w % len(pats)] for w in range(W)]).astype(np.int8)
+    E_axis = -2 * N + 4 * np.arange(N + 1)
+    for beta in (0.0, 0.4, -0.3):
+        g, o = mb.Muca(L, W, 99), mo.Oracle(L, W, 99)
+        g.set_spins(spins); o.set_spins(spins)
+        compare_state(g, o, "set_spins")
+        assert g.get_energies()[0] == -2 * N and g.get_energies()[2] == 2 * N
+        g.set_log_weights(-beta * E_axis); o.set_log_weights(-beta * E_axis)
+        for it in range(2):
+            Hg, Ho = g.run_iteration(1, 6), o.run_iteration(1, 6, n_threads=mo.max_threads())
+            assert np.array_equal(Hg, Ho)
+            compare_state(g, o, f"beta{beta} it{it}")
+        g.close(); o.close()
+
+
+def test_injected_weights_mode():
+    # the harness may inject the oracle's omega each iteration (muca_set_log_weights) instead of muca_update_weights
+    L, W = 32, 96
+    g, o = mb.Muca(L, W, 7), mo.Oracle(L, W, 7)
+    for it in range(4):
+        g.set_log_weights(o.get_log_weights())
+        Hg, Ho = g.run_iteration(2, 20), o.run_iteration(2, 20, n_threads=mo.max_threads())
+        assert np.array_equal(Hg, Ho)
+        o.update_weights()
+    compare_state(g, o)
+    g.close(); o.close()
+
+
+def test_sharded_walkers_are_independent_of_the_split():
+    # two contexts with walker_offset 0 / 50 reproduce one context of 120 walkers (R16); H adds up
+    L, seed = 16, PRIMARY_SEED
+    whole, a, b = mb.Muca(L, 120, seed), mb.Muca(L, 50, seed, 0), mb.Muca(L, 70, seed, 50)
+    for it in range(3):
+        Hw = whole.run_iteration(2, 15)
+        Hs = a.run_iteration(2, 15) + b.run_iteration(2, 15)
+        assert np.array_equal(Hw, Hs)
+        whole.update_weights(); a.update_weights_with(Hs); b.update_weights_with(Hs)
+        assert np.array_equal(whole.get_log_weights(), a.get_log_weights())
+    assert np.array_equal(whole.get_spins(), np.concatenate([a.get_spins(), b.get_spins()]))
+    assert np.array_equal(whole.get_energies(), np.concatenate([a.get_energies(), b.get_energies()]))
+    for x in (whole, a, b):
+        x.close()
+
+
+def test_unpack_device_matches_host_readback():
+    g = mb.Muca(64, 33, 3)
+    g.run_iteration(1, 2)
+    assert np.array_equal(g.unpack_spins_device().cpu().numpy(), g.get_spins())
+    g.close()
+
+
+def test_error_paths():
+    with pytest.raises(mb.MucaError):
+        mb.Muca(12, 32, 1)
+    with pytest.raises(mb.MucaError):
+        mb.Muca(32, 0, 1)
+    g = mb.Muca(8, 32, 1)
+    with pytest.raises(mb.MucaError):
+        g.set_log_weights(np.zeros(10))
+    with pytest.raises(mb.MucaError):
+        g.run_iteration(-1, 5)
+    with pytest.raises(mb.MucaError):
+        g.set_option(99, 1)
+    g.iteration = 0xFFFFFFFF
+    with pytest.raises(mb.MucaError):
+        g.run_iteration(1, 1)
+    g.close()
