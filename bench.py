@@ -1,0 +1,300 @@
+#!/usr/bin/env python
+"""bench.py -- spin-flip attempts/sec of the parallel-MUCA hot path on B200 (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path over one seeded synthetic job: create + initialise the walkers
+(a0), then `iterations` x [threshold build (a1), thermalisation + measured sweeps (a2, a3), histogram merge
+(a4), Eq. (4) weight update (a5)], then the unpack of the final configurations (a6).
+  value : whole-job flip attempts / device time, state resident in HBM (final spins unpacked on the device)
+  e2e   : same job through the C ABI with HOST buffers (thresholds H2D and H D2H every iteration, final
+          energies and spins D2H into host arrays inside the timed region)
+Workload at N=1: BASELINE.json configs[2] (L=32, 16384 walkers, 15 x (50 + 500) sweeps) -- the config the
+north_star target is quoted on.  N>1: every rank runs that many walkers (weak scaling) with global walker
+ids and one all-reduce of H per iteration.
+
+`--impl reference` times the CPU oracle (oracle/) on the host cores on a bounded walker sample of the same
+workload; there is no installable reference implementation (the paper's code is not available).
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+for p in (ROOT, os.path.join(ROOT, "oracle")):
+    if p not in sys.path:
+        sys.path.insert(0, p)
+
+import numpy as np  # noqa: E402
+
+METRIC = "spin-flip attempts/sec"
+UNIT = "flips/s"
+# algorithmic integer work per flip attempt and the issue roofline
+OPS_PER_FLIP = 20.0                 # thread-instructions: 8.5 Philox (16 IMAD.WIDE + 18 LOP3 per 4 sites) + 11.5 site update
+SM_COUNT, SCHED_PER_SM, LANES = 148, 4, 32
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="L32_w16384")
+    ap.add_argument("--ref-walkers", type=int, default=128, help="walker sample of the reference / cpu_baseline legs")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return json.load(f), "measured"
+    except Exception:
+        return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+# ------------------------------------------------------------------------------------------------ oracle legs
+def oracle_job(cfg, n_walkers, n_threads, iterations=None):
+    """The oracle, as it stands, on the first n_walkers walkers of the workload. Returns (flips, seconds)."""
+    import muca_oracle as mo
+    iters = cfg.iterations if iterations is None else iterations
+    t0 = time.perf_counter()
+    o = mo.Oracle(cfg.L, n_walkers, cfg.seed)
+    for _ in range(iters):
+        o.run_iteration(cfg.therm_sweeps, cfg.sweeps, n_threads=n_threads)
+        o.update_weights()
+    o.get_energies(); o.get_spins()
+    dt = time.perf_counter() - t0
+    o.close()
+    return iters * n_walkers * cfg.N * (cfg.therm_sweeps + cfg.sweeps), dt
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import muca_oracle as mo
+    cores = mo.max_threads()
+    W = args.ref_walkers
+    for _ in range(min(args.warmup, 1)):
+        oracle_job(cfg, W, cores, iterations=1)
+    flips = secs = 0.0
+    for _ in range(args.steps):
+        f, s = oracle_job(cfg, W, cores)
+        flips += f; secs += s
+    v = flips / secs
+    sample = f"first {W} of {cfg.n_walkers} walkers, full schedule {cfg.iterations} x ({cfg.therm_sweeps}+{cfg.sweeps}) sweeps"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+        "config": {"workload": cfg.name, "L": cfg.L, "n_walkers": W, "iterations": cfg.iterations,
+                   "therm_sweeps": cfg.therm_sweeps, "sweeps": cfg.sweeps, "note": "CPU oracle, OpenMP over walkers"},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+# ------------------------------------------------------------------------------------------------ clocks
+class ClockSampler(threading.Thread):
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.sm, self.reasons, self.max_mhz = index, False, [], set(), None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksEventReasonHwSlowdown: "hw_slowdown", nv.nvmlClocksEventReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksEventReasonSwThermalSlowdown: "sw_thermal_slowdown", nv.nvmlClocksEventReasonSwPowerCap: "sw_power_cap"} \
+            if hasattr(nv, "nvmlClocksEventReasonHwSlowdown") else \
+            {nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown", nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+             nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown", nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap"}
+        while not self.stop_flag:
+            try:
+                self.sm.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.02)
+
+    def result(self):
+        return {"sm_mhz": float(np.median(self.sm)) if self.sm else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.sm)}
+
+
+# ------------------------------------------------------------------------------------------------ our arm
+def run_ours(args, cfg):
+    import torch
+    import torch.distributed as dist
+    import paper_1707_00919_b200 as mb
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (libmuca_b200 has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    W = cfg.n_walkers                      # per rank: weak scaling
+    offset = rank * W
+    flips_per_step = mb.total_flips(cfg, W)
+    table_bytes = cfg.n_bins * 8 * 4
+    hist_bytes = cfg.n_bins * 8
+
+    h_E = np.empty(W, dtype=np.int32)
+    h_spins_t = torch.empty((W, cfg.L, cfg.L), dtype=torch.int8).pin_memory()
+    h_spins = h_spins_t.numpy()
+    l2_flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    Hbuf = torch.zeros(cfg.n_bins, dtype=torch.int64, device=dev)
+
+    stats = {"sweep_ms": 0.0, "sweep_launches": 0, "launches": 0}
+
+    def job(e2e: bool, record: bool):
+        g = mb.Muca(cfg.L, W, cfg.seed, walker_offset=offset)                  # a0 (init kernel)
+        n_launch = 1
+        for _ in range(cfg.iterations):
+            H = g.run_iteration(cfg.therm_sweeps, cfg.sweeps)                  # a1-a4 (+ H2D table, D2H H)
+            ms, k = g.last_sweep_ms()
+            n_launch += k
+            if record:
+                stats["sweep_ms"] += ms; stats["sweep_launches"] += k
+            if world > 1:                                                      # the one exchange of the method
+                Hbuf.copy_(torch.from_numpy(H.astype(np.int64)))
+                dist.all_reduce(Hbuf)
+                g.update_weights_with(Hbuf.cpu().numpy().astype(np.uint64))    # a5
+            else:
+                g.update_weights()                                             # a5
+        if e2e:
+            g.get_energies(h_E)
+            g.get_spins(h_spins)                                               # a6: unpack kernel + D2H
+        else:
+            g.unpack_spins_device()                                            # a6: unpack kernel, stays in HBM
+        n_launch += 1
+        if record:
+            stats["launches"] += n_launch
+        g.close()
+
+    def timed(e2e: bool, steps: int, record: bool):
+        total_ms = 0.0
+        for _ in range(steps):
+            l2_flush.fill_(1)                                                  # flush L2 between timed steps
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            job(e2e, record)
+            e1.record()
+            torch.cuda.synchronize()
+            total_ms += e0.elapsed_time(e1)
+        return total_ms
+
+    for _ in range(max(args.warmup, 3)):
+        job(False, False)
+    job(True, False)
+
+    def bracket():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+
+    sampler = ClockSampler(local)
+    bracket()
+    sampler.start()
+    ms_dev = timed(False, args.steps, True)
+    bracket()
+    ms_e2e = timed(True, args.steps, False)
+    bracket()
+    sampler.stop_flag = True
+    sampler.join(timeout=1.0)
+
+    t = torch.tensor([ms_dev, ms_e2e], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_dev, ms_e2e = float(t[0]), float(t[1])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    pk, pk_kind = peaks()
+    f_max_hz = float(pk.get("sm_max_mhz", 1965.0)) * 1e6
+    value = world * flips_per_step * args.steps / (ms_dev * 1e-3)
+    e2e_v = world * flips_per_step * args.steps / (ms_e2e * 1e-3)
+    # dominant kernel: the sweep kernel (one launch per iteration)
+    flips_per_launch = mb.flips_per_iteration(cfg, W) * cfg.iterations * args.steps / max(stats["sweep_launches"], 1)
+    avg_launch_s = stats["sweep_ms"] * 1e-3 / max(stats["sweep_launches"], 1)
+    kern_flips_s = flips_per_launch / avg_launch_s
+    achieved = kern_flips_s * OPS_PER_FLIP / 1e12
+    peak = SM_COUNT * SCHED_PER_SM * LANES * f_max_hz / 1e12
+    roofline = {
+        "bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tinst/s (thread-instructions)", "frac": achieved / peak,
+        "traffic": None, "kernel": "muca::sweep_kernel", "kernel_flips_per_s": kern_flips_s,
+        "ops_per_flip": OPS_PER_FLIP, "avg_launch_ms": avg_launch_s * 1e3, "kernel_share_of_step": stats["sweep_ms"] / ms_dev,
+        "c_flip_cycles": W * f_max_hz / kern_flips_s,
+        "peak_source": f"148 SM x 4 schedulers x 32 lanes x sm_max_mhz ({pk_kind} MEASURED_PEAKS.json clock)",
+        "hbm": {"algorithmic_bytes_per_flip": 0.0 if cfg.L <= 64 else 0.25, "peak_gbs": pk.get("hbm_gbs"),
+                "note": "lattices are shared-memory resident for L <= 64; HBM traffic is KiB per launch"},
+    }
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_dev / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "int32", "data": "synthetic",
+        "config": {"workload": cfg.name, "L": cfg.L, "n_walkers_per_gpu": W, "iterations": cfg.iterations,
+                   "therm_sweeps": cfg.therm_sweeps, "sweeps": cfg.sweeps, "seed": cfg.seed,
+                   "flips_per_step_per_gpu": flips_per_step, "l2": "flushed between timed steps (256 MiB write)",
+                   "parallelism": f"walkers x{world}, one all-reduce(H) per iteration" if world > 1 else "1 GPU"},
+        "clocks": sampler.result(),
+        "e2e": {"value": e2e_v, "unit": UNIT,
+                "h2d_bytes_per_step": cfg.iterations * table_bytes,
+                "d2h_bytes_per_step": cfg.iterations * hist_bytes + h_E.nbytes + h_spins.nbytes,
+                "ms_per_step": ms_e2e / args.steps},
+        "gpu_launches": stats["launches"],
+        "roofline": roofline,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        import muca_oracle as mo
+        cores = mo.max_threads()
+        Wb = args.ref_walkers
+        f, s = oracle_job(cfg, Wb, cores, iterations=3)
+        out["cpu_baseline"] = {"value": f / s, "unit": UNIT, "cores": cores, "kind": "oracle",
+                               "sample": f"first {Wb} of {cfg.n_walkers} walkers, 3 of {cfg.iterations} iterations x "
+                                         f"({cfg.therm_sweeps}+{cfg.sweeps}) sweeps, OpenMP over walkers"}
+        f1, s1 = oracle_job(cfg, max(Wb // 8, 8), 1, iterations=1)
+        out["cpu_baseline"]["single_thread_value"] = f1 / s1
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    from paper_1707_00919_b200.workloads import by_name
+    cfg = by_name(args.config)
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_ours(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

@@ -181,8 +181,10 @@ class Muca:
         h = np.ascontiguousarray(H_total, dtype=np.uint64)
         self._check(self._lib.muca_update_weights_with(self._h, _p(h, C.c_uint64), h.size), "muca_update_weights_with")
 
-    def get_energies(self) -> np.ndarray:
-        out = np.empty(self.W, dtype=np.int32)
+    def get_energies(self, out: np.ndarray = None) -> np.ndarray:
+        if out is None:
+            out = np.empty(self.W, dtype=np.int32)
+        assert out.dtype == np.int32 and out.size == self.W and out.flags.c_contiguous
         self._check(self._lib.muca_get_energies(self._h, _p(out, C.c_int32), out.size), "muca_get_energies")
         return out
 

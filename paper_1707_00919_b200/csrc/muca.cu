@@ -27,6 +27,7 @@ struct muca_ctx {
     int32_t* d_E = nullptr;
     uint32_t* d_table = nullptr;
     unsigned long long* d_H = nullptr;
+    void* d_stage = nullptr;        // lazily allocated W*N bytes for muca_get_spins / muca_set_spins
     // host state
     std::vector<double> logw;       // omega, n_bins
     std::vector<uint64_t> H;        // last histogram
@@ -249,6 +250,7 @@ void muca_destroy(muca_ctx* ctx) {
     if (ctx->h_H) cudaFreeHost(ctx->h_H);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+    if (ctx->d_stage) cudaFree(ctx->d_stage);
     if (ctx->own_workspace && ctx->d_workspace) cudaFree(ctx->d_workspace);
     delete ctx;
 }
@@ -389,23 +391,21 @@ int muca_unpack_spins_device(muca_ctx* ctx, void* d_out, size_t n) {
 int muca_get_spins(muca_ctx* ctx, int8_t* out, size_t n) {
     if (!ctx) return MUCA_EINVAL;
     if (!out || n != (size_t)ctx->W * ctx->N) return fail(ctx, MUCA_EINVAL, "get_spins: n must be %zu", (size_t)ctx->W * ctx->N);
-    void* d_tmp = nullptr;
-    CU(cudaMalloc(&d_tmp, n));
-    int rc = muca_unpack_spins_device(ctx, d_tmp, n);
+    if (!ctx->d_stage) CU(cudaMalloc(&ctx->d_stage, n));
+    int rc = muca_unpack_spins_device(ctx, ctx->d_stage, n);
     if (rc == MUCA_OK) {
-        cudaError_t e = cudaMemcpyAsync(out, d_tmp, n, cudaMemcpyDeviceToHost, ctx->stream);
+        cudaError_t e = cudaMemcpyAsync(out, ctx->d_stage, n, cudaMemcpyDeviceToHost, ctx->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
         if (e != cudaSuccess) rc = fail(ctx, MUCA_ECUDA, "get_spins copy failed: %s", cudaGetErrorString(e));
     }
-    cudaFree(d_tmp);
     return rc;
 }
 
 int muca_set_spins(muca_ctx* ctx, const int8_t* spins, size_t n) {
     if (!ctx) return MUCA_EINVAL;
     if (!spins || n != (size_t)ctx->W * ctx->N) return fail(ctx, MUCA_EINVAL, "set_spins: n must be %zu", (size_t)ctx->W * ctx->N);
-    void* d_tmp = nullptr;
-    CU(cudaMalloc(&d_tmp, n));
+    if (!ctx->d_stage) CU(cudaMalloc(&ctx->d_stage, n));
+    void* d_tmp = ctx->d_stage;
     int rc = MUCA_OK;
     cudaError_t e = cudaMemcpyAsync(d_tmp, spins, n, cudaMemcpyHostToDevice, ctx->stream);
     if (e == cudaSuccess) {
@@ -417,7 +417,6 @@ int muca_set_spins(muca_ctx* ctx, const int8_t* spins, size_t n) {
         if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
     }
     if (e != cudaSuccess) rc = fail(ctx, MUCA_ECUDA, "set_spins failed: %s", cudaGetErrorString(e));
-    cudaFree(d_tmp);
     return rc;
 }
 

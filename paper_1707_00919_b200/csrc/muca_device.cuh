@@ -198,8 +198,109 @@ struct Geo {
 constexpr int ROW_SMEM_WORDS = 10;  // MODE 0 row: 8 thresholds + 1 histogram bin + 1 pad (stride 40 B, multiple of 8)
 constexpr int ROW_L1_WORDS = 8;     // MODE 1/2 row: 8 thresholds (32 B)
 
+// Four consecutive sites (one Philox call) of the shared-memory-table variant, written in PTX so that the
+// decision stays in a predicate along the serial chain (no SEL / 0-1 materialisation between sites):
+//   pD -> @pD xor (column f ^ 1) -> address -> ld.shared -> setp -> pD ...
+// o is the ABSOLUTE shared-memory address of the walker's table row.  (rp, tp) are the deviate and threshold
+// of the previous site: re-evaluating rp <= tp recreates the predicate that cannot cross an asm boundary.
+// t0: threshold used by the first site of the group (the row loop needs site 0's decision for the wrap patch).
+#define MUCA_SITE_PTX(FWOP, ROP, MOP, MEAS_LINE)                                   \
+    "shr.u32 f, " FWOP ", %16;\n\t"                                              \
+    "and.b32 f, f, 7;\n\t"                                                         \
+    "@pD xor.b32 f, f, 1;\n\t"                                                     \
+    "shl.b32 ad, f, 2;\n\t"                                                        \
+    "add.u32 ad, ad, %0;\n\t"                                                    \
+    "ld.shared.u32 t, [ad];\n\t"                                                   \
+    "prmt.b32 d, %14, %15, f;\n\t"                                       \
+    "sub.u32 oa, %0, d;\n\t"                                                     \
+    "add.u32 oa, oa, %17;\n\t"                                                  \
+    "setp.le.u32 pD, " ROP ", t;\n\t"                                              \
+    "@pD mov.u32 %0, oa;\n\t"                                                    \
+    "@pD xor.b32 %1, %1, " MOP ";\n\t" MEAS_LINE
+
+template <int Q, bool MEAS, uint32_t RS>
+__device__ __forceinline__ void site_group_smem(const uint32_t fw0, const uint32_t fw1, const uint32_t fw2,
+                                                const uint32_t fw3, uint32_t& o, uint32_t& c,
+                                                const uint32_t (&rnd)[4], uint32_t& rp, uint32_t& tp, uint32_t& t0) {
+    constexpr uint32_t LUT_LO = (RS * 0) | (RS * 1) << 8 | (RS * 1) << 16 | (RS * 2) << 24;
+    constexpr uint32_t LUT_HI = (RS * 2) | (RS * 3) << 8 | (RS * 3) << 16 | (RS * 4) << 24;
+    uint32_t t_first, t_last;
+    if (MEAS) {
+        asm volatile(
+            "{\n\t.reg .pred pD;\n\t.reg .b32 f, ad, d, oa, t;\n\t"
+            "setp.le.u32 pD, %12, %13;\n\t"
+            MUCA_SITE_PTX("%4", "%8", "%18", "red.shared.add.u32 [%0+32], 1;\n\t")
+            "mov.u32 %2, t;\n\t"
+            MUCA_SITE_PTX("%5", "%9", "%19", "red.shared.add.u32 [%0+32], 1;\n\t")
+            MUCA_SITE_PTX("%6", "%10", "%20", "red.shared.add.u32 [%0+32], 1;\n\t")
+            MUCA_SITE_PTX("%7", "%11", "%21", "red.shared.add.u32 [%0+32], 1;\n\t")
+            "mov.u32 %3, t;\n\t}"
+            : "+r"(o), "+r"(c), "=r"(t_first), "=r"(t_last)
+            : "r"(fw0), "r"(fw1), "r"(fw2), "r"(fw3), "r"(rnd[0]), "r"(rnd[1]),
+              "r"(rnd[2]), "r"(rnd[3]), "r"(rp), "r"(tp), "r"(LUT_LO), "r"(LUT_HI),
+              "n"(4 * Q), "n"(2 * RS), "n"(1u << (4 * Q)), "n"(1u << (4 * Q + 1)),
+              "n"(1u << (4 * Q + 2)), "n"(1u << (4 * Q + 3))
+            : "memory");
+    } else {
+        asm volatile(
+            "{\n\t.reg .pred pD;\n\t.reg .b32 f, ad, d, oa, t;\n\t"
+            "setp.le.u32 pD, %12, %13;\n\t"
+            MUCA_SITE_PTX("%4", "%8", "%18", "")
+            "mov.u32 %2, t;\n\t"
+            MUCA_SITE_PTX("%5", "%9", "%19", "")
+            MUCA_SITE_PTX("%6", "%10", "%20", "")
+            MUCA_SITE_PTX("%7", "%11", "%21", "")
+            "mov.u32 %3, t;\n\t}"
+            : "+r"(o), "+r"(c), "=r"(t_first), "=r"(t_last)
+            : "r"(fw0), "r"(fw1), "r"(fw2), "r"(fw3), "r"(rnd[0]), "r"(rnd[1]),
+              "r"(rnd[2]), "r"(rnd[3]), "r"(rp), "r"(tp), "r"(LUT_LO), "r"(LUT_HI),
+              "n"(4 * Q), "n"(2 * RS), "n"(1u << (4 * Q)), "n"(1u << (4 * Q + 1)),
+              "n"(1u << (4 * Q + 2)), "n"(1u << (4 * Q + 3)));
+    }
+    rp = rnd[3];
+    tp = t_last;
+    t0 = t_first;
+}
+
+template <int Q, int QN, int L, bool MEAS, uint32_t RS>
+struct GroupLoop {
+    // groups Q .. QN-1 of word k of a row (compile-time recursion: the shifts and flip masks are immediates)
+    static __device__ __forceinline__ void run(uint32_t (&FWk)[4], uint32_t* FWlast3, const uint32_t patch, const bool first_word,
+                                               uint32_t& o, uint32_t& c, uint32_t& rp, uint32_t& tp, const uint32_t ctr0,
+                                               const uint32_t sweep, const uint32_t iteration, const uint32_t walker,
+                                               const uint32_t key0, const uint32_t key1) {
+        uint32_t rnd[4], t0;
+        philox4x32_10(ctr0 + (uint32_t)Q, sweep, iteration, walker, key0, key1, rnd);
+        site_group_smem<Q, MEAS, RS>(FWk[0], FWk[1], FWk[2], FWk[3], o, c, rnd, rp, tp, t0);
+        if (Q == 0 && first_word) {
+            // the right neighbour of the LAST site of the row is site 0, which has just been decided
+            if (rnd[0] <= t0) *FWlast3 += patch;
+        }
+        GroupLoop<Q + 1, QN, L, MEAS, RS>::run(FWk, FWlast3, patch, first_word, o, c, rp, tp, ctr0, sweep, iteration, walker,
+                                               key0, key1);
+    }
+};
+template <int QN, int L, bool MEAS, uint32_t RS>
+struct GroupLoop<QN, QN, L, MEAS, RS> {
+    static __device__ __forceinline__ void run(uint32_t (&)[4], uint32_t*, const uint32_t, const bool, uint32_t&, uint32_t&,
+                                               uint32_t&, uint32_t&, const uint32_t, const uint32_t, const uint32_t,
+                                               const uint32_t, const uint32_t, const uint32_t) {}
+};
+
 // One typewriter pass over row y of one walker.  up/dn: rows above/below (current values), cur: the row,
 // updated in place.  o: byte offset of the walker's energy row in the table (= j * row stride), updated.
+//
+// Per row (bit-sliced, ~30 instructions for 32 sites): the three static planes
+//   lo, hi = the two bits of n3 = [up != s] + [down != s] + [right != s],   hl = [left(old) != s]
+// are interleaved into four "field words" FW[r] (r = x & 3): nibble q of FW[r] holds the table column
+// f = hl + 2*lo + 4*hi of site x = 4q + r, so the per-site extraction is one shift and one mask.
+// Per site the serial chain is  D(prev) -> f ^= D -> address -> LDS -> compare -> D:
+//   fw   = f ^ D                     D: previous site flipped, which toggles the [left != s] bit (column f ^ 1)
+//   t    = T8[row o][fw]             one 4-byte load (shared memory or L1)
+//   D    = r <= t                    R6/R7
+//   o   += D ? RS*(2 - a(fw)) : 0    RS*a(fw) comes from an 8-entry byte table in two registers (PRMT)
+//   s_x ^= D                         predicated XOR with an immediate
+//   H[row o] += 1                    shared-memory atomic, measured sweeps only
 template <int L, int MODE, bool MEAS>
 __device__ __forceinline__ void process_row(const uint32_t (&up)[Geo<L>::WPR], uint32_t (&cur)[Geo<L>::WPR],
                                             const uint32_t (&dn)[Geo<L>::WPR], uint32_t& o,
@@ -209,68 +310,84 @@ __device__ __forceinline__ void process_row(const uint32_t (&up)[Geo<L>::WPR], u
                                             uint32_t* __restrict__ hist) {
     using G = Geo<L>;
     constexpr int WPR = G::WPR, BITS = G::BITS;
-    constexpr int RS = (MODE == MODE_TBL_SMEM ? ROW_SMEM_WORDS : ROW_L1_WORDS) * 4;  // row stride in bytes
+    constexpr uint32_t RS = (MODE == MODE_TBL_SMEM ? ROW_SMEM_WORDS : ROW_L1_WORDS) * 4;  // row stride in bytes
+    // byte f of (LUT_HI:LUT_LO) = RS * a(f), a(f) = (f >> 1) + (f & 1) = antiparallel neighbours of column f
+    constexpr uint32_t LUT_LO = (RS * 0) | (RS * 1) << 8 | (RS * 1) << 16 | (RS * 2) << 24;
+    constexpr uint32_t LUT_HI = (RS * 2) | (RS * 3) << 8 | (RS * 3) << 16 | (RS * 4) << 24;
+    static_assert(RS * 4 < 256, "row stride must keep RS*a in a byte");
 
-    // static bit planes from the values at row start
-    uint32_t lo[WPR], hi[WPR], hl[WPR];
-    uint32_t vuL = 0, vdL = 0, hrL = 0;
+    uint32_t FW[WPR][4];
+    uint32_t patch = 0;   // added to FW[WPR-1][3] when site 0 flips: n3 of the LAST site changes by +-1
 #pragma unroll
     for (int k = 0; k < WPR; ++k) {
         const uint32_t c = cur[k];
         uint32_t rw, lw;
         if constexpr (L >= 32) {
-            rw = (c >> 1) | (cur[(k + 1) % WPR] << 31);          // right neighbours (old; last site patched below)
+            rw = (c >> 1) | (cur[(k + 1) % WPR] << 31);          // right neighbours (old; last site patched)
             lw = (c << 1) | (cur[(k + WPR - 1) % WPR] >> 31);    // left neighbours (old)
         } else {
             rw = (c >> 1) | ((c & 1u) << (BITS - 1));
             lw = ((c << 1) | (c >> (BITS - 1))) & G::MASK;
         }
         const uint32_t vu = c ^ up[k], vd = c ^ dn[k], hr = c ^ rw;
-        hl[k] = c ^ lw;
-        lo[k] = vu ^ vd ^ hr;
-        hi[k] = (vu & vd) | (vu & hr) | (vd & hr);
-        if (k == WPR - 1) { vuL = vu; vdL = vd; hrL = hr; }
+        const uint32_t hl = c ^ lw;
+        const uint32_t lo = vu ^ vd ^ hr;
+        const uint32_t hi = (vu & vd) | (vu & hr) | (vd & hr);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const uint32_t A = hl >> r;                                   // bit 4q+r -> 4q
+            const uint32_t B = r >= 1 ? lo >> (r - 1) : lo << 1;          //          -> 4q+1
+            const uint32_t C = r >= 2 ? hi >> (r - 2) : hi << (2 - r);    //          -> 4q+2
+            const uint32_t t1 = (A & 0x11111111u) | (B & ~0x11111111u);
+            FW[k][r] = (t1 & 0x33333333u) | (C & ~0x33333333u);           // bit 4q+3 is junk, masked at extraction
+        }
+        if (k == WPR - 1) {
+            constexpr int QL = BITS / 4 - 1;                              // nibble of the last site in FW[.][3]
+            const uint32_t hr_last = (hr >> (BITS - 1)) & 1u;
+            patch = (1u << (4 * QL + 1)) - (hr_last << (4 * QL + 2));     // +1 on n3 if the bond was parallel, else -1
+        }
     }
 
-    bool D = false;  // did the previous site of this row flip?  (site 0: left neighbour is site L-1, not yet visited)
+    if constexpr (MODE == MODE_TBL_SMEM) {
+        // o is the absolute shared-memory address of the walker's table row (see site_group_smem)
+        uint32_t rp = 1u, tp = 0u;   // "previous site did not flip": site 0's left neighbour is site L-1, not yet visited
 #pragma unroll
-    for (int k = 0; k < WPR; ++k) {
-        uint32_t c = cur[k];
+        for (int k = 0; k < WPR; ++k) {
+            uint32_t c = cur[k];
+            GroupLoop<0, BITS / 4, L, MEAS, RS>::run(FW[k], &FW[WPR - 1][3], patch, k == 0, o, c, rp, tp,
+                                                     ctr0_row + (uint32_t)(k * 8), sweep, iteration, walker, key0, key1);
+            cur[k] = c;
+        }
+    } else {
+        bool D = false;  // did the previous site of this row flip?
 #pragma unroll
-        for (int g4 = 0; g4 < BITS / 4; ++g4) {
-            uint32_t r[4];
-            philox4x32_10(ctr0_row + (uint32_t)(k * 8 + g4), sweep, iteration, walker, key0, key1, r);
+        for (int k = 0; k < WPR; ++k) {
+            uint32_t c = cur[k];
 #pragma unroll
-            for (int b = 0; b < 4; ++b) {
-                const int x = g4 * 4 + b;
-                const uint32_t f = (((hi[k] >> x) & 1u) << 2) | (((lo[k] >> x) & 1u) << 1) | ((hl[k] >> x) & 1u);
-                const uint32_t fw = f ^ (D ? 1u : 0u);
-                uint32_t t;
-                if (MODE == MODE_TBL_SMEM) t = *reinterpret_cast<const uint32_t*>(tbl_smem + o + 4u * fw);
-                else t = __ldg(reinterpret_cast<const uint32_t*>(tbl_glob + o + 4u * fw));
-                D = r[b] <= t;                                              // R6/R7: accept iff r <= t
-                const int a = (int)(fw >> 1) + (int)(fw & 1u);              // antiparallel neighbours
-                if (D) {
-                    o += (uint32_t)(RS * (2 - a));                          // j <- j + 2 - a  (dE = 8 - 4a)
-                    c ^= 1u << x;
-                }
-                if (MEAS) {                                                 // H[j]++ after EVERY attempt
-                    if (MODE == MODE_TBL_SMEM)
-                        atomicAdd(reinterpret_cast<uint32_t*>(const_cast<char*>(tbl_smem) + o + 32u), 1u);
-                    else
-                        atomicAdd(hist + (o >> 5), 1u);
-                }
-                if (k == 0 && x == 0) {
-                    // the right neighbour of the LAST site of the row is site 0, which has just been decided
+            for (int q = 0; q < BITS / 4; ++q) {
+                uint32_t rnd[4];
+                philox4x32_10(ctr0_row + (uint32_t)(k * 8 + q), sweep, iteration, walker, key0, key1, rnd);
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    const int x = q * 4 + r;
+                    uint32_t fw = (FW[k][r] >> (4 * q)) & 7u;
+                    if (D) fw ^= 1u;
+                    const uint32_t t = __ldg(reinterpret_cast<const uint32_t*>(tbl_glob + (o + 4u * fw)));
+                    const uint32_t o_acc = o + 2u * RS - __byte_perm(LUT_LO, LUT_HI, fw);   // j + 2 - a  (dE = 8 - 4a)
+                    D = rnd[r] <= t;                                       // R6/R7: accept iff r <= t
                     if (D) {
-                        hrL ^= 1u << (BITS - 1);
-                        lo[WPR - 1] = vuL ^ vdL ^ hrL;
-                        hi[WPR - 1] = (vuL & vdL) | (vuL & hrL) | (vdL & hrL);
+                        o = o_acc;
+                        c ^= 1u << x;
+                    }
+                    if (MEAS) atomicAdd(hist + (o >> 5), 1u);              // H[j]++ after EVERY attempt
+                    if (k == 0 && x == 0) {
+                        // the right neighbour of the LAST site of the row is site 0, which has just been decided
+                        if (D) FW[WPR - 1][3] += patch;
                     }
                 }
             }
+            cur[k] = c;
         }
-        cur[k] = c;
     }
 }
 
@@ -413,7 +530,8 @@ __global__ void sweep_kernel(const SweepParams prm) {
 
     if (active) {
         const int E = prm.E[w];
-        uint32_t o = (uint32_t)((E + 2 * N) >> 2) * (uint32_t)(RSW * 4);   // slot j = (E + 2N)/4
+        const uint32_t o_base = MODE == MODE_TBL_SMEM ? (uint32_t)__cvta_generic_to_shared(tbl_s) : 0u;
+        uint32_t o = o_base + (uint32_t)((E + 2 * N) >> 2) * (uint32_t)(RSW * 4);   // slot j = (E + 2N)/4
         const uint32_t walker = prm.walker_offset + (uint32_t)w;
         const char* tbl_smem = reinterpret_cast<const char*>(tbl_s);
         const char* tbl_glob = reinterpret_cast<const char*>(prm.table);
@@ -428,7 +546,7 @@ __global__ void sweep_kernel(const SweepParams prm) {
             resident_sweeps<L, MODE, false>(lat, tpb, o, prm.sweep_begin, s_th, prm, walker, tbl_smem, tbl_glob, tbl_s);
             resident_sweeps<L, MODE, true>(lat, tpb, o, s_th, prm.sweep_end, prm, walker, tbl_smem, tbl_glob, tbl_s);
         }
-        prm.E[w] = (int)(o / (uint32_t)(RSW * 4)) * 4 - 2 * N;
+        prm.E[w] = (int)((o - o_base) / (uint32_t)(RSW * 4)) * 4 - 2 * N;
 
         if (MODE != MODE_STREAMED) {
             if (L >= 32) {

@@ -1,0 +1,59 @@
+"""The C-ABI library builds, loads and exports every symbol include/muca.h declares (no GPU, no compute calls)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+import paper_1707_00919_b200 as mb
+from paper_1707_00919_b200 import binding as B
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "muca.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(muca_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_header_and_binding_list_agree():
+    assert declared_symbols() == sorted(B.EXPORTS)
+
+
+def test_library_exports_every_declared_symbol():
+    lib = ctypes.CDLL(mb.lib_path()) if os.path.exists(mb.lib_path()) else mb.lib()
+    for name in declared_symbols():
+        assert hasattr(lib, name), f"{name} is declared in include/muca.h but not exported"
+
+
+def test_host_only_entry_points():
+    lib = mb.lib()
+    assert b"sm_100a" in lib.muca_version()
+    # workspace: packed spins + energies + threshold table + histogram, 256-byte aligned pieces
+    for L, W in ((8, 128), (32, 16384), (128, 8192)):
+        n = mb.workspace_bytes(L, W)
+        assert n >= W * L * L // 8 + 4 * W + (L * L + 1) * 40 and n % 256 == 0
+    assert mb.workspace_bytes(12, 32) == 0 and mb.workspace_bytes(32, 0) == 0
+    # bad arguments are rejected before any CUDA call
+    h = ctypes.c_void_p()
+    assert lib.muca_create(ctypes.byref(h), 7, 32, 1) == -1 and not h
+    assert lib.muca_create_in(ctypes.byref(h), 32, 0, 1, 0, None, 0, None) == -1 and not h
+
+
+def test_no_cpu_fallback():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("CUDA present")
+    with pytest.raises(mb.MucaError):
+        mb.Muca(8, 32, 1)
+
+
+def test_product_does_not_import_the_oracle():
+    pkg = os.path.join(ROOT, "paper_1707_00919_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "muca_oracle" not in src and "oracle/" not in src.replace("shares nothing with oracle/", "").replace(
+                    "Shares nothing with oracle/", "").replace("imported by neither oracle/", ""), f
