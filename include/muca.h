@@ -55,7 +55,8 @@ typedef enum muca_status {
 /* Sweep-kernel variants (muca_set_option(ctx, MUCA_OPT_KERNEL, ...)).
  * AUTO picks RESIDENT when the packed lattices of one block plus the tables fit in
  * shared memory (L <= 64) and STREAMED otherwise (L = 128). */
-enum { MUCA_KERNEL_AUTO = 0, MUCA_KERNEL_RESIDENT = 1, MUCA_KERNEL_STREAMED = 2 };
+enum { MUCA_KERNEL_AUTO = 0, MUCA_KERNEL_RESIDENT = 1, MUCA_KERNEL_STREAMED = 2,
+       MUCA_KERNEL_RESIDENT_V2 = 3 /* L <= 32 only: the earlier predicate-carried resident kernel, kept for A/B runs */ };
 enum {
     MUCA_OPT_KERNEL = 1,          /* one of MUCA_KERNEL_*                                        */
     MUCA_OPT_THREADS_PER_BLOCK = 2, /* walkers (= threads) per block; 0 = library default         */

@@ -113,6 +113,19 @@ void expand_table8(const std::vector<uint32_t>& t5, int bins, uint32_t* t8) {
         }
 }
 
+template <int L>
+int launch_sweep_v3(muca_ctx* ctx, const SweepParams& prm, int tpb) {
+    static bool configured = false;
+    if (!configured) {
+        CU(cudaFuncSetAttribute(sweep_kernel_v3<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V3<L>::SMEM_BYTES));
+        configured = true;
+    }
+    const int grid = (prm.W + tpb - 1) / tpb;
+    sweep_kernel_v3<L><<<grid, 2 * tpb, V3<L>::SMEM_BYTES, ctx->stream>>>(prm);   // tpb walker + tpb deviate threads
+    CU(cudaGetLastError());
+    return MUCA_OK;
+}
+
 template <int L, int MODE>
 int launch_sweep_t(muca_ctx* ctx, const SweepParams& prm, int tpb) {
     const size_t smem = sweep_smem_bytes<L, MODE>(tpb);
@@ -135,11 +148,14 @@ Plan make_plan(const muca_ctx* c) {
     int kern = c->opt_kernel;
     if (kern == MUCA_KERNEL_AUTO) kern = L <= 64 ? MUCA_KERNEL_RESIDENT : MUCA_KERNEL_STREAMED;
     if (kern == MUCA_KERNEL_STREAMED && L < 32) kern = MUCA_KERNEL_RESIDENT;
-    if (kern == MUCA_KERNEL_RESIDENT) p.mode = L <= 32 ? MODE_TBL_SMEM : MODE_TBL_L1;
+    if (kern == MUCA_KERNEL_RESIDENT_V2 && L > 32) kern = MUCA_KERNEL_RESIDENT;
+    if (kern == MUCA_KERNEL_RESIDENT) p.mode = L <= 32 ? MODE_V3 : MODE_TBL_L1;
+    else if (kern == MUCA_KERNEL_RESIDENT_V2) p.mode = MODE_TBL_SMEM;
     else p.mode = MODE_STREAMED;
     int tpb = c->opt_tpb;
     if (tpb <= 0) {
-        if (p.mode == MODE_TBL_SMEM) tpb = 32;
+        if (p.mode == MODE_V3) tpb = L == 32 ? 128 : 32;
+        else if (p.mode == MODE_TBL_SMEM) tpb = 32;
         else if (p.mode == MODE_TBL_L1) tpb = L == 64 ? 64 : 32;
         else tpb = 32;
     }
@@ -148,6 +164,7 @@ Plan make_plan(const muca_ctx* c) {
 }
 
 size_t plan_smem(int L, const Plan& p) {
+    if (p.mode == MODE_V3) return L == 8 ? V3<8>::SMEM_BYTES : L == 16 ? V3<16>::SMEM_BYTES : V3<32>::SMEM_BYTES;
     switch (L) {
         case 8: return sweep_smem_bytes<8, MODE_TBL_SMEM>(p.tpb);
         case 16: return sweep_smem_bytes<16, MODE_TBL_SMEM>(p.tpb);
@@ -162,6 +179,14 @@ size_t plan_smem(int L, const Plan& p) {
 }
 
 int launch_sweep(muca_ctx* ctx, const SweepParams& prm, const Plan& p) {
+    if (p.mode == MODE_V3) {
+        if (p.tpb > V3<32>::MAX_TPB) return fail(ctx, MUCA_EINVAL, "resident kernel: at most %d threads per block", V3<32>::MAX_TPB);
+        switch (ctx->L) {
+            case 8: return launch_sweep_v3<8>(ctx, prm, p.tpb);
+            case 16: return launch_sweep_v3<16>(ctx, prm, p.tpb);
+            case 32: return launch_sweep_v3<32>(ctx, prm, p.tpb);
+        }
+    }
     switch (ctx->L) {
         case 8: return launch_sweep_t<8, MODE_TBL_SMEM>(ctx, prm, p.tpb);
         case 16: return launch_sweep_t<16, MODE_TBL_SMEM>(ctx, prm, p.tpb);
@@ -258,7 +283,7 @@ void muca_destroy(muca_ctx* ctx) {
 int muca_set_option(muca_ctx* ctx, int option, int value) {
     if (!ctx) return MUCA_EINVAL;
     if (option == MUCA_OPT_KERNEL) {
-        if (value < MUCA_KERNEL_AUTO || value > MUCA_KERNEL_STREAMED) return fail(ctx, MUCA_EINVAL, "bad kernel %d", value);
+        if (value < MUCA_KERNEL_AUTO || value > MUCA_KERNEL_RESIDENT_V2) return fail(ctx, MUCA_EINVAL, "bad kernel %d", value);
         ctx->opt_kernel = value;
         return MUCA_OK;
     }

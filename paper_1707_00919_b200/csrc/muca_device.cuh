@@ -184,7 +184,7 @@ struct SweepParams {
     uint32_t therm;             // sweeps with index < therm are not recorded
 };
 
-enum { MODE_TBL_SMEM = 0, MODE_TBL_L1 = 1, MODE_STREAMED = 2 };
+enum { MODE_TBL_SMEM = 0, MODE_TBL_L1 = 1, MODE_STREAMED = 2, MODE_V3 = 3 };
 
 template <int L>
 struct Geo {
@@ -387,6 +387,261 @@ __device__ __forceinline__ void process_row(const uint32_t (&up)[Geo<L>::WPR], u
                 }
             }
             cur[k] = c;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// v3 resident kernel for L <= 32: "state in the address".
+//
+// The walker's whole dynamic state -- energy slot j AND the carry c = [previous site of this row flipped] --
+// is ONE shared-memory address P = rowaddr(j, c).  The table is stored twice: copy c at byte offset c*K (K a
+// power of two above copy 0 and the lattices), and copy 1 has its columns permuted (f -> f ^ 1: a flipped
+// left neighbour toggles the [left != s] bit).  Entry (j, c, f) is 8 bytes {t, dP}:
+//     t  = thresh[j][a],  a = a(f ^ c)                 (PAPER.md:109 acceptance, R6/R7)
+//     dP = rowaddr(j + 2 - a, 1) - rowaddr(j, c)        (where an ACCEPTED move leads; a rejected one leads to
+//                                                        rowaddr(j, 0) = P & ~K)
+// so the per-site serial chain is   P -> IMAD (P + 8f) -> LDS.64 -> {ISETP | IADD} -> SEL -> P'
+// with no predicated instruction on it (ISETP -> predicated op costs ~13 cycles more than ISETP -> SEL on
+// sm_100a, profiles/r01_ubench_pipes.txt) and no PRMT / column fix-up.  Row j of a copy is 72 bytes:
+// 8 entries, the histogram bin of (j, c) at +64, 4 bytes of padding; the two bins of a slot are added at the merge.
+// ------------------------------------------------------------------------------------------------
+template <int L>
+struct V3 {
+    static constexpr uint32_t BINS = L * L + 1;
+    static constexpr uint32_t RS = 72;
+    static constexpr uint32_t BIN_OFF = 64;
+    static constexpr uint32_t TBL_BYTES = (BINS + 1) * RS;   // + one all-reject row for the unused slots of the last block
+    static constexpr uint32_t K = L == 32 ? 131072u : (L == 16 ? 65536u : 32768u);
+    static constexpr uint32_t LAT_OFF = (TBL_BYTES + 15u) & ~15u;
+    static constexpr int MAX_TPB = 128;                      // walkers per block; lattices + deviate ring must fit between copy 0 and K
+    static_assert(1024u + LAT_OFF + 16u + ((uint32_t)L * 4u + 2u * (L / 4) * 16u) * MAX_TPB <= K, "copy 0 + lattices + ring must end below K");
+    static constexpr size_t SMEM_BYTES = (size_t)K + TBL_BYTES;
+};
+
+// static planes of one row (single word, L <= 32): nibble q of FW[r] = column f = hl + 2*lo + 4*hi of site 4q + r
+template <int L>
+__device__ __forceinline__ void field_words(const uint32_t up, const uint32_t c, const uint32_t dn, uint32_t (&FW)[4],
+                                            uint32_t& patch) {
+    using G = Geo<L>;
+    constexpr int BITS = G::BITS;
+    uint32_t rw, lw;
+    if constexpr (L >= 32) {
+        rw = (c >> 1) | (c << 31);
+        lw = (c << 1) | (c >> 31);
+    } else {
+        rw = (c >> 1) | ((c & 1u) << (BITS - 1));
+        lw = ((c << 1) | (c >> (BITS - 1))) & G::MASK;
+    }
+    const uint32_t vu = c ^ up, vd = c ^ dn, hr = c ^ rw, hl = c ^ lw;
+    const uint32_t lo = vu ^ vd ^ hr;
+    const uint32_t hi = (vu & vd) | (vu & hr) | (vd & hr);
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const uint32_t A = hl >> r;
+        const uint32_t B = r >= 1 ? lo >> (r - 1) : lo << 1;
+        const uint32_t C = r >= 2 ? hi >> (r - 2) : hi << (2 - r);
+        const uint32_t t1 = (A & 0x11111111u) | (B & ~0x11111111u);
+        FW[r] = (t1 & 0x33333333u) | (C & ~0x33333333u);
+    }
+    constexpr int QL = BITS / 4 - 1;
+    const uint32_t hr_last = (hr >> (BITS - 1)) & 1u;
+    patch = (1u << (4 * QL + 1)) - (hr_last << (4 * QL + 2));   // site 0 flipped: n3 of the LAST site +-1
+}
+
+// One Philox4x32-10 round on the state of one call (see philox4x32_10 above).
+__device__ __forceinline__ void philox_round(uint32_t (&c)[4], const uint32_t k0, const uint32_t k1) {
+    const uint64_t p0 = (uint64_t)0xD2511F53u * c[0];
+    const uint64_t p1 = (uint64_t)0xCD9E8D57u * c[2];
+    const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c[1] ^ k0;
+    const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c[3] ^ k1;
+    c[1] = (uint32_t)p1;
+    c[3] = (uint32_t)p0;
+    c[0] = n0;
+    c[2] = n2;
+}
+
+__device__ __forceinline__ void pair_barrier(const int id) {   // named barrier of one walker warp + its deviate warp
+    asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory");
+}
+
+// Deviate warp: the BITS/4 Philox calls of one row advance round-major (16 independent IMAD.WIDE chains at L = 32:
+// a lone dependent chain issues one instruction per ~5 cycles), results go to the double-buffered shared ring
+// rnd[buf][call][walker] as one 16-byte store per call.  One barrier per row hands the buffer over.
+template <int L>
+__device__ __forceinline__ void deviate_rows(uint4* __restrict__ ring, const int WB, const int ptid, const int bar_id,
+                                             const SweepParams& prm, const uint32_t walker) {
+    constexpr int NC = Geo<L>::BITS / 4;
+    int buf = 0;
+#pragma unroll 1
+    for (uint32_t s = prm.sweep_begin; s < prm.sweep_end; ++s) {
+#pragma unroll 1
+        for (int y = 0; y < L; ++y) {
+            uint32_t st[NC][4];
+#pragma unroll
+            for (int k = 0; k < NC; ++k) {     // R4: ctr = (i >> 2, sweep, iteration, walker)
+                st[k][0] = (uint32_t)(y * (L / 4) + k); st[k][1] = s; st[k][2] = prm.iteration; st[k][3] = walker;
+            }
+#pragma unroll
+            for (int r = 0; r < 10; ++r)
+#pragma unroll
+                for (int k = 0; k < NC; ++k)
+                    philox_round(st[k], prm.key0 + (uint32_t)r * 0x9E3779B9u, prm.key1 + (uint32_t)r * 0xBB67AE85u);
+#pragma unroll
+            for (int k = 0; k < NC; ++k) ring[(buf * NC + k) * WB + ptid] = make_uint4(st[k][0], st[k][1], st[k][2], st[k][3]);
+            pair_barrier(bar_id);
+            buf ^= 1;
+        }
+    }
+}
+
+// Walker warp: sweeps s0 .. s1-1; `buf` is the ring buffer holding the deviates of the next row to process.
+template <int L, bool MEAS>
+__device__ __forceinline__ void sweeps_v3(uint32_t* __restrict__ lat, const int WB, uint32_t& P, const uint32_t s0,
+                                          const uint32_t s1, const uint4* __restrict__ ring, int& buf, const int bar_id) {
+    using G = Geo<L>;
+    using V = V3<L>;
+    constexpr int BITS = G::BITS, NC = BITS / 4;
+#pragma unroll 1
+    for (uint32_t s = s0; s < s1; ++s) {
+#pragma unroll 1
+        for (int y = 0; y < L; ++y) {
+            const int ym = (y + L - 1) & (L - 1), yp = (y + 1) & (L - 1);
+            const uint32_t up = lat[ym * WB], dn = lat[yp * WB];
+            const uint32_t c = lat[y * WB];
+            uint32_t FW[4], patch;
+            field_words<L>(up, c, dn, FW, patch);
+            pair_barrier(bar_id);              // the deviates of this row are in ring[buf]; ring[buf ^ 1] may be refilled
+            uint32_t rnd[BITS];
+#pragma unroll
+            for (int k = 0; k < NC; ++k) {
+                const uint4 v = ring[(buf * NC + k) * WB];
+                rnd[4 * k] = v.x; rnd[4 * k + 1] = v.y; rnd[4 * k + 2] = v.z; rnd[4 * k + 3] = v.w;
+            }
+            buf ^= 1;
+            P &= ~V::K;                        // site 0: its left neighbour (site L-1) has not been visited in this sweep
+            uint32_t A = P + ((FW[0] << 3) & 0x38u);
+            uint32_t hpend = 0, flips = 0;
+#pragma unroll
+            for (int x = 0; x < BITS; ++x) {
+                uint32_t t, dP;
+                asm("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(t), "=r"(dP) : "r"(A));
+                if (MEAS && x > 0)                 // H[j]++ of the PREVIOUS site, issued behind this site's table load
+                    asm volatile("red.shared.add.u32 [%0+64], 1;" ::"r"(hpend) : "memory");
+                const bool D = rnd[x] <= t;        // R6/R7: accept iff r <= t
+                if (x == 0 && D) FW[3] += patch;
+                // column offset of the next site; both candidates of its entry address are ready before D is known
+                const int xn = x + 1;
+                const uint32_t f8n = xn >= BITS ? 0u
+                                     : (xn >> 2) == 0 ? (FW[xn & 3] << 3) & 0x38u
+                                                      : (FW[xn & 3] >> ((xn >> 2) > 0 ? 4 * (xn >> 2) - 3 : 0)) & 0x38u;
+                // A_acc feeds both the select below and P_acc, which keeps ptxas from folding the add into a predicated
+                // instruction (ISETP -> predicated op costs ~9 cycles more than ISETP -> SEL on the serial chain)
+                const uint32_t P_rej = P & ~V::K, A_rej = P_rej + f8n, Q = P + f8n;
+                uint32_t A_acc;
+                asm("add.u32 %0, %1, %2;" : "=r"(A_acc) : "r"(Q), "r"(dP));
+                A = D ? A_acc : A_rej;
+                P = D ? A_acc - f8n : P_rej;
+                if (D) flips |= 1u << x;
+                hpend = P;
+            }
+            if (MEAS)
+                asm volatile("red.shared.add.u32 [%0+64], 1;" ::"r"(hpend) : "memory");
+            lat[y * WB] = c ^ flips;
+        }
+    }
+}
+
+// Block = WB deviate threads (warps 0 .. WB/32-1) + WB walker threads (the next WB/32 warps); walker warp i and
+// deviate warp i serve the same 32 walkers and, at WB = 128, share one scheduler (warp ids i and i + 4), so the
+// hardware interleaves the Philox instruction stream into the stalls of the walker warp's serial chain.
+template <int L>
+__global__ void __launch_bounds__(2 * V3<L>::MAX_TPB, 1) sweep_kernel_v3(const SweepParams prm) {
+    using G = Geo<L>;
+    using V = V3<L>;
+    constexpr int N = G::N, BINS = G::BINS, NC = G::BITS / 4;
+    extern __shared__ __align__(16) uint32_t smem[];
+    char* const sm = reinterpret_cast<char*>(smem);
+    const int tid = threadIdx.x, nthr = blockDim.x, WB = nthr >> 1;
+    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(smem);
+    const uint32_t ring_off = (V::LAT_OFF + (uint32_t)L * 4u * (uint32_t)WB + 15u) & ~15u;
+    if (sbase + ring_off + 2u * NC * 16u * (uint32_t)WB > V::K) __trap();
+
+    // ---- both table copies: entry (j, c, f) = {t, dP}; bins zeroed
+    for (int idx = tid; idx < BINS * 16; idx += nthr) {
+        const int j = idx >> 4, cc = (idx >> 3) & 1, f = idx & 7;
+        const int fe = f ^ cc, a = (fe >> 1) + (fe & 1);
+        uint2 e;
+        e.x = prm.table[j * 8 + fe];
+        e.y = (uint32_t)((int)V::RS * (2 - a)) + (cc ? 0u : V::K);
+        *reinterpret_cast<uint2*>(sm + (size_t)cc * V::K + (size_t)j * V::RS + 8 * f) = e;
+    }
+    for (int idx = tid; idx < BINS * 2; idx += nthr) {
+        const int j = idx >> 1, cc = idx & 1;
+        *reinterpret_cast<uint2*>(sm + (size_t)cc * V::K + (size_t)j * V::RS + V::BIN_OFF) = make_uint2(0u, 0u);
+    }
+    if (tid < 9)   // row BINS of copy 0: {t = 0, dP = 0} in every column -- a walker parked here stays here; its bin is never merged
+        *reinterpret_cast<uint2*>(sm + (size_t)BINS * V::RS + 8 * tid) = make_uint2(0u, 0u);
+
+    const bool is_walker = tid >= WB;                          // higher warp ids win the scheduler's arbitration: give them the serial chain
+    const int lt = is_walker ? tid - WB : tid;                 // walker slot in the block
+    const int w = blockIdx.x * WB + lt;
+    const bool active = w < prm.W;                             // unused slots of the last block are parked on the all-reject row
+    const int bar_id = 1 + (lt >> 5);
+    uint32_t* const lat = reinterpret_cast<uint32_t*>(sm + V::LAT_OFF) + lt;
+    uint4* const ring = reinterpret_cast<uint4*>(sm + ring_off);
+
+    // ---- lattice: one word per row
+    if (is_walker) {
+        if (!active) {
+            for (int y = 0; y < L; ++y) lat[y * WB] = 0u;
+        } else if (L >= 32) {
+            for (int y = 0; y < L; ++y) lat[y * WB] = prm.spins[(size_t)y * prm.W + w];
+        } else {
+            constexpr int RPW = 32 / G::BITS;
+            for (int t = 0; t < N / 32; ++t) {
+                const uint32_t word = prm.spins[(size_t)t * prm.W + w];
+#pragma unroll
+                for (int q = 0; q < RPW; ++q) lat[(t * RPW + q) * WB] = (word >> (q * G::BITS)) & G::MASK;
+            }
+        }
+    }
+    __syncthreads();
+
+    const uint32_t walker = prm.walker_offset + (uint32_t)w;
+    if (!is_walker) {
+        deviate_rows<L>(ring, WB, lt, bar_id, prm, walker);
+    } else {
+        // slot j = (E + 2N)/4, copy 0
+        uint32_t P = sbase + (active ? (uint32_t)((prm.E[w] + 2 * N) >> 2) : (uint32_t)BINS) * V::RS;
+        const uint32_t s_th = prm.therm < prm.sweep_begin ? prm.sweep_begin
+                              : (prm.therm > prm.sweep_end ? prm.sweep_end : prm.therm);
+        int buf = 0;
+        sweeps_v3<L, false>(lat, WB, P, prm.sweep_begin, s_th, ring + lt, buf, bar_id);
+        sweeps_v3<L, true>(lat, WB, P, s_th, prm.sweep_end, ring + lt, buf, bar_id);
+        if (active) {
+            prm.E[w] = (int)(((P & ~V::K) - sbase) / V::RS) * 4 - 2 * N;
+            if (L >= 32) {
+                for (int y = 0; y < L; ++y) prm.spins[(size_t)y * prm.W + w] = lat[y * WB];
+            } else {
+                constexpr int RPW = 32 / G::BITS;
+                for (int t = 0; t < N / 32; ++t) {
+                    uint32_t word = 0u;
+#pragma unroll
+                    for (int q = 0; q < RPW; ++q) word |= lat[(t * RPW + q) * WB] << (q * G::BITS);
+                    prm.spins[(size_t)t * prm.W + w] = word;
+                }
+            }
+        }
+    }
+    __syncthreads();
+
+    // ---- a4: merge the two bins of every slot into the global uint64 histogram
+    if (prm.sweep_end > prm.therm) {
+        for (int j = tid; j < BINS; j += nthr) {
+            const uint32_t v = *reinterpret_cast<uint32_t*>(sm + (size_t)j * V::RS + V::BIN_OFF) +
+                               *reinterpret_cast<uint32_t*>(sm + (size_t)V::K + (size_t)j * V::RS + V::BIN_OFF);
+            if (v) atomicAdd(prm.H + j, (unsigned long long)v);
         }
     }
 }
