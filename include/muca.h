@@ -56,12 +56,15 @@ typedef enum muca_status {
  * AUTO picks RESIDENT when the packed lattices of one block plus the tables fit in
  * shared memory (L <= 64) and STREAMED otherwise (L = 128). */
 enum { MUCA_KERNEL_AUTO = 0, MUCA_KERNEL_RESIDENT = 1, MUCA_KERNEL_STREAMED = 2,
-       MUCA_KERNEL_RESIDENT_V2 = 3 /* L <= 32 only: the earlier predicate-carried resident kernel, kept for A/B runs */ };
+       MUCA_KERNEL_RESIDENT_V2 = 3, /* L <= 32 only: the earlier predicate-carried resident kernel, kept for A/B runs */
+       MUCA_KERNEL_RESIDENT_V3 = 4  /* L <= 32 only: the earlier paired walker/deviate-warp kernel, kept for A/B runs */ };
 enum {
     MUCA_OPT_KERNEL = 1,          /* one of MUCA_KERNEL_*                                        */
     MUCA_OPT_THREADS_PER_BLOCK = 2, /* walkers (= threads) per block; 0 = library default         */
-    MUCA_OPT_MAX_SWEEPS_PER_LAUNCH = 3 /* split an iteration into launches of at most this many sweeps;
+    MUCA_OPT_MAX_SWEEPS_PER_LAUNCH = 3, /* split an iteration into launches of at most this many sweeps;
                                           0 = only as needed to keep a block's uint32 bins from overflowing */
+    MUCA_OPT_WALKERS_PER_WARP = 4 /* resident kernel, L <= 32: walkers served by one warp (1..32); 0 = spread
+                                     the walkers evenly over all SMs */
 };
 
 /* Device workspace needed by muca_create_in() for (L, n_walkers); 0 on bad arguments. */

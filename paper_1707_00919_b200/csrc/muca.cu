@@ -11,6 +11,7 @@
 #include <vector>
 
 #include "muca_device.cuh"
+#include "muca_resident.cuh"
 
 using namespace muca;
 
@@ -39,6 +40,8 @@ struct muca_ctx {
     int opt_kernel = MUCA_KERNEL_AUTO;
     int opt_tpb = 0;
     int opt_max_sweeps = 0;
+    int opt_wpw = 0;
+    int n_sm = 0;
     char err[512] = {0};
 };
 
@@ -126,6 +129,20 @@ int launch_sweep_v3(muca_ctx* ctx, const SweepParams& prm, int tpb) {
     return MUCA_OK;
 }
 
+template <int L>
+int launch_sweep_v5(muca_ctx* ctx, const SweepParams& prm, int nw, int wpw) {
+    static bool configured = false;
+    if (!configured) {
+        CU(cudaFuncSetAttribute(sweep_kernel_v5<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V5<L>::SMEM_BYTES));
+        configured = true;
+    }
+    const int per_block = nw * wpw;
+    const int grid = (prm.W + per_block - 1) / per_block;
+    sweep_kernel_v5<L><<<grid, 64 * nw, V5<L>::SMEM_BYTES, ctx->stream>>>(prm, wpw);
+    CU(cudaGetLastError());
+    return MUCA_OK;
+}
+
 template <int L, int MODE>
 int launch_sweep_t(muca_ctx* ctx, const SweepParams& prm, int tpb) {
     const size_t smem = sweep_smem_bytes<L, MODE>(tpb);
@@ -140,7 +157,7 @@ int launch_sweep_t(muca_ctx* ctx, const SweepParams& prm, int tpb) {
     return MUCA_OK;
 }
 
-struct Plan { int mode; int tpb; };
+struct Plan { int mode; int tpb; int nw; int wpw; };   // tpb = walkers per block; v5: nw warp pairs x wpw walkers per warp
 
 Plan make_plan(const muca_ctx* c) {
     Plan p;
@@ -148,10 +165,26 @@ Plan make_plan(const muca_ctx* c) {
     int kern = c->opt_kernel;
     if (kern == MUCA_KERNEL_AUTO) kern = L <= 64 ? MUCA_KERNEL_RESIDENT : MUCA_KERNEL_STREAMED;
     if (kern == MUCA_KERNEL_STREAMED && L < 32) kern = MUCA_KERNEL_RESIDENT;
-    if (kern == MUCA_KERNEL_RESIDENT_V2 && L > 32) kern = MUCA_KERNEL_RESIDENT;
-    if (kern == MUCA_KERNEL_RESIDENT) p.mode = L <= 32 ? MODE_V3 : MODE_TBL_L1;
+    if ((kern == MUCA_KERNEL_RESIDENT_V2 || kern == MUCA_KERNEL_RESIDENT_V3) && L > 32) kern = MUCA_KERNEL_RESIDENT;
+    p.nw = p.wpw = 0;
+    if (kern == MUCA_KERNEL_RESIDENT) p.mode = L <= 32 ? MODE_V5 : MODE_TBL_L1;
+    else if (kern == MUCA_KERNEL_RESIDENT_V3) p.mode = MODE_V3;
     else if (kern == MUCA_KERNEL_RESIDENT_V2) p.mode = MODE_TBL_SMEM;
     else p.mode = MODE_STREAMED;
+    if (p.mode == MODE_V5) {
+        // spread the walkers over all SMs: as few warps per SM as possible, then as few lanes per warp as possible
+        // (one block per SM; a half-empty warp costs the same issue slots, but fewer lanes collide in the banks)
+        const int n_sm = c->n_sm > 0 ? c->n_sm : 148;
+        const int warps = (c->W + 31) / 32;
+        int nw = c->opt_tpb > 0 ? c->opt_tpb / 32 : (warps <= n_sm ? 1 : warps <= 2 * n_sm ? 2 : 4);
+        if (nw < 1) nw = 1;
+        if (nw > 4) nw = 4;
+        int wpw = c->opt_wpw > 0 ? c->opt_wpw : (c->opt_tpb > 0 ? 32 : (c->W + n_sm * nw - 1) / (n_sm * nw));
+        if (wpw < 1) wpw = 1;
+        if (wpw > 32) wpw = 32;
+        p.nw = nw; p.wpw = wpw; p.tpb = nw * wpw;
+        return p;
+    }
     int tpb = c->opt_tpb;
     if (tpb <= 0) {
         if (p.mode == MODE_V3) tpb = L == 32 ? 128 : 32;
@@ -164,6 +197,7 @@ Plan make_plan(const muca_ctx* c) {
 }
 
 size_t plan_smem(int L, const Plan& p) {
+    if (p.mode == MODE_V5) return L == 8 ? V5<8>::SMEM_BYTES : L == 16 ? V5<16>::SMEM_BYTES : V5<32>::SMEM_BYTES;
     if (p.mode == MODE_V3) return L == 8 ? V3<8>::SMEM_BYTES : L == 16 ? V3<16>::SMEM_BYTES : V3<32>::SMEM_BYTES;
     switch (L) {
         case 8: return sweep_smem_bytes<8, MODE_TBL_SMEM>(p.tpb);
@@ -179,6 +213,13 @@ size_t plan_smem(int L, const Plan& p) {
 }
 
 int launch_sweep(muca_ctx* ctx, const SweepParams& prm, const Plan& p) {
+    if (p.mode == MODE_V5) {
+        switch (ctx->L) {
+            case 8: return launch_sweep_v5<8>(ctx, prm, p.nw, p.wpw);
+            case 16: return launch_sweep_v5<16>(ctx, prm, p.nw, p.wpw);
+            case 32: return launch_sweep_v5<32>(ctx, prm, p.nw, p.wpw);
+        }
+    }
     if (p.mode == MODE_V3) {
         if (p.tpb > V3<32>::MAX_TPB) return fail(ctx, MUCA_EINVAL, "resident kernel: at most %d threads per block", V3<32>::MAX_TPB);
         switch (ctx->L) {
@@ -233,6 +274,12 @@ int create_common(muca_ctx** out, int L, int W, uint64_t seed, uint32_t walker_o
         cudaMallocHost((void**)&ctx->h_H, (size_t)ctx->n_bins * 8) != cudaSuccess ||
         cudaEventCreate(&ctx->ev0) != cudaSuccess || cudaEventCreate(&ctx->ev1) != cudaSuccess)
         return bail(MUCA_ECUDA);
+    {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+            return bail(MUCA_ECUDA);
+    }
     const int tpb = 128;
     init_kernel<<<(W + tpb - 1) / tpb, tpb, 0, ctx->stream>>>(ctx->d_spins, ctx->d_E, L, W, walker_offset,
                                                              (uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32));
@@ -283,13 +330,18 @@ void muca_destroy(muca_ctx* ctx) {
 int muca_set_option(muca_ctx* ctx, int option, int value) {
     if (!ctx) return MUCA_EINVAL;
     if (option == MUCA_OPT_KERNEL) {
-        if (value < MUCA_KERNEL_AUTO || value > MUCA_KERNEL_RESIDENT_V2) return fail(ctx, MUCA_EINVAL, "bad kernel %d", value);
+        if (value < MUCA_KERNEL_AUTO || value > MUCA_KERNEL_RESIDENT_V3) return fail(ctx, MUCA_EINVAL, "bad kernel %d", value);
         ctx->opt_kernel = value;
         return MUCA_OK;
     }
     if (option == MUCA_OPT_THREADS_PER_BLOCK) {
         if (value < 0 || value > 1024 || (value % 32) != 0) return fail(ctx, MUCA_EINVAL, "threads per block must be a multiple of 32 in [0, 1024]");
         ctx->opt_tpb = value;
+        return MUCA_OK;
+    }
+    if (option == MUCA_OPT_WALKERS_PER_WARP) {
+        if (value < 0 || value > 32) return fail(ctx, MUCA_EINVAL, "walkers per warp must be in [0, 32]");
+        ctx->opt_wpw = value;
         return MUCA_OK;
     }
     if (option == MUCA_OPT_MAX_SWEEPS_PER_LAUNCH) {

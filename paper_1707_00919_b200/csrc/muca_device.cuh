@@ -184,7 +184,7 @@ struct SweepParams {
     uint32_t therm;             // sweeps with index < therm are not recorded
 };
 
-enum { MODE_TBL_SMEM = 0, MODE_TBL_L1 = 1, MODE_STREAMED = 2, MODE_V3 = 3 };
+enum { MODE_TBL_SMEM = 0, MODE_TBL_L1 = 1, MODE_STREAMED = 2, MODE_V3 = 3, MODE_V5 = 4 };
 
 template <int L>
 struct Geo {

@@ -1,0 +1,215 @@
+// paper_1707_00919_b200/csrc/muca_resident.cuh
+// Resident sweep kernel v5 for L <= 32 (sm_100a): "state in the address", walker warps paired with deviate warps.
+// Citations: "PAPER.md:<line>" = /root/reference/PAPER.md, "R<n>" = DESIGN.md section 3.
+//
+// The walker's dynamic state -- energy slot j AND the carry c = [previous site of this row flipped] -- is ONE
+// shared-memory address S = rowaddr(j, c).  The table is stored twice: copy c at byte offset c*K (K a power of
+// two above copy 0, the lattices and the deviate ring); copy 1 has its columns permuted (f -> f ^ 1: a flipped
+// left neighbour toggles the [left != s] bit of the column index).  Row (j, c) is 68 bytes (17 words: consecutive
+// rows rotate through all 32 banks):
+//     +4f      t  = thresh[j][a],  a = a(f ^ c)          (PAPER.md:109 acceptance, R6/R7)
+//     +32+4f   Sa = rowaddr(j + 2 - a, 1)                 (state an ACCEPTED move leads to; a rejected one leads
+//                                                          to rowaddr(j, 0) = S & ~K)
+//     +64      histogram bin of (j, c); the two bins of a slot are added at the merge (a4)
+// Two 32-bit loads instead of one 64-bit load: a random-row LDS.64 takes 34 cycles (two 16-lane phases, each with
+// its own bank conflicts), a random-row LDS.32 27 (profiles/r01_ubench_chain.txt).
+// Per site the serial chain is   LDS t -> ISETP -> SEL(A_acc, A_rej) -> LDS t'   with both candidate addresses
+// ready before the decision; column extraction, flip mask, histogram increment and the second select (S) are
+// off the chain.  Philox runs in a paired "deviate" warp (same 32 walkers) that feeds a double-buffered shared
+// ring one row ahead: the hardware interleaves its instruction stream into the stalls of the walker warp
+// (a single in-order warp doing both reaches only 75 cycles per site).
+#pragma once
+#include "muca_device.cuh"
+
+namespace muca {
+
+
+template <int L>
+struct V5 {
+    static constexpr uint32_t BINS = L * L + 1;
+    static constexpr uint32_t RS = 68;
+    static constexpr uint32_t SA_OFF = 32, BIN_OFF = 64;
+    static constexpr uint32_t TBL_BYTES = (BINS + 1) * RS;   // + one all-reject row: parking place of unused lanes
+    static constexpr uint32_t K = L == 32 ? 131072u : (L == 16 ? 65536u : 32768u);
+    static constexpr uint32_t LAT_OFF = (TBL_BYTES + 15u) & ~15u;
+    static constexpr int MAX_WARPS = 4;                      // walker warps per block (+ as many deviate warps)
+    static constexpr int SLOTS = 32 * MAX_WARPS;             // lattice / ring columns
+    static constexpr int NC = Geo<L>::BITS / 4;              // Philox calls per row
+    static constexpr uint32_t RING_OFF = LAT_OFF + (uint32_t)L * 4u * SLOTS;
+    static constexpr uint32_t RING_BYTES = 2u * NC * 16u * SLOTS;
+    static_assert(1024u + RING_OFF + RING_BYTES <= K, "copy 0 + lattices + ring must end below K");
+    static constexpr size_t SMEM_BYTES = (size_t)K + TBL_BYTES;
+};
+
+// One site of the walker chain, in PTX so that the decision is consumed by SEL (ISETP -> SEL -> LDS is 9 cycles on
+// sm_100a, ISETP -> predicated instruction -> LDS is more, and ptxas prefers the latter when left to itself).
+//   S: state address (in/out)   A: entry address of this site (in), of the next site (out)
+//   g: 4 * column of the NEXT site   r: deviate   BIT: flip mask of this site
+#define MUCA_V5_SITE(HIST_LINE, EXTRA_LINE)                                      \
+    "{\n\t.reg .pred p;\n\t.reg .b32 t, sa, sr, aa, ar;\n\t"                    \
+    "ld.shared.u32 t, [%1];\n\t"                                                 \
+    "ld.shared.u32 sa, [%1+32];\n\t" HIST_LINE                                   \
+    "and.b32 sr, %0, %7;\n\t"                                                    \
+    "add.u32 ar, sr, %5;\n\t"                                                    \
+    "add.u32 aa, sa, %5;\n\t"                                                    \
+    "setp.le.u32 p, %4, t;\n\t"                                                  \
+    "selp.u32 %1, aa, ar, p;\n\t"                                                \
+    "selp.u32 %0, sa, sr, p;\n\t"                                                \
+    "@p or.b32 %2, %2, %6;\n\t" EXTRA_LINE "}"
+
+// Walker warp: sweeps s0 .. s1-1; `buf` is the ring buffer holding the deviates of the next row to process.
+template <int L, bool MEAS>
+__device__ __forceinline__ void sweeps_v5(uint32_t* __restrict__ lat, uint32_t& S, const uint32_t s0, const uint32_t s1,
+                                          const uint4* __restrict__ ring, int& buf, const int bar_id) {
+    using G = Geo<L>;
+    using V = V5<L>;
+    constexpr int BITS = G::BITS, NC = V::NC, SLOTS = V::SLOTS;
+#pragma unroll 1
+    for (uint32_t s = s0; s < s1; ++s) {
+#pragma unroll 1
+        for (int y = 0; y < L; ++y) {
+            const int ym = (y + L - 1) & (L - 1), yp = (y + 1) & (L - 1);
+            const uint32_t up = lat[ym * SLOTS], dn = lat[yp * SLOTS], c = lat[y * SLOTS];
+            uint32_t FW[4], patch;
+            field_words<L>(up, c, dn, FW, patch);
+            pair_barrier(bar_id);              // the deviates of this row are in ring[buf]; ring[buf ^ 1] may be refilled
+            uint32_t rnd[BITS];
+#pragma unroll
+            for (int k = 0; k < NC; ++k) {
+                const uint4 v = ring[(buf * NC + k) * SLOTS];
+                rnd[4 * k] = v.x; rnd[4 * k + 1] = v.y; rnd[4 * k + 2] = v.z; rnd[4 * k + 3] = v.w;
+            }
+            buf ^= 1;
+            S &= ~V::K;                        // site 0: its left neighbour (site L-1) has not been visited in this sweep
+            uint32_t A = S + ((FW[0] << 2) & 0x1Cu);
+            uint32_t flips = 0, unused = 0;   // `unused` fills operand %3 of the site macro where site 0 has FW[3]
+#pragma unroll
+            for (int x = 0; x < BITS; ++x) {
+                const int xn = x + 1, qn = xn >> 2;
+                uint32_t g = 0;                // 4 * column of the next site
+                if (xn < BITS) {
+                    if (qn == 0) g = (FW[xn & 3] << 2) & 0x1Cu;
+                    else if (qn == 1) g = (FW[xn & 3] >> 2) & 0x1Cu;
+                    else g = (FW[xn & 3] >> (4 * qn - 2)) & 0x1Cu;
+                }
+                // H[j]++ of the PREVIOUS site is issued behind this site's table loads (S still holds that state)
+                if (x == 0) {                  // site 0 also patches the last site's column: its right neighbour is site 0
+                    asm volatile(MUCA_V5_SITE("", "@p add.u32 %3, %3, %8;\n\t")
+                                 : "+r"(S), "+r"(A), "+r"(flips), "+r"(FW[3])
+                                 : "r"(rnd[x]), "r"(g), "r"(1u), "n"(~V::K), "r"(patch));
+                } else if (MEAS) {
+                    asm volatile(MUCA_V5_SITE("red.shared.add.u32 [%0+64], 1;\n\t", "")
+                                 : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused)
+                                 : "r"(rnd[x]), "r"(g), "r"(1u << (x & 31)), "n"(~V::K)
+                                 : "memory");
+                } else {
+                    asm volatile(MUCA_V5_SITE("", "")
+                                 : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused)
+                                 : "r"(rnd[x]), "r"(g), "r"(1u << (x & 31)), "n"(~V::K));
+                }
+            }
+            if (MEAS)                          // H[j]++ after EVERY attempt: the last site of the row
+                asm volatile("red.shared.add.u32 [%0+64], 1;" ::"r"(S) : "memory");
+            lat[y * SLOTS] = c ^ flips;
+        }
+    }
+}
+
+// Block = nw deviate warps (warp ids 0 .. nw-1) + nw walker warps (ids nw .. 2nw-1), nw <= 4; walker warp i and
+// deviate warp i serve the same wpw <= 32 walkers, (b*nw + i)*wpw .. +wpw-1, in their lanes 0 .. wpw-1.  At nw = 4 a
+// pair shares one scheduler (warp ids i and i + 4) and the higher id -- the serial chain -- wins the arbitration;
+// at nw <= 2 every warp has a scheduler of its own.  The host spreads the walkers over all SMs (as few warps per
+// SM, then as few lanes per warp, as possible: fewer lanes collide in the banks).  Lanes without a walker are
+// parked on the all-reject row and never leave it.
+template <int L>
+__global__ void __launch_bounds__(64 * V5<L>::MAX_WARPS, 1) sweep_kernel_v5(const SweepParams prm, const int wpw) {
+    using G = Geo<L>;
+    using V = V5<L>;
+    constexpr int N = G::N, BINS = G::BINS, SLOTS = V::SLOTS;
+    extern __shared__ __align__(16) uint32_t smem[];
+    char* const sm = reinterpret_cast<char*>(smem);
+    const int tid = threadIdx.x, nthr = blockDim.x, nw = nthr >> 6;
+    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(smem);
+    if (sbase + V::RING_OFF + V::RING_BYTES > V::K) __trap();
+
+    // ---- both table copies: row (j, c) = t[8] | Sa[8] | bin
+    for (int idx = tid; idx < BINS * 16; idx += nthr) {
+        const int j = idx >> 4, cc = (idx >> 3) & 1, f = idx & 7;
+        const int fe = f ^ cc, a = (fe >> 1) + (fe & 1);
+        int jn = j + 2 - a;                                  // where an accepted move leads (dE = 8 - 4a)
+        uint32_t t = prm.table[j * 8 + fe];
+        if (jn < 0 || jn > N) { jn = j; t = 0u; }            // R17: cannot occur for a real configuration
+        char* const row = sm + (size_t)cc * V::K + (size_t)j * V::RS;
+        *reinterpret_cast<uint32_t*>(row + 4 * f) = t;
+        *reinterpret_cast<uint32_t*>(row + V::SA_OFF + 4 * f) = sbase + V::K + (uint32_t)jn * V::RS;
+    }
+    for (int idx = tid; idx < BINS * 2; idx += nthr)
+        *reinterpret_cast<uint32_t*>(sm + (size_t)(idx & 1) * V::K + (size_t)(idx >> 1) * V::RS + V::BIN_OFF) = 0u;
+    if (tid < 17)  // row BINS of copy 0: t = 0 and Sa = itself in every column -- a lane parked here stays here
+        *reinterpret_cast<uint32_t*>(sm + (size_t)BINS * V::RS + 4 * tid) = tid >= 8 && tid < 16 ? sbase + BINS * V::RS : 0u;
+
+    const bool is_walker = tid >= 32 * nw;
+    const int slot = is_walker ? tid - 32 * nw : tid;          // lattice / ring column
+    const int pair = slot >> 5, lane = slot & 31;
+    const int w = (blockIdx.x * nw + pair) * wpw + lane;
+    const bool active = lane < wpw && w < prm.W;
+    const int bar_id = 1 + pair;
+    uint32_t* const lat = reinterpret_cast<uint32_t*>(sm + V::LAT_OFF) + slot;
+    uint4* const ring = reinterpret_cast<uint4*>(sm + V::RING_OFF);
+
+    // ---- lattice: one word per row, column `slot`
+    if (is_walker) {
+        if (!active) {
+            for (int y = 0; y < L; ++y) lat[y * SLOTS] = 0u;
+        } else if (L >= 32) {
+            for (int y = 0; y < L; ++y) lat[y * SLOTS] = prm.spins[(size_t)y * prm.W + w];
+        } else {
+            constexpr int RPW = 32 / G::BITS;
+            for (int t = 0; t < N / 32; ++t) {
+                const uint32_t word = prm.spins[(size_t)t * prm.W + w];
+#pragma unroll
+                for (int q = 0; q < RPW; ++q) lat[(t * RPW + q) * SLOTS] = (word >> (q * G::BITS)) & G::MASK;
+            }
+        }
+    }
+    __syncthreads();
+
+    const uint32_t walker = prm.walker_offset + (uint32_t)w;
+    if (!is_walker) {
+        deviate_rows<L>(ring, SLOTS, slot, bar_id, prm, walker);
+    } else {
+        // slot j = (E + 2N)/4, copy 0
+        uint32_t S = sbase + (active ? (uint32_t)((prm.E[w] + 2 * N) >> 2) : (uint32_t)BINS) * V::RS;
+        const uint32_t s_th = prm.therm < prm.sweep_begin ? prm.sweep_begin
+                              : (prm.therm > prm.sweep_end ? prm.sweep_end : prm.therm);
+        int buf = 0;
+        sweeps_v5<L, false>(lat, S, prm.sweep_begin, s_th, ring + slot, buf, bar_id);
+        sweeps_v5<L, true>(lat, S, s_th, prm.sweep_end, ring + slot, buf, bar_id);
+        if (active) {
+            prm.E[w] = (int)(((S & ~V::K) - sbase) / V::RS) * 4 - 2 * N;
+            if (L >= 32) {
+                for (int y = 0; y < L; ++y) prm.spins[(size_t)y * prm.W + w] = lat[y * SLOTS];
+            } else {
+                constexpr int RPW = 32 / G::BITS;
+                for (int t = 0; t < N / 32; ++t) {
+                    uint32_t word = 0u;
+#pragma unroll
+                    for (int q = 0; q < RPW; ++q) word |= lat[(t * RPW + q) * SLOTS] << (q * G::BITS);
+                    prm.spins[(size_t)t * prm.W + w] = word;
+                }
+            }
+        }
+    }
+    __syncthreads();
+
+    // ---- a4: merge the two bins of every slot into the global uint64 histogram
+    if (prm.sweep_end > prm.therm) {
+        for (int j = tid; j < BINS; j += nthr) {
+            const uint32_t v = *reinterpret_cast<uint32_t*>(sm + (size_t)j * V::RS + V::BIN_OFF) +
+                               *reinterpret_cast<uint32_t*>(sm + (size_t)V::K + (size_t)j * V::RS + V::BIN_OFF);
+            if (v) atomicAdd(prm.H + j, (unsigned long long)v);
+        }
+    }
+}
+
+}  // namespace muca
