@@ -41,24 +41,37 @@ struct V5 {
     static constexpr size_t SMEM_BYTES = (size_t)K + TBL_BYTES;
 };
 
-// One site of the walker chain, in PTX so that the decision is consumed by SEL (ISETP -> SEL -> LDS is 9 cycles on
-// sm_100a, ISETP -> predicated instruction -> LDS is more, and ptxas prefers the latter when left to itself).
-//   S: state address (in/out)   A: entry address of this site (in), of the next site (out)
-//   g: 4 * column of the NEXT site   r: deviate   BIT: flip mask of this site
-#define MUCA_V5_SITE(HIST_LINE, EXTRA_LINE)                                      \
-    "{\n\t.reg .pred p;\n\t.reg .b32 t, sa, sr, aa, ar;\n\t"                    \
+// One site of the walker chain, in PTX.  Three things ptxas does not do by itself:
+//  * the decision must be consumed by a SEL: ISETP -> SEL -> (IADD ->) LDS costs 9 (13) cycles on sm_100a, ISETP ->
+//    predicated instruction -> LDS about 20 (profiles/r01_ubench_chain.txt).  ptxas turns "S = p ? sa : S & ~K" into a
+//    predicated AND unless the AND has a second, unconditional use: here it is the address of the histogram
+//    increment (the bin of copy 0 serves both copies);
+//  * the walker warp is a single in-order instruction stream whose ISETP blocks until the threshold arrives, so
+//    everything that does not depend on the decision should be issued BEFORE the ISETP, in the shadow of the
+//    27-cycle table load.  The predicate chain ps -> pg -> ISETP (LOP3 with a predicate output; both are true at
+//    run time: sr is a non-zero address) pins the ISETP behind the column extraction of the next site;
+//  * H[j]++ of the PREVIOUS attempt is issued behind this site's table loads (S still holds that state).
+//   %0 S: state address (in/out)    %1 A: entry address of this site (in), of the next site (out)
+//   %2 flips (in/out)   %3 FW[3] at site 0 (in/out)   %4 deviate   %5 field word of the NEXT site   %6 its shift
+//   %7 flip mask of this site   %8 ~K   %9 patch (site 0)
+#define MUCA_V5_SITE(SHIFT_OP, EXTRA_LINE)                                       \
+    "{\n\t.reg .pred p, ps, pg;\n\t.reg .b32 t, sa, sr, g0, g;\n\t"               \
     "ld.shared.u32 t, [%1];\n\t"                                                 \
-    "ld.shared.u32 sa, [%1+32];\n\t" HIST_LINE                                   \
-    "and.b32 sr, %0, %7;\n\t"                                                    \
-    "add.u32 ar, sr, %5;\n\t"                                                    \
-    "add.u32 aa, sa, %5;\n\t"                                                    \
-    "setp.le.u32 p, %4, t;\n\t"                                                  \
-    "selp.u32 %1, aa, ar, p;\n\t"                                                \
+    "ld.shared.u32 sa, [%1+32];\n\t"                                             \
+    "setp.eq.u32 ps, 0, 0;\n\t"                                                  \
+    "lop3.and.b32 sr|ps, %0, %8, 0, 0xC0, ps;\n\t"                               \
+    "red.shared.add.u32 [sr+64], 1;\n\t"                                         \
+    SHIFT_OP " g0, %5, %6;\n\t"                                                  \
+    "lop3.or.b32 g|pg, g0, 0x1C, 0, 0xC0, ps;\n\t"                               \
+    "setp.le.and.u32 p, %4, t, pg;\n\t"                                          \
     "selp.u32 %0, sa, sr, p;\n\t"                                                \
-    "@p or.b32 %2, %2, %6;\n\t" EXTRA_LINE "}"
+    "add.u32 %1, %0, g;\n\t"                                                     \
+    "@p or.b32 %2, %2, %7;\n\t" EXTRA_LINE "}"
 
 // Walker warp: sweeps s0 .. s1-1; `buf` is the ring buffer holding the deviates of the next row to process.
-template <int L, bool MEAS>
+// Every site increments the bin of the state it STARTS from, i.e. of the state after the previous attempt; the
+// caller compensates the first and the last attempt of the measured phase.
+template <int L>
 __device__ __forceinline__ void sweeps_v5(uint32_t* __restrict__ lat, uint32_t& S, const uint32_t s0, const uint32_t s1,
                                           const uint4* __restrict__ ring, int& buf, const int bar_id) {
     using G = Geo<L>;
@@ -82,35 +95,56 @@ __device__ __forceinline__ void sweeps_v5(uint32_t* __restrict__ lat, uint32_t& 
             buf ^= 1;
             S &= ~V::K;                        // site 0: its left neighbour (site L-1) has not been visited in this sweep
             uint32_t A = S + ((FW[0] << 2) & 0x1Cu);
-            uint32_t flips = 0, unused = 0;   // `unused` fills operand %3 of the site macro where site 0 has FW[3]
+            uint32_t flips = 0, unused = 0;    // `unused` fills operand %3 of the site macro where site 0 has FW[3]
 #pragma unroll
             for (int x = 0; x < BITS; ++x) {
+                // column of the next site: nibble qn of FW[xn & 3], moved to bits 2..4 inside the site block
                 const int xn = x + 1, qn = xn >> 2;
-                uint32_t g = 0;                // 4 * column of the next site
-                if (xn < BITS) {
-                    if (qn == 0) g = (FW[xn & 3] << 2) & 0x1Cu;
-                    else if (qn == 1) g = (FW[xn & 3] >> 2) & 0x1Cu;
-                    else g = (FW[xn & 3] >> (4 * qn - 2)) & 0x1Cu;
-                }
-                // H[j]++ of the PREVIOUS site is issued behind this site's table loads (S still holds that state)
-                if (x == 0) {                  // site 0 also patches the last site's column: its right neighbour is site 0
-                    asm volatile(MUCA_V5_SITE("", "@p add.u32 %3, %3, %8;\n\t")
+                const uint32_t fwn = xn < BITS ? FW[xn & 3] : 0u;
+                const uint32_t sh = qn == 0 ? 2u : (uint32_t)(4 * qn - 2);
+                if (x == 0)                    // site 0 also patches the last site's column: its right neighbour is site 0
+                    asm volatile(MUCA_V5_SITE("shl.b32", "@p add.u32 %3, %3, %9;\n\t")
                                  : "+r"(S), "+r"(A), "+r"(flips), "+r"(FW[3])
-                                 : "r"(rnd[x]), "r"(g), "r"(1u), "n"(~V::K), "r"(patch));
-                } else if (MEAS) {
-                    asm volatile(MUCA_V5_SITE("red.shared.add.u32 [%0+64], 1;\n\t", "")
+                                 : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u), "n"(~V::K), "r"(patch) : "memory");
+                else if (qn == 0)
+                    asm volatile(MUCA_V5_SITE("shl.b32", "")
                                  : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused)
-                                 : "r"(rnd[x]), "r"(g), "r"(1u << (x & 31)), "n"(~V::K)
-                                 : "memory");
-                } else {
-                    asm volatile(MUCA_V5_SITE("", "")
+                                 : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u << (x & 31)), "n"(~V::K) : "memory");
+                else
+                    asm volatile(MUCA_V5_SITE("shr.u32", "")
                                  : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused)
-                                 : "r"(rnd[x]), "r"(g), "r"(1u << (x & 31)), "n"(~V::K));
-                }
+                                 : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u << (x & 31)), "n"(~V::K) : "memory");
             }
-            if (MEAS)                          // H[j]++ after EVERY attempt: the last site of the row
-                asm volatile("red.shared.add.u32 [%0+64], 1;" ::"r"(S) : "memory");
             lat[y * SLOTS] = c ^ flips;
+        }
+    }
+}
+
+// Deviate warp: the NC Philox calls of one row advance round-major (NC independent IMAD.WIDE chains), results go to
+// the double-buffered shared ring rnd[buf][call][slot] as one 16-byte store per call.  One barrier per row hands
+// the buffer over.  R4: ctr = (i >> 2, sweep, iteration, walker).
+template <int L>
+__device__ __forceinline__ void deviates_v5(uint4* __restrict__ ring, const uint32_t s0, const uint32_t s1, int& buf,
+                                            const int bar_id, const SweepParams& prm, const uint32_t walker) {
+    constexpr int NC = V5<L>::NC, SLOTS = V5<L>::SLOTS;
+#pragma unroll 1
+    for (uint32_t s = s0; s < s1; ++s) {
+#pragma unroll 1
+        for (int y = 0; y < L; ++y) {
+            uint32_t st[NC][4];
+#pragma unroll
+            for (int k = 0; k < NC; ++k) {
+                st[k][0] = (uint32_t)(y * (L / 4) + k); st[k][1] = s; st[k][2] = prm.iteration; st[k][3] = walker;
+            }
+#pragma unroll
+            for (int r = 0; r < 10; ++r)
+#pragma unroll
+                for (int k = 0; k < NC; ++k)
+                    philox_round(st[k], prm.key0 + (uint32_t)r * 0x9E3779B9u, prm.key1 + (uint32_t)r * 0xBB67AE85u);
+#pragma unroll
+            for (int k = 0; k < NC; ++k) ring[(buf * NC + k) * SLOTS] = make_uint4(st[k][0], st[k][1], st[k][2], st[k][3]);
+            pair_barrier(bar_id);
+            buf ^= 1;
         }
     }
 }
@@ -175,16 +209,27 @@ __global__ void __launch_bounds__(64 * V5<L>::MAX_WARPS, 1) sweep_kernel_v5(cons
     __syncthreads();
 
     const uint32_t walker = prm.walker_offset + (uint32_t)w;
-    if (!is_walker) {
-        deviate_rows<L>(ring, SLOTS, slot, bar_id, prm, walker);
+    const uint32_t s_th = prm.therm < prm.sweep_begin ? prm.sweep_begin
+                          : (prm.therm > prm.sweep_end ? prm.sweep_end : prm.therm);
+    // slot j = (E + 2N)/4, copy 0
+    uint32_t S = sbase + (is_walker && active ? (uint32_t)((prm.E[w] + 2 * N) >> 2) : (uint32_t)BINS) * V::RS;
+    int buf = 0;
+    // ---- thermalisation sweeps: same code, the bins are cleared afterwards
+    if (is_walker) sweeps_v5<L>(lat, S, prm.sweep_begin, s_th, ring + slot, buf, bar_id);
+    else deviates_v5<L>(ring + slot, prm.sweep_begin, s_th, buf, bar_id, prm, walker);
+    __syncthreads();
+    for (int j = tid; j <= BINS; j += nthr) *reinterpret_cast<uint32_t*>(sm + (size_t)j * V::RS + V::BIN_OFF) = 0u;
+    __syncthreads();
+    // ---- measured sweeps: every site counts the state it starts from, so the state before the first measured
+    //      attempt is taken out again here and the state after the last one is added below
+    if (is_walker) {
+        if (s_th < prm.sweep_end) atomicSub(reinterpret_cast<uint32_t*>(sm + ((S & ~V::K) - sbase) + V::BIN_OFF), 1u);
+        sweeps_v5<L>(lat, S, s_th, prm.sweep_end, ring + slot, buf, bar_id);
+        if (s_th < prm.sweep_end) atomicAdd(reinterpret_cast<uint32_t*>(sm + ((S & ~V::K) - sbase) + V::BIN_OFF), 1u);
     } else {
-        // slot j = (E + 2N)/4, copy 0
-        uint32_t S = sbase + (active ? (uint32_t)((prm.E[w] + 2 * N) >> 2) : (uint32_t)BINS) * V::RS;
-        const uint32_t s_th = prm.therm < prm.sweep_begin ? prm.sweep_begin
-                              : (prm.therm > prm.sweep_end ? prm.sweep_end : prm.therm);
-        int buf = 0;
-        sweeps_v5<L, false>(lat, S, prm.sweep_begin, s_th, ring + slot, buf, bar_id);
-        sweeps_v5<L, true>(lat, S, s_th, prm.sweep_end, ring + slot, buf, bar_id);
+        deviates_v5<L>(ring + slot, s_th, prm.sweep_end, buf, bar_id, prm, walker);
+    }
+    if (is_walker) {
         if (active) {
             prm.E[w] = (int)(((S & ~V::K) - sbase) / V::RS) * 4 - 2 * N;
             if (L >= 32) {
@@ -202,11 +247,10 @@ __global__ void __launch_bounds__(64 * V5<L>::MAX_WARPS, 1) sweep_kernel_v5(cons
     }
     __syncthreads();
 
-    // ---- a4: merge the two bins of every slot into the global uint64 histogram
+    // ---- a4: merge the block's bins into the global uint64 histogram
     if (prm.sweep_end > prm.therm) {
         for (int j = tid; j < BINS; j += nthr) {
-            const uint32_t v = *reinterpret_cast<uint32_t*>(sm + (size_t)j * V::RS + V::BIN_OFF) +
-                               *reinterpret_cast<uint32_t*>(sm + (size_t)V::K + (size_t)j * V::RS + V::BIN_OFF);
+            const uint32_t v = *reinterpret_cast<uint32_t*>(sm + (size_t)j * V::RS + V::BIN_OFF);
             if (v) atomicAdd(prm.H + j, (unsigned long long)v);
         }
     }
