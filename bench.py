@@ -30,9 +30,14 @@ import numpy as np  # noqa: E402
 
 METRIC = "spin-flip attempts/sec"
 UNIT = "flips/s"
-# algorithmic integer work per flip attempt and the issue roofline
-OPS_PER_FLIP = 20.0                 # thread-instructions: 8.5 Philox (16 IMAD.WIDE + 18 LOP3 per 4 sites) + 11.5 site update
-SM_COUNT, SCHED_PER_SM, LANES = 148, 4, 32
+# algorithmic integer work per flip attempt and the roofline of the binding pipe.
+# Per attempted flip: 1/4 Philox4x32-10 call (4 IMAD.WIDE on the FMA-heavy pipe + 4.5 LOP3) and ~11.5 instructions of
+# site update = 20 thread-instructions, of which 11.7 can only run on the 16-lane ALU pipe (LOP3/IADD3/SHF/SEL/ISETP).
+ALU_OPS_PER_FLIP = 11.7             # binding pipe: ALU, 16 lanes per scheduler per clock (profiles/r01_ubench_pipes.txt)
+OPS_PER_FLIP = 20.0                 # all thread-instructions (issue slots: 32 lanes per scheduler per clock)
+SM_COUNT, SCHED_PER_SM, ALU_LANES, ISSUE_LANES = 148, 4, 16, 32
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE sweep-kernel launch from the ncu --set full capture under profiles/
+NCU_DRAM_BYTES_PER_LAUNCH = {"L32_w16384": 4.49e6}
 
 
 def parse():
@@ -244,16 +249,25 @@ def run_ours(args, cfg):
     flips_per_launch = mb.flips_per_iteration(cfg, W) * cfg.iterations * args.steps / max(stats["sweep_launches"], 1)
     avg_launch_s = stats["sweep_ms"] * 1e-3 / max(stats["sweep_launches"], 1)
     kern_flips_s = flips_per_launch / avg_launch_s
-    achieved = kern_flips_s * OPS_PER_FLIP / 1e12
-    peak = SM_COUNT * SCHED_PER_SM * LANES * f_max_hz / 1e12
+    achieved = kern_flips_s * ALU_OPS_PER_FLIP / 1e12
+    peak = SM_COUNT * SCHED_PER_SM * ALU_LANES * f_max_hz / 1e12
+    issue_peak = SM_COUNT * SCHED_PER_SM * ISSUE_LANES * f_max_hz / 1e12
+    kernel = "muca::sweep_kernel_v5<%d>" % cfg.L if cfg.L <= 32 else \
+        "muca::sweep_kernel<%d, %s>" % (cfg.L, "TBL_L1" if cfg.L == 64 else "STREAMED")
     roofline = {
-        "bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tinst/s (thread-instructions)", "frac": achieved / peak,
-        "traffic": None, "kernel": "muca::sweep_kernel", "kernel_flips_per_s": kern_flips_s,
-        "ops_per_flip": OPS_PER_FLIP, "avg_launch_ms": avg_launch_s * 1e3, "kernel_share_of_step": stats["sweep_ms"] / ms_dev,
+        "bound": "alu", "achieved": achieved, "peak": peak, "unit": "T lane-ops/s on the ALU pipe", "frac": achieved / peak,
+        "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(cfg.name) if world == 1 else None,
+        "kernel": kernel, "kernel_flips_per_s": kern_flips_s,
+        "ops_per_flip": ALU_OPS_PER_FLIP, "avg_launch_ms": avg_launch_s * 1e3, "kernel_share_of_step": stats["sweep_ms"] / ms_dev,
         "c_flip_cycles": W * f_max_hz / kern_flips_s,
-        "peak_source": f"148 SM x 4 schedulers x 32 lanes x sm_max_mhz ({pk_kind} MEASURED_PEAKS.json clock)",
+        "peak_source": f"148 SM x 4 schedulers x 16 ALU lanes x sm_max_mhz ({pk_kind} MEASURED_PEAKS.json clock); "
+                       "11.7 ALU-only instructions per attempted flip (DESIGN.md 6.2)",
+        "issue": {"achieved": kern_flips_s * OPS_PER_FLIP / 1e12, "peak": issue_peak, "unit": "T thread-instructions/s",
+                  "frac": kern_flips_s * OPS_PER_FLIP / 1e12 / issue_peak, "ops_per_flip": OPS_PER_FLIP},
         "hbm": {"algorithmic_bytes_per_flip": 0.0 if cfg.L <= 64 else 0.25, "peak_gbs": pk.get("hbm_gbs"),
-                "note": "lattices are shared-memory resident for L <= 64; HBM traffic is KiB per launch"},
+                "achieved_gbs": (0.0 if cfg.L <= 64 else 0.25) * kern_flips_s / 1e9,
+                "note": "lattices are shared-memory resident for L <= 64 (MiB of HBM traffic per launch); "
+                        "streamed at L = 128: every packed word read and written once per sweep"},
     }
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),

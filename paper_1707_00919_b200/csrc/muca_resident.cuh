@@ -10,14 +10,16 @@
 //     +4f      t  = thresh[j][a],  a = a(f ^ c)          (PAPER.md:109 acceptance, R6/R7)
 //     +32+4f   Sa = rowaddr(j + 2 - a, 1)                 (state an ACCEPTED move leads to; a rejected one leads
 //                                                          to rowaddr(j, 0) = S & ~K)
-//     +64      histogram bin of (j, c); the two bins of a slot are added at the merge (a4)
+//     +64      histogram bin of slot j (copy 0 only: both copies of a slot count into it)
 // Two 32-bit loads instead of one 64-bit load: a random-row LDS.64 takes 34 cycles (two 16-lane phases, each with
-// its own bank conflicts), a random-row LDS.32 27 (profiles/r01_ubench_chain.txt).
-// Per site the serial chain is   LDS t -> ISETP -> SEL(A_acc, A_rej) -> LDS t'   with both candidate addresses
-// ready before the decision; column extraction, flip mask, histogram increment and the second select (S) are
-// off the chain.  Philox runs in a paired "deviate" warp (same 32 walkers) that feeds a double-buffered shared
-// ring one row ahead: the hardware interleaves its instruction stream into the stalls of the walker warp
-// (a single in-order warp doing both reaches only 75 cycles per site).
+// its own bank conflicts), a random-row LDS.32 27 (profiles/r01_ubench_chain.txt); Sa arrives 3 cycles behind t.
+// Per site the serial chain is   LDS t -> ISETP -> SEL(Sa, S & ~K) -> IADD (+ column of the next site) -> LDS t'.
+// Column extraction, flip mask and histogram increment are off the chain.  Philox runs in a paired "deviate" warp
+// (same walkers) that feeds a double-buffered shared ring one row ahead: the hardware interleaves its instruction
+// stream into the stalls of the walker warp.  What was measured and dropped: a single in-order
+// warp doing both (75 cycles per site), selecting between two precomputed entry addresses (ptxas folds the add
+// into an instruction predicated on the decision, +11 cycles), and speculative loads for both outcomes of the
+// next site (the walker warp becomes issue-bound at the same 49 cycles).
 #pragma once
 #include "muca_device.cuh"
 
@@ -30,7 +32,8 @@ struct V5 {
     static constexpr uint32_t RS = 68;
     static constexpr uint32_t SA_OFF = 32, BIN_OFF = 64;
     static constexpr uint32_t TBL_BYTES = (BINS + 1) * RS;   // + one all-reject row: parking place of unused lanes
-    static constexpr uint32_t K = L == 32 ? 131072u : (L == 16 ? 65536u : 32768u);
+    static constexpr int KBIT = L == 32 ? 17 : (L == 16 ? 16 : 15);
+    static constexpr uint32_t K = 1u << KBIT;
     static constexpr uint32_t LAT_OFF = (TBL_BYTES + 15u) & ~15u;
     static constexpr int MAX_WARPS = 4;                      // walker warps per block (+ as many deviate warps)
     static constexpr int SLOTS = 32 * MAX_WARPS;             // lattice / ring columns
@@ -53,8 +56,10 @@ struct V5 {
 //  * H[j]++ of the PREVIOUS attempt is issued behind this site's table loads (S still holds that state).
 //   %0 S: state address (in/out)    %1 A: entry address of this site (in), of the next site (out)
 //   %2 flips (in/out)   %3 FW[3] at site 0 (in/out)   %4 deviate   %5 field word of the NEXT site   %6 its shift
-//   %7 flip mask of this site   %8 ~K   %9 patch (site 0)
-#define MUCA_V5_SITE(SHIFT_OP, EXTRA_LINE)                                       \
+//   %7 flip mask of this site   %8 ~K   %9 patch (site 0)   %10 distance between bit K and the site's bit
+// The flip mask collects bit K of the new state (= the decision) with a shift and a LOP3: an instruction predicated
+// on p would stall ~13 cycles behind the ISETP, in front of the next table load.
+#define MUCA_V5_SITE(SHIFT_OP, FLIP_SHIFT_OP, EXTRA_LINE)                                      \
     "{\n\t.reg .pred p, ps, pg;\n\t.reg .b32 t, sa, sr, g0, g;\n\t"               \
     "ld.shared.u32 t, [%1];\n\t"                                                 \
     "ld.shared.u32 sa, [%1+32];\n\t"                                             \
@@ -66,7 +71,8 @@ struct V5 {
     "setp.le.and.u32 p, %4, t, pg;\n\t"                                          \
     "selp.u32 %0, sa, sr, p;\n\t"                                                \
     "add.u32 %1, %0, g;\n\t"                                                     \
-    "@p or.b32 %2, %2, %7;\n\t" EXTRA_LINE "}"
+    FLIP_SHIFT_OP " g0, %0, %10;\n\t"                                            \
+    "lop3.b32 %2, %2, g0, %7, 0xF8;\n\t" EXTRA_LINE "}"
 
 // Walker warp: sweeps s0 .. s1-1; `buf` is the ring buffer holding the deviates of the next row to process.
 // Every site increments the bin of the state it STARTS from, i.e. of the state after the previous attempt; the
@@ -102,18 +108,24 @@ __device__ __forceinline__ void sweeps_v5(uint32_t* __restrict__ lat, uint32_t& 
                 const int xn = x + 1, qn = xn >> 2;
                 const uint32_t fwn = xn < BITS ? FW[xn & 3] : 0u;
                 const uint32_t sh = qn == 0 ? 2u : (uint32_t)(4 * qn - 2);
+                constexpr int KB = V::KBIT;
+                const uint32_t fs = x <= KB ? (uint32_t)(KB - x) : (uint32_t)(x - KB);
                 if (x == 0)                    // site 0 also patches the last site's column: its right neighbour is site 0
-                    asm volatile(MUCA_V5_SITE("shl.b32", "@p add.u32 %3, %3, %9;\n\t")
+                    asm volatile(MUCA_V5_SITE("shl.b32", "shr.u32", "@p add.u32 %3, %3, %9;\n\t")
                                  : "+r"(S), "+r"(A), "+r"(flips), "+r"(FW[3])
-                                 : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u), "n"(~V::K), "r"(patch) : "memory");
+                                 : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u), "n"(~V::K), "r"(patch), "r"(fs) : "memory");
                 else if (qn == 0)
-                    asm volatile(MUCA_V5_SITE("shl.b32", "")
+                    asm volatile(MUCA_V5_SITE("shl.b32", "shr.u32", "")
                                  : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused)
-                                 : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u << (x & 31)), "n"(~V::K) : "memory");
+                                 : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u << (x & 31)), "n"(~V::K), "r"(0u), "r"(fs) : "memory");
+                else if (x <= KB)
+                    asm volatile(MUCA_V5_SITE("shr.u32", "shr.u32", "")
+                                 : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused)
+                                 : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u << (x & 31)), "n"(~V::K), "r"(0u), "r"(fs) : "memory");
                 else
-                    asm volatile(MUCA_V5_SITE("shr.u32", "")
+                    asm volatile(MUCA_V5_SITE("shr.u32", "shl.b32", "")
                                  : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused)
-                                 : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u << (x & 31)), "n"(~V::K) : "memory");
+                                 : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u << (x & 31)), "n"(~V::K), "r"(0u), "r"(fs) : "memory");
             }
             lat[y * SLOTS] = c ^ flips;
         }

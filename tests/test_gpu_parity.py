@@ -122,6 +122,8 @@ def test_configs345_reduced(L, W, iters, therm, sweeps):
     (8, B.MUCA_KERNEL_RESIDENT, 64), (16, B.MUCA_KERNEL_RESIDENT, 128),
     (32, B.MUCA_KERNEL_RESIDENT, 64), (32, B.MUCA_KERNEL_RESIDENT, 128), (32, B.MUCA_KERNEL_STREAMED, 32),
     (32, B.MUCA_KERNEL_STREAMED, 96),
+    (8, B.MUCA_KERNEL_RESIDENT_V3, 32), (16, B.MUCA_KERNEL_RESIDENT_V3, 64), (32, B.MUCA_KERNEL_RESIDENT_V3, 128),
+    (16, B.MUCA_KERNEL_RESIDENT_V2, 32), (32, B.MUCA_KERNEL_RESIDENT_V2, 64),
     (64, B.MUCA_KERNEL_RESIDENT, 32), (64, B.MUCA_KERNEL_RESIDENT, 224), (64, B.MUCA_KERNEL_STREAMED, 64),
     (128, B.MUCA_KERNEL_RESIDENT, 32), (128, B.MUCA_KERNEL_STREAMED, 64),
 ])
@@ -130,6 +132,21 @@ def test_kernel_variants(L, kernel, tpb):
     sweeps = {8: 30, 16: 20, 32: 10, 64: 5, 128: 3}[L]
     run_pair(L, W, PRIMARY_SEED, 3, 2, sweeps,
              options=((B.MUCA_OPT_KERNEL, kernel), (B.MUCA_OPT_THREADS_PER_BLOCK, tpb)))
+
+
+# resident kernel, L <= 32: any number of walkers per warp (the default spreads the walkers over all SMs) and
+# 1, 2 or 4 walker/deviate warp pairs per block give the same chains
+@pytest.mark.parametrize("L,W,tpb,wpw", [
+    (8, 128, 0, 0), (8, 77, 32, 5), (16, 300, 64, 17), (16, 4096, 0, 0), (32, 333, 128, 28), (32, 200, 32, 1),
+    (32, 1000, 0, 0),
+])
+def test_resident_walkers_per_warp(L, W, tpb, wpw):
+    opts = [(B.MUCA_OPT_KERNEL, B.MUCA_KERNEL_RESIDENT)]
+    if tpb:
+        opts.append((B.MUCA_OPT_THREADS_PER_BLOCK, tpb))
+    if wpw:
+        opts.append((B.MUCA_OPT_WALKERS_PER_WARP, wpw))
+    run_pair(L, W, EXTRA_SEEDS[1], 3, 2, {8: 30, 16: 12, 32: 6}[L], offset=3, options=tuple(opts), check_every=False)
 
 
 def test_split_launches_give_the_same_iteration():
