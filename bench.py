@@ -37,7 +37,7 @@ ALU_OPS_PER_FLIP = 11.7             # binding pipe: ALU, 16 lanes per scheduler 
 OPS_PER_FLIP = 20.0                 # all thread-instructions (issue slots: 32 lanes per scheduler per clock)
 SM_COUNT, SCHED_PER_SM, ALU_LANES, ISSUE_LANES = 148, 4, 16, 32
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE sweep-kernel launch from the ncu --set full capture under profiles/
-NCU_DRAM_BYTES_PER_LAUNCH = {"L32_w16384": 4.49e6}
+NCU_DRAM_BYTES_PER_LAUNCH = {"L32_w16384": 2.24e6}
 
 
 def parse():
