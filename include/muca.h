@@ -53,11 +53,13 @@ typedef enum muca_status {
 } muca_status;
 
 /* Sweep-kernel variants (muca_set_option(ctx, MUCA_OPT_KERNEL, ...)).
- * AUTO picks RESIDENT when the packed lattices of one block plus the tables fit in
- * shared memory (L <= 64) and STREAMED otherwise (L = 128). */
+ * AUTO picks RESIDENT for L <= 32 (lattices, threshold table and histogram in shared memory),
+ * STREAMED_SMEM for L = 64 (table and histogram in shared memory, lattice rows streamed from HBM/L2)
+ * and STREAMED for L = 128 (the table no longer fits: thresholds through L1). */
 enum { MUCA_KERNEL_AUTO = 0, MUCA_KERNEL_RESIDENT = 1, MUCA_KERNEL_STREAMED = 2,
        MUCA_KERNEL_RESIDENT_V2 = 3, /* L <= 32 only: the earlier predicate-carried resident kernel, kept for A/B runs */
-       MUCA_KERNEL_RESIDENT_V3 = 4  /* L <= 32 only: the earlier paired walker/deviate-warp kernel, kept for A/B runs */ };
+       MUCA_KERNEL_RESIDENT_V3 = 4, /* L <= 32 only: the earlier paired walker/deviate-warp kernel, kept for A/B runs */
+       MUCA_KERNEL_STREAMED_SMEM = 5 /* L = 32, 64: lattice rows streamed, threshold table + histogram in shared memory */ };
 enum {
     MUCA_OPT_KERNEL = 1,          /* one of MUCA_KERNEL_*                                        */
     MUCA_OPT_THREADS_PER_BLOCK = 2, /* walkers (= threads) per block; 0 = library default         */

@@ -163,13 +163,14 @@ Plan make_plan(const muca_ctx* c) {
     Plan p;
     const int L = c->L;
     int kern = c->opt_kernel;
-    if (kern == MUCA_KERNEL_AUTO) kern = L <= 64 ? MUCA_KERNEL_RESIDENT : MUCA_KERNEL_STREAMED;
+    if (kern == MUCA_KERNEL_AUTO) kern = L <= 32 ? MUCA_KERNEL_RESIDENT : (L == 64 ? MUCA_KERNEL_STREAMED_SMEM : MUCA_KERNEL_STREAMED);
     if (kern == MUCA_KERNEL_STREAMED && L < 32) kern = MUCA_KERNEL_RESIDENT;
     if ((kern == MUCA_KERNEL_RESIDENT_V2 || kern == MUCA_KERNEL_RESIDENT_V3) && L > 32) kern = MUCA_KERNEL_RESIDENT;
     p.nw = p.wpw = 0;
     if (kern == MUCA_KERNEL_RESIDENT) p.mode = L <= 32 ? MODE_V5 : MODE_TBL_L1;
     else if (kern == MUCA_KERNEL_RESIDENT_V3) p.mode = MODE_V3;
     else if (kern == MUCA_KERNEL_RESIDENT_V2) p.mode = MODE_TBL_SMEM;
+    else if (kern == MUCA_KERNEL_STREAMED_SMEM) p.mode = L >= 32 ? MODE_STREAMED_SMEM : MODE_V5;
     else p.mode = MODE_STREAMED;
     if (p.mode == MODE_V5) {
         // spread the walkers over all SMs: as few warps per SM as possible, then as few lanes per warp as possible
@@ -190,6 +191,12 @@ Plan make_plan(const muca_ctx* c) {
         if (p.mode == MODE_V3) tpb = L == 32 ? 128 : 32;
         else if (p.mode == MODE_TBL_SMEM) tpb = 32;
         else if (p.mode == MODE_TBL_L1) tpb = L == 64 ? 64 : 32;
+        else if (p.mode == MODE_STREAMED_SMEM) {
+            // one block per SM (164 KB of table at L = 64): spread the walkers over all SMs
+            const int n_sm = c->n_sm > 0 ? c->n_sm : 148;
+            tpb = ((c->W + n_sm - 1) / n_sm + 31) / 32 * 32;
+            if (tpb > 512) tpb = 512;
+        }
         else tpb = 32;
     }
     p.tpb = tpb;
@@ -202,12 +209,15 @@ size_t plan_smem(int L, const Plan& p) {
     switch (L) {
         case 8: return sweep_smem_bytes<8, MODE_TBL_SMEM>(p.tpb);
         case 16: return sweep_smem_bytes<16, MODE_TBL_SMEM>(p.tpb);
-        case 32: return p.mode == MODE_TBL_SMEM ? sweep_smem_bytes<32, MODE_TBL_SMEM>(p.tpb)
+        case 32: return p.mode == MODE_STREAMED_SMEM ? sweep_smem_bytes<32, MODE_STREAMED_SMEM>(p.tpb)
+                        : p.mode == MODE_TBL_SMEM ? sweep_smem_bytes<32, MODE_TBL_SMEM>(p.tpb)
                         : p.mode == MODE_TBL_L1 ? sweep_smem_bytes<32, MODE_TBL_L1>(p.tpb)
                                                 : sweep_smem_bytes<32, MODE_STREAMED>(p.tpb);
         case 64: return p.mode == MODE_STREAMED ? sweep_smem_bytes<64, MODE_STREAMED>(p.tpb)
+                        : p.mode == MODE_STREAMED_SMEM ? sweep_smem_bytes<64, MODE_STREAMED_SMEM>(p.tpb)
                                                 : sweep_smem_bytes<64, MODE_TBL_L1>(p.tpb);
-        default: return p.mode == MODE_STREAMED ? sweep_smem_bytes<128, MODE_STREAMED>(p.tpb)
+        default: return p.mode == MODE_STREAMED_SMEM ? sweep_smem_bytes<128, MODE_STREAMED_SMEM>(p.tpb)
+                        : p.mode == MODE_STREAMED ? sweep_smem_bytes<128, MODE_STREAMED>(p.tpb)
                                                 : sweep_smem_bytes<128, MODE_TBL_L1>(p.tpb);
     }
 }
@@ -233,12 +243,15 @@ int launch_sweep(muca_ctx* ctx, const SweepParams& prm, const Plan& p) {
         case 16: return launch_sweep_t<16, MODE_TBL_SMEM>(ctx, prm, p.tpb);
         case 32:
             if (p.mode == MODE_TBL_SMEM) return launch_sweep_t<32, MODE_TBL_SMEM>(ctx, prm, p.tpb);
+            if (p.mode == MODE_STREAMED_SMEM) return launch_sweep_t<32, MODE_STREAMED_SMEM>(ctx, prm, p.tpb);
             if (p.mode == MODE_TBL_L1) return launch_sweep_t<32, MODE_TBL_L1>(ctx, prm, p.tpb);
             return launch_sweep_t<32, MODE_STREAMED>(ctx, prm, p.tpb);
         case 64:
             if (p.mode == MODE_STREAMED) return launch_sweep_t<64, MODE_STREAMED>(ctx, prm, p.tpb);
+            if (p.mode == MODE_STREAMED_SMEM) return launch_sweep_t<64, MODE_STREAMED_SMEM>(ctx, prm, p.tpb);
             return launch_sweep_t<64, MODE_TBL_L1>(ctx, prm, p.tpb);
         case 128:
+            if (p.mode == MODE_STREAMED_SMEM) return fail(ctx, MUCA_EINVAL, "L=128: the threshold table does not fit in shared memory");
             if (p.mode == MODE_STREAMED) return launch_sweep_t<128, MODE_STREAMED>(ctx, prm, p.tpb);
             return launch_sweep_t<128, MODE_TBL_L1>(ctx, prm, p.tpb);
     }
@@ -330,7 +343,7 @@ void muca_destroy(muca_ctx* ctx) {
 int muca_set_option(muca_ctx* ctx, int option, int value) {
     if (!ctx) return MUCA_EINVAL;
     if (option == MUCA_OPT_KERNEL) {
-        if (value < MUCA_KERNEL_AUTO || value > MUCA_KERNEL_RESIDENT_V3) return fail(ctx, MUCA_EINVAL, "bad kernel %d", value);
+        if (value < MUCA_KERNEL_AUTO || value > MUCA_KERNEL_STREAMED_SMEM) return fail(ctx, MUCA_EINVAL, "bad kernel %d", value);
         ctx->opt_kernel = value;
         return MUCA_OK;
     }

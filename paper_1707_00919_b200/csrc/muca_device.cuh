@@ -184,7 +184,11 @@ struct SweepParams {
     uint32_t therm;             // sweeps with index < therm are not recorded
 };
 
-enum { MODE_TBL_SMEM = 0, MODE_TBL_L1 = 1, MODE_STREAMED = 2, MODE_V3 = 3, MODE_V5 = 4 };
+enum { MODE_TBL_SMEM = 0, MODE_TBL_L1 = 1, MODE_STREAMED = 2, MODE_V3 = 3, MODE_V5 = 4, MODE_STREAMED_SMEM = 5 };
+//   5  STREAMED_SMEM  table + histogram in shared memory as in 0, lattice rows streamed as in 2: the lattices no longer
+//                     limit the walkers per SM, so that 8 warps share an SM at L = 64 (164 KB of table) (L = 64)
+__host__ __device__ constexpr bool tbl_in_smem(int mode) { return mode == MODE_TBL_SMEM || mode == MODE_STREAMED_SMEM; }
+__host__ __device__ constexpr bool lat_streamed(int mode) { return mode == MODE_STREAMED || mode == MODE_STREAMED_SMEM; }
 
 template <int L>
 struct Geo {
@@ -310,7 +314,7 @@ __device__ __forceinline__ void process_row(const uint32_t (&up)[Geo<L>::WPR], u
                                             uint32_t* __restrict__ hist) {
     using G = Geo<L>;
     constexpr int WPR = G::WPR, BITS = G::BITS;
-    constexpr uint32_t RS = (MODE == MODE_TBL_SMEM ? ROW_SMEM_WORDS : ROW_L1_WORDS) * 4;  // row stride in bytes
+    constexpr uint32_t RS = (tbl_in_smem(MODE) ? ROW_SMEM_WORDS : ROW_L1_WORDS) * 4;  // row stride in bytes
     // byte f of (LUT_HI:LUT_LO) = RS * a(f), a(f) = (f >> 1) + (f & 1) = antiparallel neighbours of column f
     constexpr uint32_t LUT_LO = (RS * 0) | (RS * 1) << 8 | (RS * 1) << 16 | (RS * 2) << 24;
     constexpr uint32_t LUT_HI = (RS * 2) | (RS * 3) << 8 | (RS * 3) << 16 | (RS * 4) << 24;
@@ -348,7 +352,7 @@ __device__ __forceinline__ void process_row(const uint32_t (&up)[Geo<L>::WPR], u
         }
     }
 
-    if constexpr (MODE == MODE_TBL_SMEM) {
+    if constexpr (tbl_in_smem(MODE)) {
         // o is the absolute shared-memory address of the walker's table row (see site_group_smem)
         uint32_t rp = 1u, tp = 0u;   // "previous site did not flip": site 0's left neighbour is site L-1, not yet visited
 #pragma unroll
@@ -671,9 +675,9 @@ __device__ __forceinline__ void st_row(uint32_t* p, const uint32_t (&r)[WPR]) {
 template <int L, int MODE>
 __host__ __device__ constexpr size_t sweep_smem_bytes(int tpb) {
     using G = Geo<L>;
-    const size_t tbl = MODE == MODE_TBL_SMEM ? (size_t)G::BINS * ROW_SMEM_WORDS * 4 : (size_t)G::BINS * 4;
+    const size_t tbl = tbl_in_smem(MODE) ? (size_t)G::BINS * ROW_SMEM_WORDS * 4 : (size_t)G::BINS * 4;
     const size_t tbl_al = (tbl + 15) & ~(size_t)15;
-    const size_t lat = MODE == MODE_STREAMED ? 0 : (size_t)L * G::WPR * 4 * tpb;
+    const size_t lat = lat_streamed(MODE) ? 0 : (size_t)L * G::WPR * 4 * tpb;
     return tbl_al + lat;
 }
 
@@ -704,7 +708,7 @@ __device__ __forceinline__ void resident_sweeps(uint32_t* __restrict__ lat, cons
     }
 }
 
-template <int L, bool MEAS>
+template <int L, int MODE, bool MEAS>
 __device__ __forceinline__ void streamed_sweeps(uint32_t* __restrict__ rows, const size_t row_stride, uint32_t& o,
                                                 const uint32_t s0, const uint32_t s1, const SweepParams& prm,
                                                 const uint32_t walker, const char* tbl_glob, uint32_t* hist) {
@@ -723,7 +727,7 @@ __device__ __forceinline__ void streamed_sweeps(uint32_t* __restrict__ rows, con
 #pragma unroll
                 for (int k = 0; k < WPR; ++k) dn[k] = first[k];                     // row 0, already updated
             }
-            process_row<L, MODE_STREAMED, MEAS>(up, cur, dn, o, (uint32_t)(y * (L / 4)), s, prm.iteration, walker,
+            process_row<L, MODE, MEAS>(up, cur, dn, o, (uint32_t)(y * (L / 4)), s, prm.iteration, walker,
                                                 prm.key0, prm.key1, nullptr, tbl_glob, hist);
             st_row<WPR>(rows + (size_t)y * row_stride, cur);
 #pragma unroll
@@ -741,18 +745,18 @@ template <int L, int MODE>
 __global__ void sweep_kernel(const SweepParams prm) {
     using G = Geo<L>;
     constexpr int WPR = G::WPR, N = G::N, BINS = G::BINS;
-    constexpr int RSW = MODE == MODE_TBL_SMEM ? ROW_SMEM_WORDS : ROW_L1_WORDS;
+    constexpr int RSW = tbl_in_smem(MODE) ? ROW_SMEM_WORDS : ROW_L1_WORDS;
     extern __shared__ __align__(16) uint32_t smem[];
     const int tid = threadIdx.x, tpb = blockDim.x;
     const int w = blockIdx.x * tpb + tid;
     const bool active = w < prm.W;
 
     // ---- shared memory: [table+bins | bins] [lattices]
-    constexpr size_t TBL_WORDS = MODE == MODE_TBL_SMEM ? (size_t)BINS * ROW_SMEM_WORDS : (size_t)BINS;
+    constexpr size_t TBL_WORDS = tbl_in_smem(MODE) ? (size_t)BINS * ROW_SMEM_WORDS : (size_t)BINS;
     constexpr size_t TBL_WORDS_AL = (TBL_WORDS + 3) & ~(size_t)3;
     uint32_t* const tbl_s = smem;
     uint32_t* const lat = smem + TBL_WORDS_AL + tid;   // this thread's column: lat[r * tpb]
-    if (MODE == MODE_TBL_SMEM) {
+    if (tbl_in_smem(MODE)) {
         for (int idx = tid; idx < BINS * ROW_SMEM_WORDS; idx += tpb) {
             const int j = idx / ROW_SMEM_WORDS, e = idx - j * ROW_SMEM_WORDS;
             tbl_s[idx] = e < 8 ? prm.table[j * 8 + e] : 0u;   // e == 8: histogram bin, e == 9: pad
@@ -762,7 +766,7 @@ __global__ void sweep_kernel(const SweepParams prm) {
     }
 
     // ---- lattice into shared memory (unpacked to one word per row for L < 32)
-    if (MODE != MODE_STREAMED) {
+    if (!lat_streamed(MODE)) {
         if (active) {
             if (L >= 32) {
                 for (int y = 0; y < L; ++y) {
@@ -785,25 +789,25 @@ __global__ void sweep_kernel(const SweepParams prm) {
 
     if (active) {
         const int E = prm.E[w];
-        const uint32_t o_base = MODE == MODE_TBL_SMEM ? (uint32_t)__cvta_generic_to_shared(tbl_s) : 0u;
+        const uint32_t o_base = tbl_in_smem(MODE) ? (uint32_t)__cvta_generic_to_shared(tbl_s) : 0u;
         uint32_t o = o_base + (uint32_t)((E + 2 * N) >> 2) * (uint32_t)(RSW * 4);   // slot j = (E + 2N)/4
         const uint32_t walker = prm.walker_offset + (uint32_t)w;
         const char* tbl_smem = reinterpret_cast<const char*>(tbl_s);
         const char* tbl_glob = reinterpret_cast<const char*>(prm.table);
         const uint32_t s_th = prm.therm < prm.sweep_begin ? prm.sweep_begin
                               : (prm.therm > prm.sweep_end ? prm.sweep_end : prm.therm);
-        if (MODE == MODE_STREAMED) {
+        if (lat_streamed(MODE)) {
             uint32_t* rows = prm.spins + (size_t)w * WPR;
             const size_t row_stride = (size_t)prm.W * WPR;
-            streamed_sweeps<L, false>(rows, row_stride, o, prm.sweep_begin, s_th, prm, walker, tbl_glob, tbl_s);
-            streamed_sweeps<L, true>(rows, row_stride, o, s_th, prm.sweep_end, prm, walker, tbl_glob, tbl_s);
+            streamed_sweeps<L, MODE, false>(rows, row_stride, o, prm.sweep_begin, s_th, prm, walker, tbl_glob, tbl_s);
+            streamed_sweeps<L, MODE, true>(rows, row_stride, o, s_th, prm.sweep_end, prm, walker, tbl_glob, tbl_s);
         } else {
             resident_sweeps<L, MODE, false>(lat, tpb, o, prm.sweep_begin, s_th, prm, walker, tbl_smem, tbl_glob, tbl_s);
             resident_sweeps<L, MODE, true>(lat, tpb, o, s_th, prm.sweep_end, prm, walker, tbl_smem, tbl_glob, tbl_s);
         }
         prm.E[w] = (int)((o - o_base) / (uint32_t)(RSW * 4)) * 4 - 2 * N;
 
-        if (MODE != MODE_STREAMED) {
+        if (!lat_streamed(MODE)) {
             if (L >= 32) {
                 for (int y = 0; y < L; ++y) {
                     uint32_t r[WPR];
@@ -827,7 +831,7 @@ __global__ void sweep_kernel(const SweepParams prm) {
     // ---- a4: merge the block's bins into the global uint64 histogram
     if (prm.sweep_end > prm.therm) {
         for (int j = tid; j < BINS; j += tpb) {
-            const uint32_t v = MODE == MODE_TBL_SMEM ? tbl_s[j * ROW_SMEM_WORDS + 8] : tbl_s[j];
+            const uint32_t v = tbl_in_smem(MODE) ? tbl_s[j * ROW_SMEM_WORDS + 8] : tbl_s[j];
             if (v) atomicAdd(prm.H + j, (unsigned long long)v);
         }
     }

@@ -126,6 +126,7 @@ def test_configs345_reduced(L, W, iters, therm, sweeps):
     (16, B.MUCA_KERNEL_RESIDENT_V2, 32), (32, B.MUCA_KERNEL_RESIDENT_V2, 64),
     (64, B.MUCA_KERNEL_RESIDENT, 32), (64, B.MUCA_KERNEL_RESIDENT, 224), (64, B.MUCA_KERNEL_STREAMED, 64),
     (128, B.MUCA_KERNEL_RESIDENT, 32), (128, B.MUCA_KERNEL_STREAMED, 64),
+    (32, B.MUCA_KERNEL_STREAMED_SMEM, 96), (64, B.MUCA_KERNEL_STREAMED_SMEM, 64), (64, B.MUCA_KERNEL_STREAMED_SMEM, 256),
 ])
 def test_kernel_variants(L, kernel, tpb):
     W = 2 * tpb + 13
