@@ -253,7 +253,7 @@ def run_ours(args, cfg):
     peak = SM_COUNT * SCHED_PER_SM * ALU_LANES * f_max_hz / 1e12
     issue_peak = SM_COUNT * SCHED_PER_SM * ISSUE_LANES * f_max_hz / 1e12
     kernel = "muca::sweep_kernel_v5<%d>" % cfg.L if cfg.L <= 32 else \
-        "muca::sweep_kernel<%d, %s>" % (cfg.L, "TBL_L1" if cfg.L == 64 else "STREAMED")
+        "muca::sweep_kernel<%d, %s>" % (cfg.L, "STREAMED_SMEM" if cfg.L == 64 else "STREAMED")
     roofline = {
         "bound": "alu", "achieved": achieved, "peak": peak, "unit": "T lane-ops/s on the ALU pipe", "frac": achieved / peak,
         "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(cfg.name) if world == 1 else None,
@@ -264,10 +264,10 @@ def run_ours(args, cfg):
                        "11.7 ALU-only instructions per attempted flip (DESIGN.md 6.2)",
         "issue": {"achieved": kern_flips_s * OPS_PER_FLIP / 1e12, "peak": issue_peak, "unit": "T thread-instructions/s",
                   "frac": kern_flips_s * OPS_PER_FLIP / 1e12 / issue_peak, "ops_per_flip": OPS_PER_FLIP},
-        "hbm": {"algorithmic_bytes_per_flip": 0.0 if cfg.L <= 64 else 0.25, "peak_gbs": pk.get("hbm_gbs"),
-                "achieved_gbs": (0.0 if cfg.L <= 64 else 0.25) * kern_flips_s / 1e9,
-                "note": "lattices are shared-memory resident for L <= 64 (MiB of HBM traffic per launch); "
-                        "streamed at L = 128: every packed word read and written once per sweep"},
+        "hbm": {"algorithmic_bytes_per_flip": 0.0 if cfg.L <= 32 else 0.25, "peak_gbs": pk.get("hbm_gbs"),
+                "achieved_gbs": (0.0 if cfg.L <= 32 else 0.25) * kern_flips_s / 1e9,
+                "note": "lattices are shared-memory resident for L <= 32 (MiB of HBM traffic per launch); streamed at "
+                        "L >= 64: every packed word read and written once per sweep (16 MiB per config: served by L2)"},
     }
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
