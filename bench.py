@@ -285,6 +285,21 @@ def run_ours(args, cfg):
         "gpu_launches": stats["launches"],
         "roofline": roofline,
     }
+    if world == 1:
+        # secondary workload (the paper's Fig. 2 protocol): after the configured iterations,
+        # three measured-only iterations with the weights frozen (broad histogram, little bin contention)
+        g = mb.Muca(cfg.L, W, cfg.seed)
+        for _ in range(cfg.iterations):
+            g.run_iteration(cfg.therm_sweeps, cfg.sweeps)
+            g.update_weights()
+        fz = []
+        for _ in range(3):
+            g.run_iteration(0, cfg.sweeps)
+            fz.append(W * cfg.N * cfg.sweeps / (g.last_sweep_ms()[0] * 1e-3))
+        g.close()
+        out["frozen_weights"] = {"value": float(np.median(fz)), "unit": UNIT,
+                                 "what": f"sweep kernel only, 3 x {cfg.sweeps} measured sweeps after the {cfg.iterations} "
+                                         "configured iterations, weights not updated (outside the timed region)"}
     if world == 1 and not args.no_cpu_baseline:
         import muca_oracle as mo
         cores = mo.max_threads()

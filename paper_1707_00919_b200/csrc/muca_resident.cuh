@@ -176,7 +176,9 @@ __global__ void __launch_bounds__(64 * V5<L>::MAX_WARPS, 1) sweep_kernel_v5(cons
     char* const sm = reinterpret_cast<char*>(smem);
     const int tid = threadIdx.x, nthr = blockDim.x, nw = nthr >> 6;
     const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(smem);
-    if (sbase + V::RING_OFF + V::RING_BYTES > V::K) __trap();
+    // the window must end below K, and no row address may be 0 (the site macro uses "S & ~K != 0" as an always-true
+    // predicate; dynamic shared memory starts behind the 1 KB the system reserves on sm_100)
+    if (sbase == 0u || sbase + V::RING_OFF + V::RING_BYTES > V::K) __trap();
 
     // ---- both table copies: row (j, c) = t[8] | Sa[8] | bin
     for (int idx = tid; idx < BINS * 16; idx += nthr) {
