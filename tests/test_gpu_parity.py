@@ -117,6 +117,41 @@ def test_configs345_reduced(L, W, iters, therm, sweeps):
         run_pair(L, W, seed, iters, therm, sweeps, offset=11)
 
 
+# configs 3-5 at FULL size in the launch configuration bench.py times (library defaults).  The walkers are
+# independent given the weights, so the oracle follows sampled walker ranges one by one (same global
+# ids, the library's omega injected before every iteration); what cannot be sampled is checked through the
+# invariants: sum(H), the unreachable slots, tracked E == recomputed E for every walker.
+@pytest.mark.parametrize("name", ["L32_w16384", "L64_w32768", "L128_w8192"])
+def test_full_size_configs_sampled_walkers(name):
+    c = next(x for x in CONFIGS if x.name == name)
+    W, N = c.n_walkers, c.N
+    starts = sorted({0, 27, W // 3 + 5, W // 2 - 3, W - 6})        # first / inner / last walkers, across warp and block borders
+    width = 6
+    g = mb.Muca(c.L, W, c.seed)
+    oracles = [mo.Oracle(c.L, width, c.seed, walker_offset=w0) for w0 in starts]
+    try:
+        for it in range(c.iterations):
+            logw = g.get_log_weights()
+            H = g.run_iteration(c.therm_sweeps, c.sweeps)
+            assert int(H.sum()) == W * c.sweeps * N and H[1] == 0 and H[N - 1] == 0
+            for o in oracles:
+                o.set_log_weights(logw)
+                o.run_iteration(c.therm_sweeps, c.sweeps, n_threads=mo.max_threads())
+            g.update_weights()
+            assert np.max(np.abs(g.get_log_weights() - (logw - np.where(H > 0, np.log(np.maximum(H, 1).astype(np.float64)), 0.0)))) <= LOGW_TOL
+        E, spins = g.get_energies(), g.get_spins()
+        for w0, o in zip(starts, oracles):
+            assert np.array_equal(E[w0:w0 + width], o.get_energies()), f"{name}: energies of walkers {w0}.."
+            assert np.array_equal(spins[w0:w0 + width], o.get_spins()), f"{name}: spins of walkers {w0}.."
+        step = 4096                                                  # tracked E == recomputed E, all walkers
+        for a in range(0, W, step):
+            assert np.array_equal(energy_numpy(spins[a:a + step]), E[a:a + step])
+    finally:
+        g.close()
+        for o in oracles:
+            o.close()
+
+
 # every kernel variant / block size must give the same chains
 @pytest.mark.parametrize("L,kernel,tpb", [
     (8, B.MUCA_KERNEL_RESIDENT, 64), (16, B.MUCA_KERNEL_RESIDENT, 128),
