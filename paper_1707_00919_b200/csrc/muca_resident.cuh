@@ -44,6 +44,43 @@ struct V5 {
     static constexpr size_t SMEM_BYTES = (size_t)K + TBL_BYTES;
 };
 
+// Static planes of a row, split so that the part that does not depend on the row ABOVE (which the walker has only
+// just finished) can be prepared one row ahead, in the shadow of the current row's table loads:
+//   partial_words: nibble q of P[r] = hl + 2*(vd + hr) of site 4q + r   (hl/hr: left/right bond, vd: bond to the row below)
+//   finish_words : FW[r] = P[r] + 2*vu   (vu: bond to the row above)  =  column f = hl + 2*n3 of field_words()
+template <int L>
+__device__ __forceinline__ void partial_words(const uint32_t c, const uint32_t dn, uint32_t (&P)[4], uint32_t& patch) {
+    using G = Geo<L>;
+    constexpr int BITS = G::BITS;
+    uint32_t rw, lw;
+    if constexpr (L >= 32) {
+        rw = (c >> 1) | (c << 31);
+        lw = (c << 1) | (c >> 31);
+    } else {
+        rw = (c >> 1) | ((c & 1u) << (BITS - 1));
+        lw = ((c << 1) | (c >> (BITS - 1))) & G::MASK;
+    }
+    const uint32_t vd = c ^ dn, hr = c ^ rw, hl = c ^ lw;
+    const uint32_t m0 = vd ^ hr, m1 = vd & hr;
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const uint32_t A = hl >> r;
+        const uint32_t B = r >= 1 ? m0 >> (r - 1) : m0 << 1;
+        const uint32_t C = r >= 2 ? m1 >> (r - 2) : m1 << (2 - r);
+        const uint32_t t1 = (A & 0x11111111u) | (B & 0x22222222u);
+        P[r] = t1 | (C & 0x44444444u);
+    }
+    constexpr int QL = BITS / 4 - 1;
+    const uint32_t hr_last = (hr >> (BITS - 1)) & 1u;
+    patch = (1u << (4 * QL + 1)) - (hr_last << (4 * QL + 2));   // site 0 flipped: n3 of the LAST site +-1
+}
+template <int L>
+__device__ __forceinline__ void finish_words(const uint32_t (&P)[4], const uint32_t vu, uint32_t (&FW)[4]) {
+    constexpr uint32_t M = Geo<L>::BITS == 32 ? 0x11111111u : (Geo<L>::BITS == 16 ? 0x1111u : 0x11u);
+#pragma unroll
+    for (int r = 0; r < 4; ++r) FW[r] = P[r] + 2u * ((vu >> r) & M);
+}
+
 // One site of the walker chain, in PTX.  Three things ptxas does not do by itself:
 //  * the decision must be consumed by a SEL: ISETP -> SEL -> (IADD ->) LDS costs 9 (13) cycles on sm_100a, ISETP ->
 //    predicated instruction -> LDS about 20 (profiles/r01_ubench_chain.txt).  ptxas turns "S = p ? sa : S & ~K" into a
@@ -74,60 +111,92 @@ struct V5 {
     FLIP_SHIFT_OP " g0, %0, %10;\n\t"                                            \
     "lop3.b32 %2, %2, g0, %7, 0xF8;\n\t" EXTRA_LINE "}"
 
-// Walker warp: sweeps s0 .. s1-1; `buf` is the ring buffer holding the deviates of the next row to process.
-// Every site increments the bin of the state it STARTS from, i.e. of the state after the previous attempt; the
-// caller compensates the first and the last attempt of the measured phase.
+// One row of the walker warp.  In: the row above (`up`, final), this row (`c`, `P`, `patch`, `rnd`: old values, partial
+// planes, deviates).  Out: the same for row y + 1 in (c1, P1, patch1, rnd1), fetched / prepared while this row is
+// processed (none of it depends on this row; only "FW = P + 2*vu" waits for the row above), and `up` = this row's new
+// value.  Every site increments the bin of the state it STARTS from, i.e. of the state after the previous attempt.
+template <int L>
+__device__ __forceinline__ void row_v5(uint32_t* __restrict__ lat, uint32_t& S, const int y, const bool more, uint32_t& up,
+                                       const uint32_t c, const uint32_t (&P)[4], const uint32_t patch,
+                                       const uint32_t (&rnd)[Geo<L>::BITS], uint32_t& c1, uint32_t (&P1)[4], uint32_t& patch1,
+                                       uint32_t (&rnd1)[Geo<L>::BITS], const uint4* __restrict__ ring, int& buf,
+                                       const int bar_id) {
+    using G = Geo<L>;
+    using V = V5<L>;
+    constexpr int BITS = G::BITS, NC = V::NC, SLOTS = V::SLOTS;
+    // the deviates of row y + 1 are in ring[buf]; ring[buf ^ 1] (this row's, already in registers) may be refilled.
+    // After the last row of a phase there is no such barrier (the deviate warp has left its loop) and what is
+    // fetched below is not used.
+    if (more) pair_barrier(bar_id);
+    uint32_t FW[4];
+    finish_words<L>(P, c ^ up, FW);
+    const int y1 = (y + 1) & (L - 1), y2 = (y + 2) & (L - 1);
+    c1 = lat[y1 * SLOTS];
+    partial_words<L>(c1, lat[y2 * SLOTS], P1, patch1);   // row y + 2 is old (or row 0, final in this sweep, when y + 1 = L - 1)
+#pragma unroll
+    for (int k = 0; k < NC; ++k) {
+        const uint4 v = ring[(buf * NC + k) * SLOTS];
+        rnd1[4 * k] = v.x; rnd1[4 * k + 1] = v.y; rnd1[4 * k + 2] = v.z; rnd1[4 * k + 3] = v.w;
+    }
+    buf ^= (int)more;
+    S &= ~V::K;                        // site 0: its left neighbour (site L-1) has not been visited in this sweep
+    uint32_t A = S + ((FW[0] << 2) & 0x1Cu);
+    uint32_t flips = 0, unused = 0;    // `unused` fills operand %3 of the site macro where site 0 has FW[3]
+#pragma unroll
+    for (int x = 0; x < BITS; ++x) {
+        // column of the next site: nibble qn of FW[xn & 3], moved to bits 2..4 inside the site block
+        const int xn = x + 1, qn = xn >> 2;
+        const uint32_t fwn = xn < BITS ? FW[xn & 3] : 0u;
+        const uint32_t sh = qn == 0 ? 2u : (uint32_t)(4 * qn - 2);
+        constexpr int KB = V::KBIT;
+        const uint32_t fs = x <= KB ? (uint32_t)(KB - x) : (uint32_t)(x - KB);
+        if (x == 0)                    // site 0 also patches the last site's column: its right neighbour is site 0
+            asm volatile(MUCA_V5_SITE("shl.b32", "shr.u32", "@p add.u32 %3, %3, %9;\n\t")
+                         : "+r"(S), "+r"(A), "+r"(flips), "+r"(FW[3])
+                         : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u), "n"(~V::K), "r"(patch), "r"(fs) : "memory");
+        else if (qn == 0)
+            asm volatile(MUCA_V5_SITE("shl.b32", "shr.u32", "")
+                         : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused)
+                         : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u << (x & 31)), "n"(~V::K), "r"(0u), "r"(fs) : "memory");
+        else if (x <= KB)
+            asm volatile(MUCA_V5_SITE("shr.u32", "shr.u32", "")
+                         : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused)
+                         : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u << (x & 31)), "n"(~V::K), "r"(0u), "r"(fs) : "memory");
+        else
+            asm volatile(MUCA_V5_SITE("shr.u32", "shl.b32", "")
+                         : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused)
+                         : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u << (x & 31)), "n"(~V::K), "r"(0u), "r"(fs) : "memory");
+    }
+    up = c ^ flips;
+    lat[y * SLOTS] = up;
+}
+
+// Walker warp: sweeps s0 .. s1-1; `buf` is the ring buffer holding the deviates of the next row to fetch.  Rows are
+// processed in pairs so that the two register sets (this row / next row) swap roles without copies.
+// The caller compensates the first and the last attempt of the measured phase in the histogram (see row_v5).
 template <int L>
 __device__ __forceinline__ void sweeps_v5(uint32_t* __restrict__ lat, uint32_t& S, const uint32_t s0, const uint32_t s1,
                                           const uint4* __restrict__ ring, int& buf, const int bar_id) {
     using G = Geo<L>;
     using V = V5<L>;
     constexpr int BITS = G::BITS, NC = V::NC, SLOTS = V::SLOTS;
+    if (s1 <= s0) return;
+    uint32_t up = lat[(L - 1) * SLOTS], cA = lat[0], cB;
+    uint32_t PA[4], PB[4], patchA, patchB, rndA[BITS], rndB[BITS];
+    partial_words<L>(cA, lat[SLOTS], PA, patchA);
+    pair_barrier(bar_id);                      // the deviates of the first row are in ring[buf]
+#pragma unroll
+    for (int k = 0; k < NC; ++k) {
+        const uint4 v = ring[(buf * NC + k) * SLOTS];
+        rndA[4 * k] = v.x; rndA[4 * k + 1] = v.y; rndA[4 * k + 2] = v.z; rndA[4 * k + 3] = v.w;
+    }
+    buf ^= 1;
 #pragma unroll 1
     for (uint32_t s = s0; s < s1; ++s) {
 #pragma unroll 1
-        for (int y = 0; y < L; ++y) {
-            const int ym = (y + L - 1) & (L - 1), yp = (y + 1) & (L - 1);
-            const uint32_t up = lat[ym * SLOTS], dn = lat[yp * SLOTS], c = lat[y * SLOTS];
-            uint32_t FW[4], patch;
-            field_words<L>(up, c, dn, FW, patch);
-            pair_barrier(bar_id);              // the deviates of this row are in ring[buf]; ring[buf ^ 1] may be refilled
-            uint32_t rnd[BITS];
-#pragma unroll
-            for (int k = 0; k < NC; ++k) {
-                const uint4 v = ring[(buf * NC + k) * SLOTS];
-                rnd[4 * k] = v.x; rnd[4 * k + 1] = v.y; rnd[4 * k + 2] = v.z; rnd[4 * k + 3] = v.w;
-            }
-            buf ^= 1;
-            S &= ~V::K;                        // site 0: its left neighbour (site L-1) has not been visited in this sweep
-            uint32_t A = S + ((FW[0] << 2) & 0x1Cu);
-            uint32_t flips = 0, unused = 0;    // `unused` fills operand %3 of the site macro where site 0 has FW[3]
-#pragma unroll
-            for (int x = 0; x < BITS; ++x) {
-                // column of the next site: nibble qn of FW[xn & 3], moved to bits 2..4 inside the site block
-                const int xn = x + 1, qn = xn >> 2;
-                const uint32_t fwn = xn < BITS ? FW[xn & 3] : 0u;
-                const uint32_t sh = qn == 0 ? 2u : (uint32_t)(4 * qn - 2);
-                constexpr int KB = V::KBIT;
-                const uint32_t fs = x <= KB ? (uint32_t)(KB - x) : (uint32_t)(x - KB);
-                if (x == 0)                    // site 0 also patches the last site's column: its right neighbour is site 0
-                    asm volatile(MUCA_V5_SITE("shl.b32", "shr.u32", "@p add.u32 %3, %3, %9;\n\t")
-                                 : "+r"(S), "+r"(A), "+r"(flips), "+r"(FW[3])
-                                 : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u), "n"(~V::K), "r"(patch), "r"(fs) : "memory");
-                else if (qn == 0)
-                    asm volatile(MUCA_V5_SITE("shl.b32", "shr.u32", "")
-                                 : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused)
-                                 : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u << (x & 31)), "n"(~V::K), "r"(0u), "r"(fs) : "memory");
-                else if (x <= KB)
-                    asm volatile(MUCA_V5_SITE("shr.u32", "shr.u32", "")
-                                 : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused)
-                                 : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u << (x & 31)), "n"(~V::K), "r"(0u), "r"(fs) : "memory");
-                else
-                    asm volatile(MUCA_V5_SITE("shr.u32", "shl.b32", "")
-                                 : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused)
-                                 : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u << (x & 31)), "n"(~V::K), "r"(0u), "r"(fs) : "memory");
-            }
-            lat[y * SLOTS] = c ^ flips;
+        for (int y = 0; y < L; y += 2) {
+            row_v5<L>(lat, S, y, true, up, cA, PA, patchA, rndA, cB, PB, patchB, rndB, ring, buf, bar_id);
+            row_v5<L>(lat, S, y + 1, s + 1 < s1 || y + 2 < L, up, cB, PB, patchB, rndB, cA, PA, patchA, rndA, ring, buf, bar_id);
         }
     }
 }
@@ -196,9 +265,15 @@ __global__ void __launch_bounds__(64 * V5<L>::MAX_WARPS, 1) sweep_kernel_v5(cons
     if (tid < 17)  // row BINS of copy 0: t = 0 and Sa = itself in every column -- a lane parked here stays here
         *reinterpret_cast<uint32_t*>(sm + (size_t)BINS * V::RS + 4 * tid) = tid >= 8 && tid < 16 ? sbase + BINS * V::RS : 0u;
 
-    const bool is_walker = tid >= 32 * nw;
-    const int slot = is_walker ? tid - 32 * nw : tid;          // lattice / ring column
-    const int pair = slot >> 5, lane = slot & 31;
+    // warp -> role.  A warp runs on scheduler (warp id % 4).  With 4 pairs per block the walker warps take warp ids
+    // {0, 1, 4, 5} and the deviate warps {2, 3, 6, 7}: two walker warps share a scheduler (each is latency-bound and
+    // leaves 60 % of the issue slots to the other) and two deviate warps share one; a walker sharing with its deviate
+    // warp instead loses 12 cycles per site to the Philox stream (profiles/README.md).  With 1 or 2 pairs every warp
+    // has a scheduler of its own (deviate ids 0 .. nw-1, walker ids nw .. 2nw-1).
+    const int warp_id = tid >> 5;
+    const bool is_walker = nw == 4 ? (warp_id & 2) == 0 : warp_id >= nw;
+    const int pair = nw == 4 ? (warp_id & 1) | ((warp_id >> 2) << 1) : (is_walker ? warp_id - nw : warp_id);
+    const int lane = tid & 31, slot = 32 * pair + lane;          // slot: lattice / ring column
     const int w = (blockIdx.x * nw + pair) * wpw + lane;
     const bool active = lane < wpw && w < prm.W;
     const int bar_id = 1 + pair;
