@@ -93,10 +93,10 @@ __device__ __forceinline__ void finish_words(const uint32_t (&P)[4], const uint3
 //  * H[j]++ of the PREVIOUS attempt is issued behind this site's table loads (S still holds that state).
 //   %0 S: state address (in/out)    %1 A: entry address of this site (in), of the next site (out)
 //   %2 flips (in/out)   %3 FW[3] at site 0 (in/out)   %4 deviate   %5 field word of the NEXT site   %6 its shift
-//   %7 flip mask of this site   %8 ~K   %9 patch (site 0)   %10 distance between bit K and the site's bit
-// The flip mask collects bit K of the new state (= the decision) with a shift and a LOP3: an instruction predicated
-// on p would stall ~13 cycles behind the ISETP, in front of the next table load.
-#define MUCA_V5_SITE(SHIFT_OP, FLIP_SHIFT_OP, EXTRA_LINE)                                      \
+//   %7 flip mask of this site   %8 ~K   %9 patch (site 0)
+// The flip mask is a predicated OR (one ALU instruction; collecting bit K of the new state with SHF + LOP3 instead
+// costs 1.7 cycles per site once two walker warps share a scheduler and its ALU pipe).
+#define MUCA_V5_SITE(SHIFT_OP, EXTRA_LINE)                                       \
     "{\n\t.reg .pred p, ps, pg;\n\t.reg .b32 t, sa, sr, g0, g;\n\t"               \
     "ld.shared.u32 t, [%1];\n\t"                                                 \
     "ld.shared.u32 sa, [%1+32];\n\t"                                             \
@@ -108,8 +108,7 @@ __device__ __forceinline__ void finish_words(const uint32_t (&P)[4], const uint3
     "setp.le.and.u32 p, %4, t, pg;\n\t"                                          \
     "selp.u32 %0, sa, sr, p;\n\t"                                                \
     "add.u32 %1, %0, g;\n\t"                                                     \
-    FLIP_SHIFT_OP " g0, %0, %10;\n\t"                                            \
-    "lop3.b32 %2, %2, g0, %7, 0xF8;\n\t" EXTRA_LINE "}"
+    "@p or.b32 %2, %2, %7;\n\t" EXTRA_LINE "}"
 
 // One row of the walker warp.  In: the row above (`up`, final), this row (`c`, `P`, `patch`, `rnd`: old values, partial
 // planes, deviates).  Out: the same for row y + 1 in (c1, P1, patch1, rnd1), fetched / prepared while this row is
@@ -148,24 +147,18 @@ __device__ __forceinline__ void row_v5(uint32_t* __restrict__ lat, uint32_t& S, 
         const int xn = x + 1, qn = xn >> 2;
         const uint32_t fwn = xn < BITS ? FW[xn & 3] : 0u;
         const uint32_t sh = qn == 0 ? 2u : (uint32_t)(4 * qn - 2);
-        constexpr int KB = V::KBIT;
-        const uint32_t fs = x <= KB ? (uint32_t)(KB - x) : (uint32_t)(x - KB);
         if (x == 0)                    // site 0 also patches the last site's column: its right neighbour is site 0
-            asm volatile(MUCA_V5_SITE("shl.b32", "shr.u32", "@p add.u32 %3, %3, %9;\n\t")
+            asm volatile(MUCA_V5_SITE("shl.b32", "@p add.u32 %3, %3, %9;\n\t")
                          : "+r"(S), "+r"(A), "+r"(flips), "+r"(FW[3])
-                         : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u), "n"(~V::K), "r"(patch), "r"(fs) : "memory");
+                         : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u), "n"(~V::K), "r"(patch) : "memory");
         else if (qn == 0)
-            asm volatile(MUCA_V5_SITE("shl.b32", "shr.u32", "")
+            asm volatile(MUCA_V5_SITE("shl.b32", "")
                          : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused)
-                         : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u << (x & 31)), "n"(~V::K), "r"(0u), "r"(fs) : "memory");
-        else if (x <= KB)
-            asm volatile(MUCA_V5_SITE("shr.u32", "shr.u32", "")
-                         : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused)
-                         : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u << (x & 31)), "n"(~V::K), "r"(0u), "r"(fs) : "memory");
+                         : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u << (x & 31)), "n"(~V::K) : "memory");
         else
-            asm volatile(MUCA_V5_SITE("shr.u32", "shl.b32", "")
+            asm volatile(MUCA_V5_SITE("shr.u32", "")
                          : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused)
-                         : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u << (x & 31)), "n"(~V::K), "r"(0u), "r"(fs) : "memory");
+                         : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u << (x & 31)), "n"(~V::K) : "memory");
     }
     up = c ^ flips;
     lat[y * SLOTS] = up;
