@@ -16,7 +16,8 @@
 // Per site the serial chain is   LDS t -> ISETP -> SEL(Sa, S & ~K) -> IADD (+ column of the next site) -> LDS t'.
 // Column extraction, flip mask and histogram increment are off the chain.  Philox runs in a paired "deviate" warp
 // (same walkers) that feeds a double-buffered shared ring one row ahead: the hardware interleaves its instruction
-// stream into the stalls of the walker warp.  What was measured and dropped: a single in-order
+// stream into the stalls of the walker warps (at 4 pairs per SM, walker warps share schedulers with walker warps and
+// deviate warps with deviate warps).  What was measured and dropped: a single in-order
 // warp doing both (75 cycles per site), selecting between two precomputed entry addresses (ptxas folds the add
 // into an instruction predicated on the decision, +11 cycles), and speculative loads for both outcomes of the
 // next site (the walker warp becomes issue-bound at the same 49 cycles).
@@ -223,12 +224,10 @@ __device__ __forceinline__ void deviates_v5(uint4* __restrict__ ring, const uint
     }
 }
 
-// Block = nw deviate warps (warp ids 0 .. nw-1) + nw walker warps (ids nw .. 2nw-1), nw <= 4; walker warp i and
-// deviate warp i serve the same wpw <= 32 walkers, (b*nw + i)*wpw .. +wpw-1, in their lanes 0 .. wpw-1.  At nw = 4 a
-// pair shares one scheduler (warp ids i and i + 4) and the higher id -- the serial chain -- wins the arbitration;
-// at nw <= 2 every warp has a scheduler of its own.  The host spreads the walkers over all SMs (as few warps per
-// SM, then as few lanes per warp, as possible: fewer lanes collide in the banks).  Lanes without a walker are
-// parked on the all-reject row and never leave it.
+// Block = nw walker warps + nw deviate warps, nw <= 4; walker warp i and deviate warp i ("pair" i) serve the same
+// wpw <= 32 walkers, (b*nw + i)*wpw .. +wpw-1, in their lanes 0 .. wpw-1 (see the warp -> role map in the kernel).
+// The host spreads the walkers over all SMs (as few pairs per SM, then as few lanes per warp, as possible: fewer
+// lanes collide in the banks).  Lanes without a walker are parked on the all-reject row and never leave it.
 template <int L>
 __global__ void __launch_bounds__(64 * V5<L>::MAX_WARPS, 1) sweep_kernel_v5(const SweepParams prm, const int wpw) {
     using G = Geo<L>;
