@@ -139,6 +139,48 @@ int muca_set_spins(muca_ctx* ctx, const int8_t* spins, size_t n);
  * context's stream. */
 int muca_unpack_spins_device(muca_ctx* ctx, void* d_spins_out, size_t n);
 
+/* ---- Convergence driver (Sec. 3, Eq. (6), (7), Appendix A Eq. (A.1)) ----------------
+ * Host logic around muca_run_iteration / muca_update_weights; the paper's schedule with whole sweeps as the unit
+ * of work (R18: a number of attempted flips per walker is rounded UP to whole sweeps, at least one).
+ *
+ * muca_flatness: statistics of one histogram H (host uint64[n_bins]) against the flat distribution Q = 1/w:
+ *   j_lo, j_hi  first / last visited slot;  width = j_hi - j_lo + 1 slots ("w'", in units of dE = 4; 0 if H == 0)
+ *   d_k = sum_{H>0} P ln(P w),  P = H / sum(H)                                  (Eq. (6))
+ *   d_c = max over the N - 1 accessible slots of |H / m - 1|,  m = sum(H)/(N - 1)   (Eq. (A.1))
+ * w >= 1: the width of the flat reference;  w = 0: the paper's w = max(w', 10) under DESIGN.md R19:
+ * w' = number of ACCESSIBLE slots (not 1 and N-1) in [j_lo, j_hi] of THIS histogram.  With the width
+ * of an earlier, narrower histogram, or with the two unreachable slots counted, Q would not be normalised over the
+ * support of P: d_k could be negative, and a perfectly flat histogram would give ln((N+1)/(N-1)) > 1e-4. */
+typedef struct muca_flatness_t {
+    int j_lo, j_hi, width;
+    double d_k, d_c;
+    uint64_t n_updates;   /* sum(H) */
+} muca_flatness_t;
+int muca_flatness(const uint64_t* H, int n_bins, int w, muca_flatness_t* out);
+
+/* muca_schedule: work of the next iteration from the width w' covered by the previous one (0 before the first):
+ *   w = max(w', 10);  N_therm = 30 w attempted flips per walker;
+ *   N_updates = floor(6 w^2.25 / n_walkers) + 1 flips per walker (Eq. (7)), also in the first iteration with
+ *   w = N + 1; from the second such iteration on N_updates <- floor(1.1 N_updates) + 1.
+ *   *n_updates_io and *full_range_io carry N_updates and "the previous iteration had w = N + 1" over (start: 0, 0).
+ *   therm_sweeps = ceil(N_therm / N), sweeps = ceil(N_updates / N)   (R18). */
+int muca_schedule(int L, int n_walkers, int w_prev, double* n_updates_io, int* full_range_io, int* w_out,
+                  int* therm_sweeps, int* sweeps);
+
+/* One record per iteration of muca_converge. */
+typedef struct muca_iteration_log_t {
+    int w, therm_sweeps, sweeps;
+    muca_flatness_t flat;
+    double sweep_ms;      /* device time of the sweep kernel(s) */
+} muca_iteration_log_t;
+
+/* muca_converge: repeat { schedule; run_iteration; flatness; update_weights } until d_k < d_flat (the paper: 1e-4)
+ * or max_iterations.  The weights are updated after EVERY iteration, the last one included.  log: host array of
+ * log_capacity records (may be NULL); *iterations_out = iterations done; *converged_out = 1 if d_k < d_flat.
+ * w_prev / n_updates start from 0 (first call on a context) -- the context keeps them, so a second call continues. */
+int muca_converge(muca_ctx* ctx, int max_iterations, double d_flat, muca_iteration_log_t* log, int log_capacity,
+                  int* iterations_out, int* converged_out);
+
 /* Debug / diagnostics.
  * thresholds: host uint32[n = n_bins*5], out[j*5 + a] as defined under muca_run_iteration, from the
  *             current omega.

@@ -23,7 +23,20 @@ EXPORTS = (
     "muca_update_weights", "muca_update_weights_with", "muca_get_energies", "muca_get_spins", "muca_set_spins",
     "muca_unpack_spins_device", "muca_get_thresholds", "muca_get_iteration", "muca_set_iteration",
     "muca_last_sweep_ms", "muca_last_error", "muca_debug_philox", "muca_version",
+    "muca_flatness", "muca_schedule", "muca_converge",
 )
+
+
+class Flatness(C.Structure):
+    """muca_flatness_t (include/muca.h)."""
+    _fields_ = [("j_lo", C.c_int), ("j_hi", C.c_int), ("width", C.c_int), ("d_k", C.c_double), ("d_c", C.c_double),
+                ("n_updates", C.c_uint64)]
+
+
+class IterationLog(C.Structure):
+    """muca_iteration_log_t (include/muca.h)."""
+    _fields_ = [("w", C.c_int), ("therm_sweeps", C.c_int), ("sweeps", C.c_int), ("flat", Flatness),
+                ("sweep_ms", C.c_double)]
 
 
 class MucaError(RuntimeError):
@@ -77,6 +90,11 @@ def lib():
     L.muca_last_error.restype = C.c_char_p
     L.muca_debug_philox.argtypes = [u32p, u32p, u32p, C.c_int]
     L.muca_version.restype = C.c_char_p
+    L.muca_flatness.argtypes = [u64p, C.c_int, C.c_int, C.POINTER(Flatness)]
+    L.muca_schedule.argtypes = [C.c_int, C.c_int, C.c_int, f64p, C.POINTER(C.c_int), C.POINTER(C.c_int),
+                                C.POINTER(C.c_int), C.POINTER(C.c_int)]
+    L.muca_converge.argtypes = [vp, C.c_int, C.c_double, C.POINTER(IterationLog), C.c_int, C.POINTER(C.c_int),
+                                C.POINTER(C.c_int)]
     _lib = L
     return L
 
@@ -98,6 +116,25 @@ def debug_philox(ctr, key) -> np.ndarray:
     if rc != MUCA_OK:
         raise MucaError(f"muca_debug_philox failed rc={rc}")
     return out
+
+
+def flatness(H, w: int) -> dict:
+    """muca_flatness: width, d_k (Eq. (6)), d_c (Eq. (A.1)) of a histogram against Q = 1/w (host only)."""
+    h = np.ascontiguousarray(H, dtype=np.uint64)
+    f = Flatness()
+    rc = lib().muca_flatness(_p(h, C.c_uint64), h.size, int(w), C.byref(f))
+    if rc != MUCA_OK:
+        raise MucaError(f"muca_flatness failed rc={rc}")
+    return {k: getattr(f, k) for k, _ in Flatness._fields_}
+
+
+def schedule(L: int, n_walkers: int, w_prev: int, n_updates: float = 0.0, full_range: int = 0):
+    """muca_schedule: (w, therm_sweeps, sweeps, n_updates, full_range) of the next iteration (Eq. (7); host only)."""
+    nu, fr, w, th, sw = C.c_double(n_updates), C.c_int(full_range), C.c_int(), C.c_int(), C.c_int()
+    rc = lib().muca_schedule(L, n_walkers, int(w_prev), C.byref(nu), C.byref(fr), C.byref(w), C.byref(th), C.byref(sw))
+    if rc != MUCA_OK:
+        raise MucaError(f"muca_schedule failed rc={rc}")
+    return w.value, th.value, sw.value, nu.value, fr.value
 
 
 class Muca:
@@ -222,6 +259,20 @@ class Muca:
     @iteration.setter
     def iteration(self, n: int):
         self._check(self._lib.muca_set_iteration(self._h, C.c_uint32(n)), "muca_set_iteration")
+
+    def converge(self, max_iterations: int, d_flat: float = 1e-4):
+        """muca_converge: the paper's weight iteration until d_k < d_flat.  Returns (log records, converged)."""
+        cap = max(int(max_iterations), 1)
+        log = (IterationLog * cap)()
+        n, conv = C.c_int(), C.c_int()
+        self._check(self._lib.muca_converge(self._h, int(max_iterations), float(d_flat), log, cap, C.byref(n), C.byref(conv)),
+                    "muca_converge")
+        out = []
+        for r in log[:n.value]:
+            d = {"w": r.w, "therm_sweeps": r.therm_sweeps, "sweeps": r.sweeps, "sweep_ms": r.sweep_ms}
+            d.update({k: getattr(r.flat, k) for k, _ in Flatness._fields_})
+            out.append(d)
+        return out, bool(conv.value)
 
     def last_sweep_ms(self):
         ms, k = C.c_double(), C.c_int()

@@ -41,6 +41,9 @@ struct muca_ctx {
     int opt_tpb = 0;
     int opt_max_sweeps = 0;
     int opt_wpw = 0;
+    int conv_w_prev = 0;            // width covered by the previous iteration of muca_converge (0: none yet)
+    double conv_n_updates = 0.0;    // N_updates (flips per walker) of the previous iteration of muca_converge
+    int conv_full = 0;              // the previous iteration already worked on the whole energy range
     int n_sm = 0;
     char err[512] = {0};
 };
@@ -457,6 +460,84 @@ int muca_update_weights_with(muca_ctx* ctx, const uint64_t* H_total, int n_bins)
 int muca_update_weights(muca_ctx* ctx) {
     if (!ctx) return MUCA_EINVAL;
     return muca_update_weights_with(ctx, ctx->H.data(), ctx->n_bins);
+}
+
+// ---- convergence driver (host logic; Eq. (6), (7), (A.1); R18) ----
+int muca_flatness(const uint64_t* H, int n_bins, int w, muca_flatness_t* out) {
+    if (!H || !out || n_bins < 3 || w < 0) return MUCA_EINVAL;
+    const int N = n_bins - 1;
+    uint64_t total = 0;
+    int lo = -1, hi = -1;
+    for (int j = 0; j < n_bins; ++j)
+        if (H[j]) { total += H[j]; if (lo < 0) lo = j; hi = j; }
+    out->j_lo = lo; out->j_hi = hi; out->width = lo < 0 ? 0 : hi - lo + 1; out->n_updates = total;
+    out->d_k = 0.0; out->d_c = 0.0;
+    if (total == 0) return MUCA_OK;
+    if (w == 0) {   // R19: w = max(w', 10), w' = ACCESSIBLE slots of the range covered by THIS histogram
+        w = out->width - ((lo <= 1 && hi >= 1) ? 1 : 0) - ((lo <= N - 1 && hi >= N - 1) ? 1 : 0);
+        if (w < 10) w = 10;
+    }
+    double dk = 0.0;                                         // Eq. (6): empty bins do not contribute
+    for (int j = 0; j < n_bins; ++j)
+        if (H[j]) { const double P = (double)H[j] / (double)total; dk += P * std::log(P * (double)w); }
+    out->d_k = dk;
+    const double m = (double)total / (double)(N - 1);       // Eq. (A.1): N - 1 accessible slots
+    double dc = 0.0;
+    for (int j = 0; j < n_bins; ++j) {
+        if (j == 1 || j == N - 1) continue;
+        const double d = std::fabs((double)H[j] / m - 1.0);
+        if (d > dc) dc = d;
+    }
+    out->d_c = dc;
+    return MUCA_OK;
+}
+
+int muca_schedule(int L, int n_walkers, int w_prev, double* n_updates_io, int* full_range_io, int* w_out, int* therm_sweeps,
+                  int* sweeps) {
+    if (!valid_L(L) || n_walkers < 1 || w_prev < 0 || !n_updates_io || !full_range_io || !w_out || !therm_sweeps || !sweeps)
+        return MUCA_EINVAL;
+    const int N = L * L;
+    const int w = w_prev > 10 ? w_prev : 10;                // w = max(w', 10)
+    double n_up;
+    const bool full = w >= N + 1;
+    if (full && *full_range_io) n_up = std::floor(1.1 * *n_updates_io) + 1.0;                   // whole range covered before: x 1.1
+    else n_up = std::floor(6.0 * std::pow((double)w, 2.25) / (double)n_walkers) + 1.0;          // Eq. (7), z = 2.25
+    const double n_th = 30.0 * (double)w;                    // f_therm = 30
+    const double max_sweeps = 1.0e9;
+    double sw = std::ceil(n_up / (double)N), th = std::ceil(n_th / (double)N);
+    if (sw < 1.0) sw = 1.0;
+    if (th < 1.0) th = 1.0;
+    if (sw > max_sweeps || th > max_sweeps) return MUCA_ERANGE;
+    *n_updates_io = n_up; *full_range_io = full ? 1 : 0; *w_out = w; *therm_sweeps = (int)th; *sweeps = (int)sw;
+    return MUCA_OK;
+}
+
+int muca_converge(muca_ctx* ctx, int max_iterations, double d_flat, muca_iteration_log_t* log, int log_capacity,
+                  int* iterations_out, int* converged_out) {
+    if (!ctx) return MUCA_EINVAL;
+    if (max_iterations < 0 || (log && log_capacity < 0)) return fail(ctx, MUCA_EINVAL, "converge: bad arguments");
+    int it = 0, conv = 0;
+    while (it < max_iterations && !conv) {
+        int w = 0, th = 0, sw = 0;
+        int rc = muca_schedule(ctx->L, ctx->W, ctx->conv_w_prev, &ctx->conv_n_updates, &ctx->conv_full, &w, &th, &sw);
+        if (rc != MUCA_OK) return fail(ctx, rc, "converge: schedule out of range");
+        rc = muca_run_iteration(ctx, th, sw, nullptr, ctx->n_bins);
+        if (rc != MUCA_OK) return rc;
+        muca_flatness_t fl;
+        rc = muca_flatness(ctx->H.data(), ctx->n_bins, 0, &fl);
+        if (rc != MUCA_OK) return fail(ctx, rc, "converge: flatness failed");
+        rc = muca_update_weights(ctx);
+        if (rc != MUCA_OK) return rc;
+        if (log && it < log_capacity) {
+            log[it].w = w; log[it].therm_sweeps = th; log[it].sweeps = sw; log[it].flat = fl; log[it].sweep_ms = ctx->last_sweep_ms;
+        }
+        ctx->conv_w_prev = fl.width;
+        conv = fl.d_k < d_flat ? 1 : 0;
+        ++it;
+    }
+    if (iterations_out) *iterations_out = it;
+    if (converged_out) *converged_out = conv;
+    return MUCA_OK;
 }
 
 int muca_get_energies(muca_ctx* ctx, int32_t* E_out, int n_walkers) {
