@@ -181,6 +181,19 @@ typedef struct muca_iteration_log_t {
 int muca_converge(muca_ctx* ctx, int max_iterations, double d_flat, muca_iteration_log_t* log, int log_capacity,
                   int* iterations_out, int* converged_out);
 
+/* ---- Production run with fixed weights and jackknife errors (Fig. 7) -----------------
+ * n_calls >= 2 calls of muca_run_iteration(therm_sweeps, sweeps) with the CURRENT weights (which are not updated),
+ * then, all in logarithms (R21):
+ *   ln Omega(E_j) = ln H(E_j) - omega(E_j), H the sum of the call histograms, shifted so that
+ *                   sum_j exp[ln Omega(E_j)] = 2^(L*L)
+ *   err(E_j)      = delete-one jackknife error over the n_calls histograms, every leave-one-out estimate normalised
+ *                   on its own: sqrt((n-1)/n * sum_k (x_k - mean x)^2)                       (ref. [46])
+ * ln_omega_out, err_out: host double[n_bins]; NaN where a slot was not visited (ln Omega) or not visited by every
+ * leave-one-out histogram (err).  H_calls_out: host uint64[n_calls * n_bins] or NULL.  The iteration counter advances
+ * by n_calls; muca_get_histogram afterwards returns the histogram of the last call. */
+int muca_production(muca_ctx* ctx, int n_calls, int therm_sweeps, int sweeps, double* ln_omega_out, double* err_out,
+                    uint64_t* H_calls_out, int n_bins);
+
 /* Debug / diagnostics.
  * thresholds: host uint32[n = n_bins*5], out[j*5 + a] as defined under muca_run_iteration, from the
  *             current omega.

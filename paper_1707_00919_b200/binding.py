@@ -23,7 +23,7 @@ EXPORTS = (
     "muca_update_weights", "muca_update_weights_with", "muca_get_energies", "muca_get_spins", "muca_set_spins",
     "muca_unpack_spins_device", "muca_get_thresholds", "muca_get_iteration", "muca_set_iteration",
     "muca_last_sweep_ms", "muca_last_error", "muca_debug_philox", "muca_version",
-    "muca_flatness", "muca_schedule", "muca_converge",
+    "muca_flatness", "muca_schedule", "muca_converge", "muca_production",
 )
 
 
@@ -93,6 +93,7 @@ def lib():
     L.muca_flatness.argtypes = [u64p, C.c_int, C.c_int, C.POINTER(Flatness)]
     L.muca_schedule.argtypes = [C.c_int, C.c_int, C.c_int, f64p, C.POINTER(C.c_int), C.POINTER(C.c_int),
                                 C.POINTER(C.c_int), C.POINTER(C.c_int)]
+    L.muca_production.argtypes = [vp, C.c_int, C.c_int, C.c_int, f64p, f64p, u64p, C.c_int]
     L.muca_converge.argtypes = [vp, C.c_int, C.c_double, C.POINTER(IterationLog), C.c_int, C.POINTER(C.c_int),
                                 C.POINTER(C.c_int)]
     _lib = L
@@ -273,6 +274,14 @@ class Muca:
             d.update({k: getattr(r.flat, k) for k, _ in Flatness._fields_})
             out.append(d)
         return out, bool(conv.value)
+
+    def production(self, n_calls: int, therm_sweeps: int, sweeps: int):
+        """muca_production: fixed-weight calls + jackknife.  Returns (ln_omega, err, histograms[n_calls, n_bins])."""
+        ln_om, err = np.empty(self.n_bins, dtype=np.float64), np.empty(self.n_bins, dtype=np.float64)
+        Hs = np.empty((max(int(n_calls), 0), self.n_bins), dtype=np.uint64)
+        self._check(self._lib.muca_production(self._h, int(n_calls), int(therm_sweeps), int(sweeps), _p(ln_om, C.c_double),
+                                              _p(err, C.c_double), _p(Hs, C.c_uint64), self.n_bins), "muca_production")
+        return ln_om, err, Hs
 
     def last_sweep_ms(self):
         ms, k = C.c_double(), C.c_int()

@@ -7,6 +7,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <limits>
 #include <new>
 #include <vector>
 
@@ -537,6 +538,55 @@ int muca_converge(muca_ctx* ctx, int max_iterations, double d_flat, muca_iterati
     }
     if (iterations_out) *iterations_out = it;
     if (converged_out) *converged_out = conv;
+    return MUCA_OK;
+}
+
+// ---- production run + jackknife (host logic; R21) ----
+namespace {
+// ln Omega from one histogram (double counts): ln H - omega on visited slots, normalised to sum exp = 2^N; NaN elsewhere
+void ln_omega_estimate(const std::vector<double>& H, const std::vector<double>& logw, int N, std::vector<double>& out) {
+    const double nan = std::numeric_limits<double>::quiet_NaN();
+    const int bins = (int)H.size();
+    out.assign(bins, nan);
+    double mx = -std::numeric_limits<double>::infinity();
+    for (int j = 0; j < bins; ++j)
+        if (H[j] > 0.0) { out[j] = std::log(H[j]) - logw[j]; if (out[j] > mx) mx = out[j]; }
+    double sum = 0.0;
+    for (int j = 0; j < bins; ++j)
+        if (H[j] > 0.0) sum += std::exp(out[j] - mx);
+    const double shift = (double)N * std::log(2.0) - (mx + std::log(sum));
+    for (int j = 0; j < bins; ++j)
+        if (H[j] > 0.0) out[j] += shift;
+}
+}  // namespace
+
+int muca_production(muca_ctx* ctx, int n_calls, int therm_sweeps, int sweeps, double* ln_omega_out, double* err_out,
+                    uint64_t* H_calls_out, int n_bins) {
+    if (!ctx) return MUCA_EINVAL;
+    if (n_calls < 2 || n_bins != ctx->n_bins || !ln_omega_out || !err_out)
+        return fail(ctx, MUCA_EINVAL, "production: n_calls >= 2, n_bins must be %d, outputs must not be NULL", ctx->n_bins);
+    const int bins = ctx->n_bins;
+    std::vector<uint64_t> calls((size_t)n_calls * bins);
+    for (int k = 0; k < n_calls; ++k) {
+        const int rc = muca_run_iteration(ctx, therm_sweeps, sweeps, calls.data() + (size_t)k * bins, bins);
+        if (rc != MUCA_OK) return rc;
+    }
+    if (H_calls_out) std::memcpy(H_calls_out, calls.data(), sizeof(uint64_t) * calls.size());
+    std::vector<double> total(bins, 0.0), loo(bins), est, mean(bins, 0.0), var(bins, 0.0);
+    for (int k = 0; k < n_calls; ++k)
+        for (int j = 0; j < bins; ++j) total[j] += (double)calls[(size_t)k * bins + j];
+    ln_omega_estimate(total, ctx->logw, ctx->N, est);
+    for (int j = 0; j < bins; ++j) ln_omega_out[j] = est[j];
+    std::vector<double> all((size_t)n_calls * bins);
+    for (int k = 0; k < n_calls; ++k) {
+        for (int j = 0; j < bins; ++j) loo[j] = total[j] - (double)calls[(size_t)k * bins + j];
+        ln_omega_estimate(loo, ctx->logw, ctx->N, est);
+        for (int j = 0; j < bins; ++j) { all[(size_t)k * bins + j] = est[j]; mean[j] += est[j]; }
+    }
+    for (int j = 0; j < bins; ++j) mean[j] /= (double)n_calls;
+    for (int k = 0; k < n_calls; ++k)
+        for (int j = 0; j < bins; ++j) { const double d = all[(size_t)k * bins + j] - mean[j]; var[j] += d * d; }
+    for (int j = 0; j < bins; ++j) err_out[j] = std::sqrt((double)(n_calls - 1) / (double)n_calls * var[j]);   // NaN propagates
     return MUCA_OK;
 }
 
