@@ -1,4 +1,4 @@
-"""Writes tests/golden/ising_dos_L{4,8,16}.txt: exact g(E_j), one integer per line, j = 0..N.
+"""Writes tests/golden/ising_dos_L{4,8,16,32}.txt: exact g(E_j), one integer per line, j = 0..N.
 
 Source of the values: the closed form in tests/exact_dos.py (Kaufman/Beale, the
 paper's own ground truth: PAPER.md:129, :215-221, ref. [43] at :305), evaluated
@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, os.path.dirname(HERE))
 import exact_dos  # noqa: E402
 
-for L in (4, 8, 16):
+for L in (4, 8, 16, 32):
     g = exact_dos.exact_g(L)
     path = os.path.join(HERE, f"ising_dos_L{L}.txt")
     with open(path, "w") as f:
