@@ -116,6 +116,18 @@ int muca_get_log_weights(muca_ctx* ctx, double* logw_out, int n_bins);
  * Synchronises the context's stream before returning. */
 int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_out, int n_bins);
 
+/* One iteration with the PAPER'S OWN update scheme (R22) instead of
+ * typewriter sweeps: every update proposes the same random site in all walkers, each walker accepts with a deviate
+ * of its own stream:
+ *   update u = 0 .. therm_updates + updates - 1 of iteration n:
+ *     site i_u = word (u & 3) of Philox4x32-10(ctr = (u >> 2 mod 2^32, u >> 34, n, 0xFFFFFFFF), key)  mod N,
+ *     global walker g accepts iff word (u & 3) of Philox4x32-10(ctr = (u >> 2 mod 2^32, u >> 34, n, g), key) <= t,
+ *     t = thresh[j][a] as in muca_run_iteration;  H[j] += 1 after every update with u >= therm_updates.
+ * Work is counted in updates (attempted flips per walker), the paper's own unit.
+ * Everything else (thresholds, H, iteration counter, muca_update_weights, muca_last_sweep_ms) as muca_run_iteration.
+ * A straightforward kernel, not the tuned path. */
+int muca_run_iteration_random_site(muca_ctx* ctx, uint64_t therm_updates, uint64_t updates, uint64_t* H_out, int n_bins);
+
 /* Histogram of the last muca_run_iteration (host uint64[n_bins]). */
 int muca_get_histogram(muca_ctx* ctx, uint64_t* H_out, int n_bins);
 

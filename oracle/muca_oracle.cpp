@@ -200,6 +200,51 @@ void run_walker(const Oracle& o, int w, int therm, int sweeps, const uint32_t* t
     E_io = E;
 }
 
+// ---------------------------------------------------------------------------
+// The paper's own update scheme: "using the same
+// random number sequence for selecting the spins for all walkers, such that
+// an update attempt simultaneously occurs at the same site of each replica
+// ... The acceptance of updates using the Metropolis criterion is then tested
+// with a second stream of random numbers that is chosen independently for
+// each walker".  Work is counted in updates (attempted flips per walker,
+// PAPER.md:138, :150-157), not sweeps.  Reading R22: update u = 0, 1, ... of
+// iteration n proposes site i_u = (word (u & 3) of Philox(ctr = (u >> 2 mod 2^32,
+// u >> 34, n, 0xFFFFFFFF), key)) mod N for EVERY walker; global walker g
+// accepts iff word (u & 3) of Philox(ctr = (u >> 2 mod 2^32, u >> 34, n, g), key)
+// <= thresh[j][a]  (walker ids are < 0xFFFFFFFF, so the site stream is nobody's
+// acceptance stream).  The first `therm` updates are not recorded.
+// ---------------------------------------------------------------------------
+void run_walker_random_site(const Oracle& o, int w, uint64_t therm, uint64_t updates, const uint32_t* thresh,
+                            int8_t* s, int32_t& E_io, uint64_t* H) {
+    const int L = o.L, N = o.N;
+    const uint32_t key[2] = {(uint32_t)(o.seed & 0xFFFFFFFFu), (uint32_t)(o.seed >> 32)};
+    const uint32_t g = o.walker_offset + (uint32_t)w;
+    int E = E_io;
+    uint32_t rs[4] = {0, 0, 0, 0}, ra[4] = {0, 0, 0, 0};
+    for (uint64_t u = 0; u < therm + updates; ++u) {
+        if ((u & 3) == 0) {
+            const uint32_t cs[4] = {(uint32_t)((u >> 2) & 0xFFFFFFFFu), (uint32_t)(u >> 34), o.iteration, 0xFFFFFFFFu};
+            const uint32_t ca[4] = {(uint32_t)((u >> 2) & 0xFFFFFFFFu), (uint32_t)(u >> 34), o.iteration, g};
+            philox4x32_10(cs, key, rs);
+            philox4x32_10(ca, key, ra);
+        }
+        const int i = (int)(rs[u & 3] % (uint32_t)N);
+        const int x = i % L, y = i / L;
+        const int here = s[i];
+        const int nb[4] = {s[y * L + (x + 1) % L], s[y * L + (x + L - 1) % L], s[((y + 1) % L) * L + x],
+                           s[((y + L - 1) % L) * L + x]};
+        int a = 0;
+        for (int k = 0; k < 4; ++k) a += (nb[k] != here);
+        const int j = slot_of(E, N);
+        if (ra[u & 3] <= thresh[j * 5 + a]) {
+            s[i] = (int8_t)(-here);
+            E += 8 - 4 * a;
+        }
+        if (u >= therm) H[slot_of(E, N)] += 1;
+    }
+    E_io = E;
+}
+
 }  // namespace
 
 // ---------------------------------------------------------------------------
@@ -278,6 +323,36 @@ int oracle_run_iteration(void* h, int therm_sweeps, int sweeps, uint64_t* H_out,
 #endif
         run_walker(*o, w, therm_sweeps, sweeps, thresh.data(), &o->spin[(size_t)w * o->N], o->E[w],
                    Hpriv[t].data());
+    }
+    for (int j = 0; j < n_bins; ++j) {
+        uint64_t sum = 0;
+        for (int t = 0; t < n_threads; ++t) sum += Hpriv[t][j];
+        o->H[j] = sum;
+        H_out[j] = sum;
+    }
+    o->iteration += 1;
+    return 0;
+}
+
+int oracle_run_iteration_random_site(void* h, uint64_t therm_updates, uint64_t updates, uint64_t* H_out, int n_bins,
+                                     int n_threads) {
+    Oracle* o = (Oracle*)h;
+    if (n_bins != o->N + 1) return -1;
+    if (o->iteration == 0xFFFFFFFFu) return -2;
+    std::vector<uint32_t> thresh((size_t)n_bins * 5);
+    build_thresholds(n_bins, o->logw.data(), thresh.data());
+    if (n_threads < 1) n_threads = 1;
+    std::vector<std::vector<uint64_t>> Hpriv(n_threads, std::vector<uint64_t>(n_bins, 0));
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) num_threads(n_threads)
+#endif
+    for (int w = 0; w < o->W; ++w) {
+        int t = 0;
+#ifdef _OPENMP
+        t = omp_get_thread_num();
+#endif
+        run_walker_random_site(*o, w, therm_updates, updates, thresh.data(), &o->spin[(size_t)w * o->N], o->E[w],
+                               Hpriv[t].data());
     }
     for (int j = 0; j < n_bins; ++j) {
         uint64_t sum = 0;

@@ -43,6 +43,7 @@ def lib():
         L.oracle_set_log_weights.argtypes = [C.c_void_p, f64p, C.c_int]
         L.oracle_get_log_weights.argtypes = [C.c_void_p, f64p, C.c_int]
         L.oracle_run_iteration.argtypes = [C.c_void_p, C.c_int, C.c_int, u64p, C.c_int, C.c_int]
+        L.oracle_run_iteration_random_site.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, u64p, C.c_int, C.c_int]
         L.oracle_update_weights.argtypes = [C.c_void_p]
         L.oracle_update_weights_with.argtypes = [C.c_void_p, u64p, C.c_int]
         L.oracle_get_energies.argtypes = [C.c_void_p, i32p, C.c_int]
@@ -133,6 +134,15 @@ class Oracle:
                                         n_threads)
         if rc != 0:
             raise ValueError(f"oracle_run_iteration failed rc={rc}")
+        return H
+
+    def run_iteration_random_site(self, therm_updates: int, updates: int, n_threads: int = 1) -> np.ndarray:
+        """The paper's own scheme (R22): same random site for all walkers, per-walker acceptance stream; counts in updates."""
+        H = np.zeros(self.n_bins, dtype=np.uint64)
+        rc = lib().oracle_run_iteration_random_site(self._h, C.c_uint64(therm_updates), C.c_uint64(updates),
+                                                    _p(H, C.c_uint64), H.size, n_threads)
+        if rc != 0:
+            raise ValueError(f"oracle_run_iteration_random_site failed rc={rc}")
         return H
 
     def update_weights(self):

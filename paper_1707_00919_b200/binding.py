@@ -23,7 +23,7 @@ EXPORTS = (
     "muca_update_weights", "muca_update_weights_with", "muca_get_energies", "muca_get_spins", "muca_set_spins",
     "muca_unpack_spins_device", "muca_get_thresholds", "muca_get_iteration", "muca_set_iteration",
     "muca_last_sweep_ms", "muca_last_error", "muca_debug_philox", "muca_version",
-    "muca_flatness", "muca_schedule", "muca_converge", "muca_production",
+    "muca_flatness", "muca_schedule", "muca_converge", "muca_production", "muca_run_iteration_random_site",
 )
 
 
@@ -93,6 +93,7 @@ def lib():
     L.muca_flatness.argtypes = [u64p, C.c_int, C.c_int, C.POINTER(Flatness)]
     L.muca_schedule.argtypes = [C.c_int, C.c_int, C.c_int, f64p, C.POINTER(C.c_int), C.POINTER(C.c_int),
                                 C.POINTER(C.c_int), C.POINTER(C.c_int)]
+    L.muca_run_iteration_random_site.argtypes = [vp, C.c_uint64, C.c_uint64, u64p, C.c_int]
     L.muca_production.argtypes = [vp, C.c_int, C.c_int, C.c_int, f64p, f64p, u64p, C.c_int]
     L.muca_converge.argtypes = [vp, C.c_int, C.c_double, C.POINTER(IterationLog), C.c_int, C.POINTER(C.c_int),
                                 C.POINTER(C.c_int)]
@@ -260,6 +261,13 @@ class Muca:
     @iteration.setter
     def iteration(self, n: int):
         self._check(self._lib.muca_set_iteration(self._h, C.c_uint32(n)), "muca_set_iteration")
+
+    def run_iteration_random_site(self, therm_updates: int, updates: int) -> np.ndarray:
+        """muca_run_iteration_random_site: the paper's own scheme (same random site in all walkers); counts in updates."""
+        H = np.empty(self.n_bins, dtype=np.uint64)
+        self._check(self._lib.muca_run_iteration_random_site(self._h, C.c_uint64(therm_updates), C.c_uint64(updates),
+                                                             _p(H, C.c_uint64), self.n_bins), "muca_run_iteration_random_site")
+        return H
 
     def converge(self, max_iterations: int, d_flat: float = 1e-4):
         """muca_converge: the paper's weight iteration until d_k < d_flat.  Returns (log records, converged)."""

@@ -13,6 +13,7 @@
 
 #include "muca_device.cuh"
 #include "muca_resident.cuh"
+#include "muca_random_site.cuh"
 
 using namespace muca;
 
@@ -308,6 +309,21 @@ int create_common(muca_ctx** out, int L, int W, uint64_t seed, uint32_t walker_o
 
 }  // namespace
 
+namespace {
+template <int L>
+int launch_random_site(muca_ctx* ctx, const RandomSiteParams& prm, int tpb) {
+    const size_t smem = random_site_smem_bytes<L>(tpb);
+    static size_t configured = 0;
+    if (smem > configured) {
+        CU(cudaFuncSetAttribute(random_site_kernel<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured = smem;
+    }
+    random_site_kernel<L><<<(prm.W + tpb - 1) / tpb, tpb, smem, ctx->stream>>>(prm);
+    CU(cudaGetLastError());
+    return MUCA_OK;
+}
+}  // namespace
+
 extern "C" {
 
 const char* muca_version(void) { return "muca_b200 0.1 (sm_100a)"; }
@@ -428,6 +444,58 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
         if (rc != MUCA_OK) return rc;
         ++launches;
         s = e;
+    }
+    CU(cudaEventRecord(ctx->ev1, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->h_H, ctx->d_H, (size_t)ctx->n_bins * 8, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
+    ctx->last_sweep_ms = ms;
+    ctx->last_launches = launches;
+    for (int j = 0; j < ctx->n_bins; ++j) ctx->H[j] = (uint64_t)ctx->h_H[j];
+    if (H_out) std::memcpy(H_out, ctx->H.data(), sizeof(uint64_t) * ctx->n_bins);
+    ctx->iteration += 1;
+    return MUCA_OK;
+}
+
+// The paper's own update scheme (R22): same random site in all walkers.
+int muca_run_iteration_random_site(muca_ctx* ctx, uint64_t therm_updates, uint64_t updates, uint64_t* H_out, int n_bins) {
+    if (!ctx) return MUCA_EINVAL;
+    if (n_bins != ctx->n_bins) return fail(ctx, MUCA_EINVAL, "run_iteration_random_site: n_bins must be %d", ctx->n_bins);
+    if (ctx->iteration == 0xFFFFFFFFu) return fail(ctx, MUCA_ERANGE, "iteration counter exhausted");
+    if (therm_updates > (1ull << 60) || updates > (1ull << 60)) return fail(ctx, MUCA_EINVAL, "too many updates");
+    std::vector<uint32_t> t5;
+    build_thresholds5(ctx->logw, t5);                                           // a1, as in muca_run_iteration
+    expand_table8(t5, ctx->n_bins, ctx->h_table);
+    CU(cudaMemcpyAsync(ctx->d_table, ctx->h_table, (size_t)ctx->n_bins * 8 * 4, cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaMemsetAsync(ctx->d_H, 0, (size_t)ctx->n_bins * 8, ctx->stream));
+    const int tpb = ctx->L == 128 ? 32 : 128;                                     // 64 KiB of lattice words per block at L >= 64
+    RandomSiteParams prm;
+    prm.spins = ctx->d_spins; prm.E = ctx->d_E; prm.table = ctx->d_table; prm.H = ctx->d_H;
+    prm.W = ctx->W; prm.walker_offset = ctx->walker_offset;
+    prm.key0 = (uint32_t)(ctx->seed & 0xFFFFFFFFull); prm.key1 = (uint32_t)(ctx->seed >> 32);
+    prm.iteration = ctx->iteration; prm.therm = therm_updates;
+    const uint64_t total = therm_updates + updates;
+    const uint64_t max_meas = 0xFFFFFFFFull / (uint64_t)tpb;                      // a block's uint32 bins must not overflow
+    int launches = 0;
+    CU(cudaEventRecord(ctx->ev0, ctx->stream));
+    uint64_t u = 0;
+    while (u < total) {
+        const uint64_t meas_begin = u > therm_updates ? u : therm_updates;
+        uint64_t e = total;
+        if (e > meas_begin + max_meas) e = meas_begin + max_meas;
+        prm.u_begin = u; prm.u_end = e;
+        int rc = MUCA_EINVAL;
+        switch (ctx->L) {
+            case 8: rc = launch_random_site<8>(ctx, prm, tpb); break;
+            case 16: rc = launch_random_site<16>(ctx, prm, tpb); break;
+            case 32: rc = launch_random_site<32>(ctx, prm, tpb); break;
+            case 64: rc = launch_random_site<64>(ctx, prm, tpb); break;
+            case 128: rc = launch_random_site<128>(ctx, prm, tpb); break;
+        }
+        if (rc != MUCA_OK) return rc;
+        ++launches;
+        u = e;
     }
     CU(cudaEventRecord(ctx->ev1, ctx->stream));
     CU(cudaMemcpyAsync(ctx->h_H, ctx->d_H, (size_t)ctx->n_bins * 8, cudaMemcpyDeviceToHost, ctx->stream));
