@@ -21,6 +21,8 @@
 //   whole recursion    -> exact finite-lattice density of states (Beale/Kaufman), max |d ln g| < 0.05
 //   weight update      -> Eq. (4) retold in numpy on hand-made H
 //   invariants         -> tracked E == recomputed E, sum H = W*sweeps*N, forbidden slots empty
+//   random-site scheme -> omega == 0 closed form (site stream recomputed from the pinned Philox, H replayed in
+//                         numpy), canonical weights against exact g(E) at L = 4   (tests/test_random_site.py)
 // No function here is "parity unpinned".
 
 #include <cmath>
