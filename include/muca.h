@@ -65,9 +65,14 @@ enum {
     MUCA_OPT_THREADS_PER_BLOCK = 2, /* walkers (= threads) per block; 0 = library default         */
     MUCA_OPT_MAX_SWEEPS_PER_LAUNCH = 3, /* split an iteration into launches of at most this many sweeps;
                                           0 = only as needed to keep a block's uint32 bins from overflowing */
-    MUCA_OPT_WALKERS_PER_WARP = 4 /* resident kernel, L <= 32: walkers served by one warp (1..32); 0 = spread
+    MUCA_OPT_WALKERS_PER_WARP = 4, /* resident kernel, L <= 32: walkers served by one warp (1..32); 0 = spread
                                      the walkers evenly over all SMs */
+    MUCA_OPT_UPDATE_SCHEME = 5    /* update scheme of muca_converge / muca_production: MUCA_SCHEME_TYPEWRITER (default;
+                                     schedule rounded up to whole sweeps, R18) or MUCA_SCHEME_RANDOM_SITE (the paper's
+                                     own scheme and units: N_therm = 30 w and N_updates attempted flips per walker;
+                                     muca_production then runs therm_sweeps * N and sweeps * N updates per call) */
 };
+enum { MUCA_SCHEME_TYPEWRITER = 0, MUCA_SCHEME_RANDOM_SITE = 1 };
 
 /* Device workspace needed by muca_create_in() for (L, n_walkers); 0 on bad arguments. */
 size_t muca_workspace_bytes(int L, int n_walkers);
@@ -179,7 +184,8 @@ int muca_flatness(const uint64_t* H, int n_bins, int w, muca_flatness_t* out);
 int muca_schedule(int L, int n_walkers, int w_prev, double* n_updates_io, int* full_range_io, int* w_out,
                   int* therm_sweeps, int* sweeps);
 
-/* One record per iteration of muca_converge. */
+/* One record per iteration of muca_converge (therm_sweeps / sweeps: the typewriter schedule; with
+ * MUCA_SCHEME_RANDOM_SITE the iteration ran 30 w and flat.n_updates / n_walkers updates per walker instead). */
 typedef struct muca_iteration_log_t {
     int w, therm_sweeps, sweeps;
     muca_flatness_t flat;

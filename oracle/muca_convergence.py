@@ -60,12 +60,16 @@ def schedule(L, n_walkers, w_prev, n_updates=0.0, full_range=0):
     return w, therm_sweeps, sweeps, float(n_up), int(full)
 
 
-def converge(oracle, max_iterations, d_flat=1e-4, n_threads=1):
-    """Drive an oracle context (muca_oracle.Oracle) through the weight iteration. Returns (log, converged)."""
+def converge(oracle, max_iterations, d_flat=1e-4, n_threads=1, random_site=False):
+    """Drive an oracle context (muca_oracle.Oracle) through the weight iteration. Returns (log, converged).
+    random_site: the paper's own update scheme and units (30 w and N_updates attempted flips per walker, no rounding)."""
     log, w_prev, n_up, full, conv = [], 0, 0.0, 0, False
     while len(log) < max_iterations and not conv:
         w, th, sw, n_up, full = schedule(oracle.L, oracle.W, w_prev, n_up, full)
-        H = oracle.run_iteration(th, sw, n_threads=n_threads)
+        if random_site:
+            H = oracle.run_iteration_random_site(30 * w, int(n_up), n_threads=n_threads)
+        else:
+            H = oracle.run_iteration(th, sw, n_threads=n_threads)
         fl = flatness(H)
         oracle.update_weights()
         rec = {"w": w, "therm_sweeps": th, "sweeps": sw}

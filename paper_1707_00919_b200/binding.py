@@ -15,6 +15,8 @@ MUCA_OK = 0
 MUCA_KERNEL_AUTO, MUCA_KERNEL_RESIDENT, MUCA_KERNEL_STREAMED, MUCA_KERNEL_RESIDENT_V2, MUCA_KERNEL_RESIDENT_V3 = 0, 1, 2, 3, 4
 MUCA_KERNEL_STREAMED_SMEM = 5
 MUCA_OPT_KERNEL, MUCA_OPT_THREADS_PER_BLOCK, MUCA_OPT_MAX_SWEEPS_PER_LAUNCH, MUCA_OPT_WALKERS_PER_WARP = 1, 2, 3, 4
+MUCA_OPT_UPDATE_SCHEME = 5
+MUCA_SCHEME_TYPEWRITER, MUCA_SCHEME_RANDOM_SITE = 0, 1
 
 # every symbol include/muca.h declares (tests/test_abi.py checks the header against this list and the .so)
 EXPORTS = (

@@ -45,6 +45,7 @@ struct muca_ctx {
     int opt_wpw = 0;
     int conv_w_prev = 0;            // width covered by the previous iteration of muca_converge (0: none yet)
     double conv_n_updates = 0.0;    // N_updates (flips per walker) of the previous iteration of muca_converge
+    int opt_scheme = MUCA_SCHEME_TYPEWRITER;   // update scheme used by muca_converge / muca_production
     int conv_full = 0;              // the previous iteration already worked on the whole energy range
     int n_sm = 0;
     char err[512] = {0};
@@ -377,6 +378,11 @@ int muca_set_option(muca_ctx* ctx, int option, int value) {
         ctx->opt_wpw = value;
         return MUCA_OK;
     }
+    if (option == MUCA_OPT_UPDATE_SCHEME) {
+        if (value != MUCA_SCHEME_TYPEWRITER && value != MUCA_SCHEME_RANDOM_SITE) return fail(ctx, MUCA_EINVAL, "bad update scheme %d", value);
+        ctx->opt_scheme = value;
+        return MUCA_OK;
+    }
     if (option == MUCA_OPT_MAX_SWEEPS_PER_LAUNCH) {
         if (value < 0) return fail(ctx, MUCA_EINVAL, "max sweeps per launch must be >= 0");
         ctx->opt_max_sweeps = value;
@@ -590,7 +596,10 @@ int muca_converge(muca_ctx* ctx, int max_iterations, double d_flat, muca_iterati
         int w = 0, th = 0, sw = 0;
         int rc = muca_schedule(ctx->L, ctx->W, ctx->conv_w_prev, &ctx->conv_n_updates, &ctx->conv_full, &w, &th, &sw);
         if (rc != MUCA_OK) return fail(ctx, rc, "converge: schedule out of range");
-        rc = muca_run_iteration(ctx, th, sw, nullptr, ctx->n_bins);
+        if (ctx->opt_scheme == MUCA_SCHEME_RANDOM_SITE)   // the paper's own units: attempted flips per walker
+            rc = muca_run_iteration_random_site(ctx, (uint64_t)(30.0 * (double)w), (uint64_t)ctx->conv_n_updates, nullptr, ctx->n_bins);
+        else
+            rc = muca_run_iteration(ctx, th, sw, nullptr, ctx->n_bins);
         if (rc != MUCA_OK) return rc;
         muca_flatness_t fl;
         rc = muca_flatness(ctx->H.data(), ctx->n_bins, 0, &fl);
@@ -636,7 +645,10 @@ int muca_production(muca_ctx* ctx, int n_calls, int therm_sweeps, int sweeps, do
     const int bins = ctx->n_bins;
     std::vector<uint64_t> calls((size_t)n_calls * bins);
     for (int k = 0; k < n_calls; ++k) {
-        const int rc = muca_run_iteration(ctx, therm_sweeps, sweeps, calls.data() + (size_t)k * bins, bins);
+        const int rc = ctx->opt_scheme == MUCA_SCHEME_RANDOM_SITE
+                           ? muca_run_iteration_random_site(ctx, (uint64_t)therm_sweeps * (uint64_t)ctx->N,
+                                                            (uint64_t)sweeps * (uint64_t)ctx->N, calls.data() + (size_t)k * bins, bins)
+                           : muca_run_iteration(ctx, therm_sweeps, sweeps, calls.data() + (size_t)k * bins, bins);
         if (rc != MUCA_OK) return rc;
     }
     if (H_calls_out) std::memcpy(H_calls_out, calls.data(), sizeof(uint64_t) * calls.size());

@@ -113,12 +113,16 @@ def test_library_host_functions_match_the_oracle_protocol():
 
 # ------------------------------------------------------------------------------------------------ GPU parity
 @pytest.mark.gpu
-@pytest.mark.parametrize("L,W,seed,max_it", [(8, 128, 170700919, 60), (16, 512, 1, 25), (32, 300, 7, 8)])
-def test_gpu_converge_matches_oracle(L, W, seed, max_it):
+@pytest.mark.parametrize("L,W,seed,max_it,random_site", [(8, 128, 170700919, 60, False), (16, 512, 1, 25, False), (32, 300, 7, 8, False),
+                                                         (8, 128, 170700919, 60, True), (16, 512, 1, 25, True)])
+def test_gpu_converge_matches_oracle(L, W, seed, max_it, random_site):
+    from paper_1707_00919_b200 import binding as B
     g, o = mb.Muca(L, W, seed), mo.Oracle(L, W, seed)
     try:
+        if random_site:                          # the paper's own update scheme and units (R22)
+            g.set_option(B.MUCA_OPT_UPDATE_SCHEME, B.MUCA_SCHEME_RANDOM_SITE)
         lg, cg = g.converge(max_it, 1e-4)
-        lo, co = mc.converge(o, max_it, 1e-4, n_threads=mo.max_threads())
+        lo, co = mc.converge(o, max_it, 1e-4, n_threads=mo.max_threads(), random_site=random_site)
         assert cg == co and len(lg) == len(lo)
         for a, b in zip(lg, lo):
             for k in ("w", "therm_sweeps", "sweeps", "j_lo", "j_hi", "width", "n_updates"):
