@@ -53,13 +53,14 @@ typedef enum muca_status {
 } muca_status;
 
 /* Sweep-kernel variants (muca_set_option(ctx, MUCA_OPT_KERNEL, ...)).
- * AUTO picks RESIDENT for L <= 32 (lattices, threshold table and histogram in shared memory),
- * STREAMED_SMEM for L = 64 (table and histogram in shared memory, lattice rows streamed from HBM/L2)
- * and STREAMED for L = 128 (the table no longer fits: thresholds through L1). */
+ * AUTO picks RESIDENT for L <= 32 (lattices, threshold table and histogram in shared memory) and STREAMED_SMEM for
+ * L >= 64 (table and histogram in shared memory, lattice rows streamed from HBM/L2).  At L = 128 the table no longer
+ * fits: shared memory then holds a WINDOW of it around the walkers' energies; an iteration in which a walker leaves
+ * the window is detected and repeated from a snapshot with STREAMED (thresholds through L1) -- same results. */
 enum { MUCA_KERNEL_AUTO = 0, MUCA_KERNEL_RESIDENT = 1, MUCA_KERNEL_STREAMED = 2,
        MUCA_KERNEL_RESIDENT_V2 = 3, /* L <= 32 only: the earlier predicate-carried resident kernel, kept for A/B runs */
        MUCA_KERNEL_RESIDENT_V3 = 4, /* L <= 32 only: the earlier paired walker/deviate-warp kernel, kept for A/B runs */
-       MUCA_KERNEL_STREAMED_SMEM = 5 /* L = 32, 64: lattice rows streamed, threshold table + histogram in shared memory */ };
+       MUCA_KERNEL_STREAMED_SMEM = 5 /* L >= 32: lattice rows streamed, threshold table (or a window of it) + histogram in shared memory */ };
 enum {
     MUCA_OPT_KERNEL = 1,          /* one of MUCA_KERNEL_*                                        */
     MUCA_OPT_THREADS_PER_BLOCK = 2, /* walkers (= threads) per block; 0 = library default         */
@@ -67,10 +68,12 @@ enum {
                                           0 = only as needed to keep a block's uint32 bins from overflowing */
     MUCA_OPT_WALKERS_PER_WARP = 4, /* resident kernel, L <= 32: walkers served by one warp (1..32); 0 = spread
                                      the walkers evenly over all SMs */
-    MUCA_OPT_UPDATE_SCHEME = 5    /* update scheme of muca_converge / muca_production: MUCA_SCHEME_TYPEWRITER (default;
+    MUCA_OPT_UPDATE_SCHEME = 5,   /* update scheme of muca_converge / muca_production: MUCA_SCHEME_TYPEWRITER (default;
                                      schedule rounded up to whole sweeps, R18) or MUCA_SCHEME_RANDOM_SITE (the paper's
                                      own scheme and units: N_therm = 30 w and N_updates attempted flips per walker;
                                      muca_production then runs therm_sweeps * N and sweeps * N updates per call) */
+    MUCA_OPT_TABLE_WINDOW_ROWS = 6 /* STREAMED_SMEM kernel: rows of the threshold-table window held in shared memory;
+                                     0 = as many as fit.  A value below L*L+1 forces the windowed kernel (testing) */
 };
 enum { MUCA_SCHEME_TYPEWRITER = 0, MUCA_SCHEME_RANDOM_SITE = 1 };
 
@@ -222,6 +225,9 @@ int muca_get_thresholds(muca_ctx* ctx, uint32_t* out, size_t n);
 int muca_get_iteration(muca_ctx* ctx, uint32_t* n_out);
 int muca_set_iteration(muca_ctx* ctx, uint32_t n);
 int muca_last_sweep_ms(muca_ctx* ctx, double* ms_out, int* launches_out);
+/* windowed STREAMED_SMEM kernel: iterations run with a table window so far, and how many of them were repeated
+ * with STREAMED because a walker left the window. */
+int muca_window_stats(muca_ctx* ctx, int* windowed_iterations_out, int* fallbacks_out);
 const char* muca_last_error(const muca_ctx* ctx);
 
 /* Test hook: Philox4x32-10 evaluated ON THE DEVICE for n (ctr, key) pairs.

@@ -16,6 +16,7 @@ MUCA_KERNEL_AUTO, MUCA_KERNEL_RESIDENT, MUCA_KERNEL_STREAMED, MUCA_KERNEL_RESIDE
 MUCA_KERNEL_STREAMED_SMEM = 5
 MUCA_OPT_KERNEL, MUCA_OPT_THREADS_PER_BLOCK, MUCA_OPT_MAX_SWEEPS_PER_LAUNCH, MUCA_OPT_WALKERS_PER_WARP = 1, 2, 3, 4
 MUCA_OPT_UPDATE_SCHEME = 5
+MUCA_OPT_TABLE_WINDOW_ROWS = 6
 MUCA_SCHEME_TYPEWRITER, MUCA_SCHEME_RANDOM_SITE = 0, 1
 
 # every symbol include/muca.h declares (tests/test_abi.py checks the header against this list and the .so)
@@ -25,7 +26,7 @@ EXPORTS = (
     "muca_update_weights", "muca_update_weights_with", "muca_get_energies", "muca_get_spins", "muca_set_spins",
     "muca_unpack_spins_device", "muca_get_thresholds", "muca_get_iteration", "muca_set_iteration",
     "muca_last_sweep_ms", "muca_last_error", "muca_debug_philox", "muca_version",
-    "muca_flatness", "muca_schedule", "muca_converge", "muca_production", "muca_run_iteration_random_site",
+    "muca_flatness", "muca_schedule", "muca_converge", "muca_production", "muca_run_iteration_random_site", "muca_window_stats",
 )
 
 
@@ -96,6 +97,7 @@ def lib():
     L.muca_schedule.argtypes = [C.c_int, C.c_int, C.c_int, f64p, C.POINTER(C.c_int), C.POINTER(C.c_int),
                                 C.POINTER(C.c_int), C.POINTER(C.c_int)]
     L.muca_run_iteration_random_site.argtypes = [vp, C.c_uint64, C.c_uint64, u64p, C.c_int]
+    L.muca_window_stats.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int)]
     L.muca_production.argtypes = [vp, C.c_int, C.c_int, C.c_int, f64p, f64p, u64p, C.c_int]
     L.muca_converge.argtypes = [vp, C.c_int, C.c_double, C.POINTER(IterationLog), C.c_int, C.POINTER(C.c_int),
                                 C.POINTER(C.c_int)]
@@ -292,6 +294,11 @@ class Muca:
         self._check(self._lib.muca_production(self._h, int(n_calls), int(therm_sweeps), int(sweeps), _p(ln_om, C.c_double),
                                               _p(err, C.c_double), _p(Hs, C.c_uint64), self.n_bins), "muca_production")
         return ln_om, err, Hs
+
+    def window_stats(self):
+        a, b = C.c_int(), C.c_int()
+        self._check(self._lib.muca_window_stats(self._h, C.byref(a), C.byref(b)), "muca_window_stats")
+        return int(a.value), int(b.value)
 
     def last_sweep_ms(self):
         ms, k = C.c_double(), C.c_int()

@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SOURCES = [os.path.join(CSRC, "muca.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "muca_device.cuh"), os.path.join(CSRC, "muca_resident.cuh"), os.path.join(CSRC, "muca_random_site.cuh"),
+DEPS = SOURCES + [os.path.join(CSRC, "muca_device.cuh"), os.path.join(CSRC, "muca_resident.cuh"), os.path.join(CSRC, "muca_random_site.cuh"), os.path.join(CSRC, "muca_window.cuh"),
                   os.path.join(os.path.dirname(HERE), "include", "muca.h")]
 LIB = os.path.join(HERE, "libmuca_b200.so")
 

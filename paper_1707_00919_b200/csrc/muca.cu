@@ -14,6 +14,7 @@
 #include "muca_device.cuh"
 #include "muca_resident.cuh"
 #include "muca_random_site.cuh"
+#include "muca_window.cuh"
 
 using namespace muca;
 
@@ -43,6 +44,11 @@ struct muca_ctx {
     int opt_tpb = 0;
     int opt_max_sweeps = 0;
     int opt_wpw = 0;
+    int opt_window_rows = 0;        // MUCA_OPT_TABLE_WINDOW_ROWS: 0 = as many table rows as shared memory holds
+    void* d_snap = nullptr;         // snapshot of spins + E for the windowed kernel's fallback (lazily allocated)
+    int* d_flag = nullptr;          // device int[4]: window-left flag, smallest / largest slot of the walkers
+    int* h_flag = nullptr;          // pinned copy
+    int stat_window_iterations = 0, stat_window_fallbacks = 0;
     int conv_w_prev = 0;            // width covered by the previous iteration of muca_converge (0: none yet)
     double conv_n_updates = 0.0;    // N_updates (flips per walker) of the previous iteration of muca_converge
     int opt_scheme = MUCA_SCHEME_TYPEWRITER;   // update scheme used by muca_converge / muca_production
@@ -163,20 +169,22 @@ int launch_sweep_t(muca_ctx* ctx, const SweepParams& prm, int tpb) {
     return MUCA_OK;
 }
 
+constexpr int MODE_WINDOW = 6;   // sweep_kernel_window (muca_window.cuh): streamed lattices + a window of the table in shared memory
 struct Plan { int mode; int tpb; int nw; int wpw; };   // tpb = walkers per block; v5: nw warp pairs x wpw walkers per warp
 
 Plan make_plan(const muca_ctx* c) {
     Plan p;
     const int L = c->L;
     int kern = c->opt_kernel;
-    if (kern == MUCA_KERNEL_AUTO) kern = L <= 32 ? MUCA_KERNEL_RESIDENT : (L == 64 ? MUCA_KERNEL_STREAMED_SMEM : MUCA_KERNEL_STREAMED);
+    if (kern == MUCA_KERNEL_AUTO) kern = L <= 32 ? MUCA_KERNEL_RESIDENT : MUCA_KERNEL_STREAMED_SMEM;
     if (kern == MUCA_KERNEL_STREAMED && L < 32) kern = MUCA_KERNEL_RESIDENT;
     if ((kern == MUCA_KERNEL_RESIDENT_V2 || kern == MUCA_KERNEL_RESIDENT_V3) && L > 32) kern = MUCA_KERNEL_RESIDENT;
     p.nw = p.wpw = 0;
     if (kern == MUCA_KERNEL_RESIDENT) p.mode = L <= 32 ? MODE_V5 : MODE_TBL_L1;
     else if (kern == MUCA_KERNEL_RESIDENT_V3) p.mode = MODE_V3;
     else if (kern == MUCA_KERNEL_RESIDENT_V2) p.mode = MODE_TBL_SMEM;
-    else if (kern == MUCA_KERNEL_STREAMED_SMEM) p.mode = L >= 32 ? MODE_STREAMED_SMEM : MODE_V5;
+    else if (kern == MUCA_KERNEL_STREAMED_SMEM)
+        p.mode = L < 32 ? MODE_V5 : (L == 128 || c->opt_window_rows > 0) ? MODE_WINDOW : MODE_STREAMED_SMEM;
     else p.mode = MODE_STREAMED;
     if (p.mode == MODE_V5) {
         // spread the walkers over all SMs: as few warps per SM as possible, then as few lanes per warp as possible
@@ -197,7 +205,7 @@ Plan make_plan(const muca_ctx* c) {
         if (p.mode == MODE_V3) tpb = L == 32 ? 128 : 32;
         else if (p.mode == MODE_TBL_SMEM) tpb = 32;
         else if (p.mode == MODE_TBL_L1) tpb = L == 64 ? 64 : 32;
-        else if (p.mode == MODE_STREAMED_SMEM) {
+        else if (p.mode == MODE_STREAMED_SMEM || p.mode == MODE_WINDOW) {
             // one block per SM (164 KB of table at L = 64): spread the walkers over all SMs
             const int n_sm = c->n_sm > 0 ? c->n_sm : 148;
             tpb = ((c->W + n_sm - 1) / n_sm + 31) / 32 * 32;
@@ -210,6 +218,7 @@ Plan make_plan(const muca_ctx* c) {
 }
 
 size_t plan_smem(int L, const Plan& p) {
+    if (p.mode == MODE_WINDOW) return 0;   // sized at run time from what the device allows
     if (p.mode == MODE_V5) return L == 8 ? V5<8>::SMEM_BYTES : L == 16 ? V5<16>::SMEM_BYTES : V5<32>::SMEM_BYTES;
     if (p.mode == MODE_V3) return L == 8 ? V3<8>::SMEM_BYTES : L == 16 ? V3<16>::SMEM_BYTES : V3<32>::SMEM_BYTES;
     switch (L) {
@@ -226,6 +235,31 @@ size_t plan_smem(int L, const Plan& p) {
                         : p.mode == MODE_STREAMED ? sweep_smem_bytes<128, MODE_STREAMED>(p.tpb)
                                                 : sweep_smem_bytes<128, MODE_TBL_L1>(p.tpb);
     }
+}
+
+struct Window { int j_lo = 0, n_rows = 0, sent_lo = 0, sent_hi = 0; };
+
+template <int L>
+int launch_window_t(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& win) {
+    const size_t smem = window_smem_bytes(win.n_rows);
+    static size_t configured = 0;
+    if (smem > configured) {
+        CU(cudaFuncSetAttribute(sweep_kernel_window<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured = smem;
+    }
+    sweep_kernel_window<L><<<(prm.W + tpb - 1) / tpb, tpb, smem, ctx->stream>>>(prm, win.j_lo, win.n_rows, win.sent_lo,
+                                                                               win.sent_hi, ctx->d_flag);
+    CU(cudaGetLastError());
+    return MUCA_OK;
+}
+
+int launch_window(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& win) {
+    switch (ctx->L) {
+        case 32: return launch_window_t<32>(ctx, prm, tpb, win);
+        case 64: return launch_window_t<64>(ctx, prm, tpb, win);
+        case 128: return launch_window_t<128>(ctx, prm, tpb, win);
+    }
+    return fail(ctx, MUCA_EINVAL, "windowed kernel: L must be 32, 64 or 128");
 }
 
 int launch_sweep(muca_ctx* ctx, const SweepParams& prm, const Plan& p) {
@@ -257,7 +291,6 @@ int launch_sweep(muca_ctx* ctx, const SweepParams& prm, const Plan& p) {
             if (p.mode == MODE_STREAMED_SMEM) return launch_sweep_t<64, MODE_STREAMED_SMEM>(ctx, prm, p.tpb);
             return launch_sweep_t<64, MODE_TBL_L1>(ctx, prm, p.tpb);
         case 128:
-            if (p.mode == MODE_STREAMED_SMEM) return fail(ctx, MUCA_EINVAL, "L=128: the threshold table does not fit in shared memory");
             if (p.mode == MODE_STREAMED) return launch_sweep_t<128, MODE_STREAMED>(ctx, prm, p.tpb);
             return launch_sweep_t<128, MODE_TBL_L1>(ctx, prm, p.tpb);
     }
@@ -291,6 +324,7 @@ int create_common(muca_ctx** out, int L, int W, uint64_t seed, uint32_t walker_o
     ctx->H.assign(ctx->n_bins, 0);
     if (cudaMallocHost((void**)&ctx->h_table, (size_t)ctx->n_bins * 8 * 4) != cudaSuccess ||
         cudaMallocHost((void**)&ctx->h_H, (size_t)ctx->n_bins * 8) != cudaSuccess ||
+        cudaMallocHost((void**)&ctx->h_flag, 4 * sizeof(int)) != cudaSuccess || cudaMalloc((void**)&ctx->d_flag, 4 * sizeof(int)) != cudaSuccess ||
         cudaEventCreate(&ctx->ev0) != cudaSuccess || cudaEventCreate(&ctx->ev1) != cudaSuccess)
         return bail(MUCA_ECUDA);
     {
@@ -357,6 +391,9 @@ void muca_destroy(muca_ctx* ctx) {
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
     if (ctx->d_stage) cudaFree(ctx->d_stage);
+    if (ctx->d_snap) cudaFree(ctx->d_snap);
+    if (ctx->d_flag) cudaFree(ctx->d_flag);
+    if (ctx->h_flag) cudaFreeHost(ctx->h_flag);
     if (ctx->own_workspace && ctx->d_workspace) cudaFree(ctx->d_workspace);
     delete ctx;
 }
@@ -376,6 +413,11 @@ int muca_set_option(muca_ctx* ctx, int option, int value) {
     if (option == MUCA_OPT_WALKERS_PER_WARP) {
         if (value < 0 || value > 32) return fail(ctx, MUCA_EINVAL, "walkers per warp must be in [0, 32]");
         ctx->opt_wpw = value;
+        return MUCA_OK;
+    }
+    if (option == MUCA_OPT_TABLE_WINDOW_ROWS) {
+        if (value < 0) return fail(ctx, MUCA_EINVAL, "table window rows must be >= 0");
+        ctx->opt_window_rows = value;
         return MUCA_OK;
     }
     if (option == MUCA_OPT_UPDATE_SCHEME) {
@@ -410,9 +452,10 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
     if (n_bins != ctx->n_bins || therm_sweeps < 0 || sweeps < 0)
         return fail(ctx, MUCA_EINVAL, "run_iteration: n_bins must be %d, sweeps >= 0", ctx->n_bins);
     if (ctx->iteration == 0xFFFFFFFFu) return fail(ctx, MUCA_ERANGE, "iteration counter exhausted");
-    const Plan plan = make_plan(ctx);
+    Plan plan = make_plan(ctx);
+    int max_smem = 0;
     {
-        int dev = 0, max_smem = 0;
+        int dev = 0;
         CU(cudaGetDevice(&dev));
         CU(cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
         if (plan_smem(ctx->L, plan) > (size_t)max_smem)
@@ -426,30 +469,89 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
     CU(cudaMemcpyAsync(ctx->d_table, ctx->h_table, (size_t)ctx->n_bins * 8 * 4, cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaMemsetAsync(ctx->d_H, 0, (size_t)ctx->n_bins * 8, ctx->stream));
 
-    // a2-a4: sweeps.  A block's uint32 bins must not overflow: tpb * measured sweeps * N < 2^32 per launch.
     const uint64_t total = (uint64_t)therm_sweeps + (uint64_t)sweeps;
     if (total > 0xFFFFFFFFull) return fail(ctx, MUCA_EINVAL, "too many sweeps");
-    uint64_t max_meas = 0xFFFFFFFFull / ((uint64_t)plan.tpb * (uint64_t)ctx->N);
-    if (max_meas < 1) max_meas = 1;
-    const uint64_t max_any = ctx->opt_max_sweeps > 0 ? (uint64_t)ctx->opt_max_sweeps : total + 1;
+
+    // windowed table (muca_window.cuh): pick the window around the walkers' slots, keep a snapshot for the fallback
+    Plan fallback;
+    fallback.mode = MODE_STREAMED; fallback.tpb = 32; fallback.nw = fallback.wpw = 0;
+    Window win;
+    bool guarded = false;   // the window has sentinel rows: the result counts only if no walker entered one
+    if (plan.mode == MODE_WINDOW) {
+        const size_t spin_bytes = (size_t)ctx->W * (ctx->N / 8);
+        ctx->h_flag[0] = 0; ctx->h_flag[1] = 0x7FFFFFFF; ctx->h_flag[2] = -1;
+        CU(cudaMemcpyAsync(ctx->d_flag, ctx->h_flag, 3 * sizeof(int), cudaMemcpyHostToDevice, ctx->stream));
+        slot_range_kernel<<<148, 256, 0, ctx->stream>>>(ctx->d_E, ctx->W, ctx->N, ctx->d_flag + 1);
+        CU(cudaGetLastError());
+        CU(cudaMemcpyAsync(ctx->h_flag, ctx->d_flag, 3 * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        const int lo = ctx->h_flag[1], hi = ctx->h_flag[2];
+        int cap = (int)(((size_t)max_smem - 1024) / (ROW_SMEM_WORDS * 4)) - 2 * WINDOW_PAD_ROWS;
+        if (ctx->opt_window_rows > 0 && ctx->opt_window_rows < cap) cap = ctx->opt_window_rows;
+        const int margin = 8;   // rows between the outermost walker and a sentinel at the start of the iteration
+        if (cap >= ctx->n_bins) {
+            win.j_lo = 0; win.n_rows = ctx->n_bins;                          // the whole table fits: nothing to guard
+        } else if (hi - lo + 1 + 2 * (2 + margin) > cap) {
+            plan = fallback;                                                  // the walkers are spread too widely
+        } else {
+            int j_lo = lo - (cap - (hi - lo + 1)) / 2;
+            if (j_lo < 0) j_lo = 0;
+            if (j_lo + cap > ctx->n_bins) j_lo = ctx->n_bins - cap;
+            win.j_lo = j_lo; win.n_rows = cap;
+            win.sent_lo = j_lo > 0 ? 2 : 0;
+            win.sent_hi = j_lo + cap < ctx->n_bins ? 2 : 0;
+            guarded = true;
+            if (!ctx->d_snap) CU(cudaMalloc(&ctx->d_snap, align_up(spin_bytes) + (size_t)ctx->W * 4));
+            CU(cudaMemcpyAsync(ctx->d_snap, ctx->d_spins, spin_bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+            CU(cudaMemcpyAsync((char*)ctx->d_snap + align_up(spin_bytes), ctx->d_E, (size_t)ctx->W * 4, cudaMemcpyDeviceToDevice, ctx->stream));
+        }
+        if (plan.mode == MODE_WINDOW) ctx->stat_window_iterations += 1;
+    }
+
+    // a2-a4: sweeps.  A block's uint32 bins must not overflow: tpb * measured sweeps * N < 2^32 per launch.
     SweepParams prm;
     prm.spins = ctx->d_spins; prm.E = ctx->d_E; prm.table = ctx->d_table; prm.H = ctx->d_H;
     prm.W = ctx->W; prm.walker_offset = ctx->walker_offset;
     prm.key0 = (uint32_t)(ctx->seed & 0xFFFFFFFFull); prm.key1 = (uint32_t)(ctx->seed >> 32);
     prm.iteration = ctx->iteration; prm.therm = (uint32_t)therm_sweeps;
     int launches = 0;
+    auto run_sweeps = [&](const Plan& pl) -> int {
+        uint64_t max_meas = 0xFFFFFFFFull / ((uint64_t)pl.tpb * (uint64_t)ctx->N);
+        if (pl.mode == MODE_WINDOW) max_meas = 0xFFFFFFFFull / ((uint64_t)pl.tpb * (uint64_t)ctx->N) / 2;   // thermalisation counts too
+        if (max_meas < 1) max_meas = 1;
+        const uint64_t max_any = ctx->opt_max_sweeps > 0 ? (uint64_t)ctx->opt_max_sweeps
+                                 : (pl.mode == MODE_WINDOW ? max_meas : total + 1);
+        uint64_t s = 0;
+        while (s < total) {
+            uint64_t e = total;
+            const uint64_t meas_begin = s > (uint64_t)therm_sweeps ? s : (uint64_t)therm_sweeps;
+            if (e > meas_begin + max_meas) e = meas_begin + max_meas;
+            if (e > s + max_any) e = s + max_any;
+            prm.sweep_begin = (uint32_t)s; prm.sweep_end = (uint32_t)e;
+            const int rc = pl.mode == MODE_WINDOW ? launch_window(ctx, prm, pl.tpb, win) : launch_sweep(ctx, prm, pl);
+            if (rc != MUCA_OK) return rc;
+            ++launches;
+            s = e;
+        }
+        return MUCA_OK;
+    };
     CU(cudaEventRecord(ctx->ev0, ctx->stream));
-    uint64_t s = 0;
-    while (s < total) {
-        uint64_t e = total;
-        const uint64_t meas_begin = s > (uint64_t)therm_sweeps ? s : (uint64_t)therm_sweeps;
-        if (e > meas_begin + max_meas) e = meas_begin + max_meas;
-        if (e > s + max_any) e = s + max_any;
-        prm.sweep_begin = (uint32_t)s; prm.sweep_end = (uint32_t)e;
-        const int rc = launch_sweep(ctx, prm, plan);
+    {
+        const int rc = run_sweeps(plan);
         if (rc != MUCA_OK) return rc;
-        ++launches;
-        s = e;
+    }
+    if (plan.mode == MODE_WINDOW && guarded) {
+        CU(cudaMemcpyAsync(ctx->h_flag, ctx->d_flag, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        if (ctx->h_flag[0]) {   // a walker left the window: repeat the iteration from the snapshot with the L1 kernel
+            const size_t spin_bytes = (size_t)ctx->W * (ctx->N / 8);
+            CU(cudaMemcpyAsync(ctx->d_spins, ctx->d_snap, spin_bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+            CU(cudaMemcpyAsync(ctx->d_E, (char*)ctx->d_snap + align_up(spin_bytes), (size_t)ctx->W * 4, cudaMemcpyDeviceToDevice, ctx->stream));
+            CU(cudaMemsetAsync(ctx->d_H, 0, (size_t)ctx->n_bins * 8, ctx->stream));
+            ctx->stat_window_fallbacks += 1;
+            const int rc = run_sweeps(fallback);
+            if (rc != MUCA_OK) return rc;
+        }
     }
     CU(cudaEventRecord(ctx->ev1, ctx->stream));
     CU(cudaMemcpyAsync(ctx->h_H, ctx->d_H, (size_t)ctx->n_bins * 8, cudaMemcpyDeviceToHost, ctx->stream));
@@ -746,6 +848,13 @@ int muca_last_sweep_ms(muca_ctx* ctx, double* ms_out, int* launches_out) {
     if (!ctx) return MUCA_EINVAL;
     if (ms_out) *ms_out = ctx->last_sweep_ms;
     if (launches_out) *launches_out = ctx->last_launches;
+    return MUCA_OK;
+}
+
+int muca_window_stats(muca_ctx* ctx, int* windowed_iterations_out, int* fallbacks_out) {
+    if (!ctx) return MUCA_EINVAL;
+    if (windowed_iterations_out) *windowed_iterations_out = ctx->stat_window_iterations;
+    if (fallbacks_out) *fallbacks_out = ctx->stat_window_fallbacks;
     return MUCA_OK;
 }
 

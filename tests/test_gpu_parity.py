@@ -185,6 +185,32 @@ def test_resident_walkers_per_warp(L, W, tpb, wpw):
     run_pair(L, W, EXTRA_SEEDS[1], 3, 2, {8: 30, 16: 12, 32: 6}[L], offset=3, options=tuple(opts), check_every=False)
 
 
+# L = 128 default: a WINDOW of the threshold table in shared memory; an iteration in which a walker leaves the window is
+# repeated from a snapshot with the L1 kernel.  Small forced windows exercise that fallback; the chains must not change.
+@pytest.mark.parametrize("L,W,rows,iters,therm,sweeps,expect_fallback", [
+    (128, 70, 0, 3, 2, 5, False), (128, 70, 600, 4, 2, 6, None), (64, 150, 300, 6, 3, 12, None),
+    (32, 200, 120, 8, 5, 40, True), (32, 100, 40, 3, 2, 10, None),
+])
+def test_windowed_table_and_fallback(L, W, rows, iters, therm, sweeps, expect_fallback):
+    g, o = mb.Muca(L, W, PRIMARY_SEED, walker_offset=4), mo.Oracle(L, W, PRIMARY_SEED, walker_offset=4)
+    try:
+        g.set_option(B.MUCA_OPT_KERNEL, B.MUCA_KERNEL_STREAMED_SMEM)
+        if rows:
+            g.set_option(B.MUCA_OPT_TABLE_WINDOW_ROWS, rows)
+        for it in range(iters):
+            Hg, Ho = g.run_iteration(therm, sweeps), o.run_iteration(therm, sweeps, n_threads=mo.max_threads())
+            assert np.array_equal(Hg, Ho), f"it{it}: H differs in slots {np.nonzero(Hg != Ho)[0][:8]}"
+            compare_state(g, o, f"it{it}")
+            g.update_weights(); o.update_weights()
+        windowed, fallbacks = g.window_stats()
+        if expect_fallback is True:
+            assert windowed > 0 and fallbacks > 0, (windowed, fallbacks)
+        if expect_fallback is False:
+            assert windowed == iters and fallbacks == 0, (windowed, fallbacks)
+    finally:
+        g.close(); o.close()
+
+
 def test_split_launches_give_the_same_iteration():
     # an iteration split into several launches (the uint32-bin overflow guard) is the same Markov chain
     run_pair(32, 70, PRIMARY_SEED, 3, 3, 9, options=((B.MUCA_OPT_MAX_SWEEPS_PER_LAUNCH, 2),))
