@@ -253,7 +253,7 @@ def run_ours(args, cfg):
     peak = SM_COUNT * SCHED_PER_SM * ALU_LANES * f_max_hz / 1e12
     issue_peak = SM_COUNT * SCHED_PER_SM * ISSUE_LANES * f_max_hz / 1e12
     kernel = "muca::sweep_kernel_v5<%d>" % cfg.L if cfg.L <= 32 else \
-        "muca::sweep_kernel<%d, %s>" % (cfg.L, "STREAMED_SMEM" if cfg.L == 64 else "STREAMED")
+        ("muca::sweep_kernel<64, STREAMED_SMEM>" if cfg.L == 64 else "muca::sweep_kernel_window<%d>" % cfg.L)
     roofline = {
         "bound": "alu", "achieved": achieved, "peak": peak, "unit": "T lane-ops/s on the ALU pipe", "frac": achieved / peak,
         "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(cfg.name) if world == 1 else None,
