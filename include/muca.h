@@ -63,7 +63,9 @@ enum { MUCA_KERNEL_AUTO = 0, MUCA_KERNEL_RESIDENT = 1, MUCA_KERNEL_STREAMED = 2,
        MUCA_KERNEL_STREAMED_SMEM = 5 /* L >= 32: lattice rows streamed, threshold table (or a window of it) + histogram in shared memory */ };
 enum {
     MUCA_OPT_KERNEL = 1,          /* one of MUCA_KERNEL_*                                        */
-    MUCA_OPT_THREADS_PER_BLOCK = 2, /* walkers (= threads) per block; 0 = library default         */
+    MUCA_OPT_THREADS_PER_BLOCK = 2, /* walkers per block (a multiple of 32); 0 = library default (walkers spread over all
+                                      SMs).  RESIDENT, L <= 32: value / 32 (at most 4) walker warps, each paired with a
+                                      deviate warp, i.e. twice as many threads */
     MUCA_OPT_MAX_SWEEPS_PER_LAUNCH = 3, /* split an iteration into launches of at most this many sweeps;
                                           0 = only as needed to keep a block's uint32 bins from overflowing */
     MUCA_OPT_WALKERS_PER_WARP = 4, /* resident kernel, L <= 32: walkers served by one warp (1..32); 0 = spread
