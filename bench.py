@@ -18,7 +18,6 @@ import argparse
 import json
 import os
 import sys
-import threading
 import time
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
@@ -105,45 +104,48 @@ def run_reference(args, cfg):
 
 
 # ------------------------------------------------------------------------------------------------ clocks
-class ClockSampler(threading.Thread):
+class ClockSampler:
+    """SM clock and throttle reasons through NVML, sampled from the MAIN thread between the kernels of the timed
+    region (after every iteration).  A background thread polling NVML contends with the CUDA calls of the job for a
+    driver lock: single queries then took up to 0.8 s and stalled kernel launches (profiles/README.md)."""
+
     def __init__(self, index):
-        super().__init__(daemon=True)
-        self.index, self.stop_flag, self.sm, self.reasons, self.max_mhz = index, False, [], set(), None
+        self.sm, self.reasons, self.max_mhz = [], set(), None
         try:
             import pynvml
             pynvml.nvmlInit()
             self.nv = pynvml
             self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
             self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            nv = pynvml
+            self.names = {nv.nvmlClocksEventReasonHwSlowdown: "hw_slowdown", nv.nvmlClocksEventReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                          nv.nvmlClocksEventReasonSwThermalSlowdown: "sw_thermal_slowdown", nv.nvmlClocksEventReasonSwPowerCap: "sw_power_cap"} \
+                if hasattr(nv, "nvmlClocksEventReasonHwSlowdown") else \
+                {nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown", nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown", nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap"}
         except Exception:
             self.nv = None
 
-    def run(self):
+    def sample(self):
         if self.nv is None:
             return
         nv = self.nv
-        names = {nv.nvmlClocksEventReasonHwSlowdown: "hw_slowdown", nv.nvmlClocksEventReasonHwThermalSlowdown: "hw_thermal_slowdown",
-                 nv.nvmlClocksEventReasonSwThermalSlowdown: "sw_thermal_slowdown", nv.nvmlClocksEventReasonSwPowerCap: "sw_power_cap"} \
-            if hasattr(nv, "nvmlClocksEventReasonHwSlowdown") else \
-            {nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown", nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
-             nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown", nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap"}
-        while not self.stop_flag:
+        try:
+            self.sm.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
             try:
-                self.sm.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
-                try:
-                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
-                except Exception:
-                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
-                for bit, name in names.items():
-                    if r & bit:
-                        self.reasons.add(name)
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
             except Exception:
-                pass
-            time.sleep(0.02)
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+            for bit, name in self.names.items():
+                if r & bit:
+                    self.reasons.add(name)
+        except Exception:
+            pass
 
     def result(self):
         return {"sm_mhz": float(np.median(self.sm)) if self.sm else None, "sm_max_mhz": self.max_mhz,
-                "reasons": sorted(self.reasons), "samples": len(self.sm)}
+                "reasons": sorted(self.reasons), "samples": len(self.sm),
+                "how": "NVML from the main thread after every iteration of the timed steps"}
 
 
 # ------------------------------------------------------------------------------------------------ our arm
@@ -174,6 +176,7 @@ def run_ours(args, cfg):
     Hbuf = torch.zeros(cfg.n_bins, dtype=torch.int64, device=dev)
 
     stats = {"sweep_ms": 0.0, "sweep_launches": 0, "launches": 0}
+    sampler = ClockSampler(local)
 
     def job(e2e: bool, record: bool):
         g = mb.Muca(cfg.L, W, cfg.seed, walker_offset=offset)                  # a0 (init kernel)
@@ -184,6 +187,7 @@ def run_ours(args, cfg):
             n_launch += k
             if record:
                 stats["sweep_ms"] += ms; stats["sweep_launches"] += k
+                sampler.sample()                                               # clocks line of the contract (see ClockSampler)
             if world > 1:                                                      # the one exchange of the method
                 Hbuf.copy_(torch.from_numpy(H.astype(np.int64)))
                 dist.all_reduce(Hbuf)
@@ -215,22 +219,20 @@ def run_ours(args, cfg):
 
     for _ in range(max(args.warmup, 3)):
         job(False, False)
-    job(True, False)
 
     def bracket():
         torch.cuda.synchronize()
         if world > 1:
             dist.barrier()
 
-    sampler = ClockSampler(local)
+    job(True, False)
+    sampler.sample()            # first NVML queries outside the timed region
+    sampler.sm.clear(); sampler.reasons.clear()
     bracket()
-    sampler.start()
     ms_dev = timed(False, args.steps, True)
     bracket()
     ms_e2e = timed(True, args.steps, False)
     bracket()
-    sampler.stop_flag = True
-    sampler.join(timeout=1.0)
 
     t = torch.tensor([ms_dev, ms_e2e], dtype=torch.float64, device=dev)
     if world > 1:
@@ -253,7 +255,7 @@ def run_ours(args, cfg):
     peak = SM_COUNT * SCHED_PER_SM * ALU_LANES * f_max_hz / 1e12
     issue_peak = SM_COUNT * SCHED_PER_SM * ISSUE_LANES * f_max_hz / 1e12
     kernel = "muca::sweep_kernel_v5<%d>" % cfg.L if cfg.L <= 32 else \
-        ("muca::sweep_kernel<64, STREAMED_SMEM>" if cfg.L == 64 else "muca::sweep_kernel_window<%d>" % cfg.L)
+        "muca::sweep_kernel_wpair<%d>" % cfg.L
     roofline = {
         "bound": "alu", "achieved": achieved, "peak": peak, "unit": "T lane-ops/s on the ALU pipe", "frac": achieved / peak,
         "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(cfg.name) if world == 1 else None,

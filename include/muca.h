@@ -53,14 +53,16 @@ typedef enum muca_status {
 } muca_status;
 
 /* Sweep-kernel variants (muca_set_option(ctx, MUCA_OPT_KERNEL, ...)).
- * AUTO picks RESIDENT for L <= 32 (lattices, threshold table and histogram in shared memory) and STREAMED_SMEM for
- * L >= 64 (table and histogram in shared memory, lattice rows streamed from HBM/L2).  At L = 128 the table no longer
+ * AUTO picks RESIDENT for L <= 32 (lattices, threshold table and histogram in shared memory) and STREAMED_PAIRS for
+ * L >= 64 (table and histogram in shared memory, lattice rows streamed from HBM/L2, Philox in paired deviate warps;
+ * STREAMED_SMEM is the same with Philox in the walker thread).  At L = 128 the table no longer
  * fits: shared memory then holds a WINDOW of it around the walkers' energies; an iteration in which a walker leaves
  * the window is detected and repeated from a snapshot with STREAMED (thresholds through L1) -- same results. */
 enum { MUCA_KERNEL_AUTO = 0, MUCA_KERNEL_RESIDENT = 1, MUCA_KERNEL_STREAMED = 2,
        MUCA_KERNEL_RESIDENT_V2 = 3, /* L <= 32 only: the earlier predicate-carried resident kernel, kept for A/B runs */
        MUCA_KERNEL_RESIDENT_V3 = 4, /* L <= 32 only: the earlier paired walker/deviate-warp kernel, kept for A/B runs */
-       MUCA_KERNEL_STREAMED_SMEM = 5 /* L >= 32: lattice rows streamed, threshold table (or a window of it) + histogram in shared memory */ };
+       MUCA_KERNEL_STREAMED_SMEM = 5, /* L >= 32: lattice rows streamed, threshold table (or a window of it) + histogram in shared memory */
+       MUCA_KERNEL_STREAMED_PAIRS = 6 /* L >= 32: the same with Philox in paired deviate warps (as in RESIDENT) */ };
 enum {
     MUCA_OPT_KERNEL = 1,          /* one of MUCA_KERNEL_*                                        */
     MUCA_OPT_THREADS_PER_BLOCK = 2, /* walkers per block (a multiple of 32); 0 = library default (walkers spread over all

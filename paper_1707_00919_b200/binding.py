@@ -14,6 +14,7 @@ from . import build as _build
 MUCA_OK = 0
 MUCA_KERNEL_AUTO, MUCA_KERNEL_RESIDENT, MUCA_KERNEL_STREAMED, MUCA_KERNEL_RESIDENT_V2, MUCA_KERNEL_RESIDENT_V3 = 0, 1, 2, 3, 4
 MUCA_KERNEL_STREAMED_SMEM = 5
+MUCA_KERNEL_STREAMED_PAIRS = 6
 MUCA_OPT_KERNEL, MUCA_OPT_THREADS_PER_BLOCK, MUCA_OPT_MAX_SWEEPS_PER_LAUNCH, MUCA_OPT_WALKERS_PER_WARP = 1, 2, 3, 4
 MUCA_OPT_UPDATE_SCHEME = 5
 MUCA_OPT_TABLE_WINDOW_ROWS = 6

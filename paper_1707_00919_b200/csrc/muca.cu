@@ -31,7 +31,8 @@ struct muca_ctx {
     int32_t* d_E = nullptr;
     uint32_t* d_table = nullptr;
     unsigned long long* d_H = nullptr;
-    void* d_stage = nullptr;        // lazily allocated W*N bytes for muca_get_spins / muca_set_spins
+    void* d_stage = nullptr;        // W*N bytes for muca_get_spins / muca_set_spins (in the workspace: a cudaMalloc per
+                                    // context of 128 MB at configs 4 and 5 stalled for up to 0.3 s now and then)
     // host state
     std::vector<double> logw;       // omega, n_bins
     std::vector<uint64_t> H;        // last histogram
@@ -45,9 +46,9 @@ struct muca_ctx {
     int opt_max_sweeps = 0;
     int opt_wpw = 0;
     int opt_window_rows = 0;        // MUCA_OPT_TABLE_WINDOW_ROWS: 0 = as many table rows as shared memory holds
-    void* d_snap = nullptr;         // snapshot of spins + E for the windowed kernel's fallback (lazily allocated)
+    void* d_snap = nullptr;         // snapshot of spins + E for the windowed kernels' fallback (in the workspace, L >= 32)
     int* d_flag = nullptr;          // device int[4]: window-left flag, smallest / largest slot of the walkers
-    int* h_flag = nullptr;          // pinned copy
+    int* h_flag = nullptr;          // pinned copy (tail of h_H's allocation)
     int stat_window_iterations = 0, stat_window_fallbacks = 0;
     int conv_w_prev = 0;            // width covered by the previous iteration of muca_converge (0: none yet)
     double conv_n_updates = 0.0;    // N_updates (flips per walker) of the previous iteration of muca_converge
@@ -64,7 +65,7 @@ inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 bool valid_L(int L) { return L == 8 || L == 16 || L == 32 || L == 64 || L == 128; }
 
-struct Carve { size_t spins, E, table, H, total; };
+struct Carve { size_t spins, E, table, H, flag, snap, stage, total; };
 Carve carve(int L, int W) {
     const size_t N = (size_t)L * L, bins = N + 1;
     Carve c;
@@ -73,6 +74,9 @@ Carve carve(int L, int W) {
     c.E = off;     off += align_up((size_t)W * 4);
     c.table = off; off += align_up(bins * 8 * 4);
     c.H = off;     off += align_up(bins * 8);
+    c.flag = off;  off += align_up(4 * sizeof(int));                       // windowed kernels: left-the-window flag, slot range
+    c.snap = off;  off += L >= 32 ? align_up((size_t)W * (N / 8)) + align_up((size_t)W * 4) : 0;   // and their snapshot of spins + E
+    c.stage = off; off += align_up((size_t)W * N);                        // int8 spins of muca_get_spins / muca_set_spins
     c.total = off;
     return c;
 }
@@ -169,6 +173,7 @@ int launch_sweep_t(muca_ctx* ctx, const SweepParams& prm, int tpb) {
     return MUCA_OK;
 }
 
+constexpr int MODE_WPAIR = 7;    // sweep_kernel_wpair: the same with Philox in paired deviate warps
 constexpr int MODE_WINDOW = 6;   // sweep_kernel_window (muca_window.cuh): streamed lattices + a window of the table in shared memory
 struct Plan { int mode; int tpb; int nw; int wpw; };   // tpb = walkers per block; v5: nw warp pairs x wpw walkers per warp
 
@@ -176,13 +181,14 @@ Plan make_plan(const muca_ctx* c) {
     Plan p;
     const int L = c->L;
     int kern = c->opt_kernel;
-    if (kern == MUCA_KERNEL_AUTO) kern = L <= 32 ? MUCA_KERNEL_RESIDENT : MUCA_KERNEL_STREAMED_SMEM;
+    if (kern == MUCA_KERNEL_AUTO) kern = L <= 32 ? MUCA_KERNEL_RESIDENT : MUCA_KERNEL_STREAMED_PAIRS;
     if (kern == MUCA_KERNEL_STREAMED && L < 32) kern = MUCA_KERNEL_RESIDENT;
     if ((kern == MUCA_KERNEL_RESIDENT_V2 || kern == MUCA_KERNEL_RESIDENT_V3) && L > 32) kern = MUCA_KERNEL_RESIDENT;
     p.nw = p.wpw = 0;
     if (kern == MUCA_KERNEL_RESIDENT) p.mode = L <= 32 ? MODE_V5 : MODE_TBL_L1;
     else if (kern == MUCA_KERNEL_RESIDENT_V3) p.mode = MODE_V3;
     else if (kern == MUCA_KERNEL_RESIDENT_V2) p.mode = MODE_TBL_SMEM;
+    else if (kern == MUCA_KERNEL_STREAMED_PAIRS) p.mode = L < 32 ? MODE_V5 : MODE_WPAIR;
     else if (kern == MUCA_KERNEL_STREAMED_SMEM)
         p.mode = L < 32 ? MODE_V5 : (L == 128 || c->opt_window_rows > 0) ? MODE_WINDOW : MODE_STREAMED_SMEM;
     else p.mode = MODE_STREAMED;
@@ -205,11 +211,12 @@ Plan make_plan(const muca_ctx* c) {
         if (p.mode == MODE_V3) tpb = L == 32 ? 128 : 32;
         else if (p.mode == MODE_TBL_SMEM) tpb = 32;
         else if (p.mode == MODE_TBL_L1) tpb = L == 64 ? 64 : 32;
-        else if (p.mode == MODE_STREAMED_SMEM || p.mode == MODE_WINDOW) {
+        else if (p.mode == MODE_STREAMED_SMEM || p.mode == MODE_WINDOW || p.mode == MODE_WPAIR) {
             // one block per SM (164 KB of table at L = 64): spread the walkers over all SMs
             const int n_sm = c->n_sm > 0 ? c->n_sm : 148;
             tpb = ((c->W + n_sm - 1) / n_sm + 31) / 32 * 32;
             if (tpb > 512) tpb = 512;
+            if (p.mode == MODE_WPAIR && tpb > 32 * WPAIR_MAX_PAIRS) tpb = 32 * WPAIR_MAX_PAIRS;
         }
         else tpb = 32;
     }
@@ -218,7 +225,7 @@ Plan make_plan(const muca_ctx* c) {
 }
 
 size_t plan_smem(int L, const Plan& p) {
-    if (p.mode == MODE_WINDOW) return 0;   // sized at run time from what the device allows
+    if (p.mode == MODE_WINDOW || p.mode == MODE_WPAIR) return 0;   // sized at run time from what the device allows
     if (p.mode == MODE_V5) return L == 8 ? V5<8>::SMEM_BYTES : L == 16 ? V5<16>::SMEM_BYTES : V5<32>::SMEM_BYTES;
     if (p.mode == MODE_V3) return L == 8 ? V3<8>::SMEM_BYTES : L == 16 ? V3<16>::SMEM_BYTES : V3<32>::SMEM_BYTES;
     switch (L) {
@@ -251,6 +258,30 @@ int launch_window_t(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window
                                                                                win.sent_hi, ctx->d_flag);
     CU(cudaGetLastError());
     return MUCA_OK;
+}
+
+template <int L>
+int launch_wpair_t(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& win) {
+    const int npairs = tpb / 32;
+    const size_t smem = wpair_smem_bytes(win.n_rows, npairs);
+    static size_t configured = 0;
+    if (smem > configured) {
+        CU(cudaFuncSetAttribute(sweep_kernel_wpair<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured = smem;
+    }
+    sweep_kernel_wpair<L><<<(prm.W + tpb - 1) / tpb, 2 * tpb, smem, ctx->stream>>>(prm, win.j_lo, win.n_rows, win.sent_lo,
+                                                                                  win.sent_hi, ctx->d_flag);
+    CU(cudaGetLastError());
+    return MUCA_OK;
+}
+
+int launch_wpair(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& win) {
+    switch (ctx->L) {
+        case 32: return launch_wpair_t<32>(ctx, prm, tpb, win);
+        case 64: return launch_wpair_t<64>(ctx, prm, tpb, win);
+        case 128: return launch_wpair_t<128>(ctx, prm, tpb, win);
+    }
+    return fail(ctx, MUCA_EINVAL, "paired streamed kernel: L must be 32, 64 or 128");
 }
 
 int launch_window(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& win) {
@@ -320,13 +351,16 @@ int create_common(muca_ctx** out, int L, int W, uint64_t seed, uint32_t walker_o
     ctx->d_E = (int32_t*)(base + c.E);
     ctx->d_table = (uint32_t*)(base + c.table);
     ctx->d_H = (unsigned long long*)(base + c.H);
+    ctx->d_flag = (int*)(base + c.flag);
+    ctx->d_stage = (void*)(base + c.stage);
+    ctx->d_snap = L >= 32 ? (void*)(base + c.snap) : nullptr;
     ctx->logw.assign(ctx->n_bins, 0.0);   // R2: omega == 0
     ctx->H.assign(ctx->n_bins, 0);
     if (cudaMallocHost((void**)&ctx->h_table, (size_t)ctx->n_bins * 8 * 4) != cudaSuccess ||
-        cudaMallocHost((void**)&ctx->h_H, (size_t)ctx->n_bins * 8) != cudaSuccess ||
-        cudaMallocHost((void**)&ctx->h_flag, 4 * sizeof(int)) != cudaSuccess || cudaMalloc((void**)&ctx->d_flag, 4 * sizeof(int)) != cudaSuccess ||
+        cudaMallocHost((void**)&ctx->h_H, (size_t)ctx->n_bins * 8 + 4 * sizeof(int)) != cudaSuccess ||
         cudaEventCreate(&ctx->ev0) != cudaSuccess || cudaEventCreate(&ctx->ev1) != cudaSuccess)
         return bail(MUCA_ECUDA);
+    ctx->h_flag = reinterpret_cast<int*>(ctx->h_H + ctx->n_bins);
     {
         int dev = 0;
         if (cudaGetDevice(&dev) != cudaSuccess ||
@@ -390,10 +424,7 @@ void muca_destroy(muca_ctx* ctx) {
     if (ctx->h_H) cudaFreeHost(ctx->h_H);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
-    if (ctx->d_stage) cudaFree(ctx->d_stage);
-    if (ctx->d_snap) cudaFree(ctx->d_snap);
-    if (ctx->d_flag) cudaFree(ctx->d_flag);
-    if (ctx->h_flag) cudaFreeHost(ctx->h_flag);
+
     if (ctx->own_workspace && ctx->d_workspace) cudaFree(ctx->d_workspace);
     delete ctx;
 }
@@ -401,7 +432,7 @@ void muca_destroy(muca_ctx* ctx) {
 int muca_set_option(muca_ctx* ctx, int option, int value) {
     if (!ctx) return MUCA_EINVAL;
     if (option == MUCA_OPT_KERNEL) {
-        if (value < MUCA_KERNEL_AUTO || value > MUCA_KERNEL_STREAMED_SMEM) return fail(ctx, MUCA_EINVAL, "bad kernel %d", value);
+        if (value < MUCA_KERNEL_AUTO || value > MUCA_KERNEL_STREAMED_PAIRS) return fail(ctx, MUCA_EINVAL, "bad kernel %d", value);
         ctx->opt_kernel = value;
         return MUCA_OK;
     }
@@ -477,7 +508,8 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
     fallback.mode = MODE_STREAMED; fallback.tpb = 32; fallback.nw = fallback.wpw = 0;
     Window win;
     bool guarded = false;   // the window has sentinel rows: the result counts only if no walker entered one
-    if (plan.mode == MODE_WINDOW) {
+    const bool windowed_plan = plan.mode == MODE_WINDOW || plan.mode == MODE_WPAIR;
+    if (windowed_plan) {
         const size_t spin_bytes = (size_t)ctx->W * (ctx->N / 8);
         ctx->h_flag[0] = 0; ctx->h_flag[1] = 0x7FFFFFFF; ctx->h_flag[2] = -1;
         CU(cudaMemcpyAsync(ctx->d_flag, ctx->h_flag, 3 * sizeof(int), cudaMemcpyHostToDevice, ctx->stream));
@@ -486,7 +518,8 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
         CU(cudaMemcpyAsync(ctx->h_flag, ctx->d_flag, 3 * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
         CU(cudaStreamSynchronize(ctx->stream));
         const int lo = ctx->h_flag[1], hi = ctx->h_flag[2];
-        int cap = (int)(((size_t)max_smem - 1024) / (ROW_SMEM_WORDS * 4)) - 2 * WINDOW_PAD_ROWS;
+        const size_t ring = plan.mode == MODE_WPAIR ? wpair_ring_bytes(plan.tpb / 32) : 0;
+        int cap = (int)(((size_t)max_smem - 1024 - ring) / (ROW_SMEM_WORDS * 4)) - 2 * WINDOW_PAD_ROWS;
         if (ctx->opt_window_rows > 0 && ctx->opt_window_rows < cap) cap = ctx->opt_window_rows;
         const int margin = 8;   // rows between the outermost walker and a sentinel at the start of the iteration
         if (cap >= ctx->n_bins) {
@@ -501,11 +534,10 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
             win.sent_lo = j_lo > 0 ? 2 : 0;
             win.sent_hi = j_lo + cap < ctx->n_bins ? 2 : 0;
             guarded = true;
-            if (!ctx->d_snap) CU(cudaMalloc(&ctx->d_snap, align_up(spin_bytes) + (size_t)ctx->W * 4));
             CU(cudaMemcpyAsync(ctx->d_snap, ctx->d_spins, spin_bytes, cudaMemcpyDeviceToDevice, ctx->stream));
             CU(cudaMemcpyAsync((char*)ctx->d_snap + align_up(spin_bytes), ctx->d_E, (size_t)ctx->W * 4, cudaMemcpyDeviceToDevice, ctx->stream));
         }
-        if (plan.mode == MODE_WINDOW) ctx->stat_window_iterations += 1;
+        if (plan.mode != MODE_STREAMED) ctx->stat_window_iterations += 1;
     }
 
     // a2-a4: sweeps.  A block's uint32 bins must not overflow: tpb * measured sweeps * N < 2^32 per launch.
@@ -517,10 +549,10 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
     int launches = 0;
     auto run_sweeps = [&](const Plan& pl) -> int {
         uint64_t max_meas = 0xFFFFFFFFull / ((uint64_t)pl.tpb * (uint64_t)ctx->N);
-        if (pl.mode == MODE_WINDOW) max_meas = 0xFFFFFFFFull / ((uint64_t)pl.tpb * (uint64_t)ctx->N) / 2;   // thermalisation counts too
+        if (pl.mode == MODE_WINDOW || pl.mode == MODE_WPAIR) max_meas = 0xFFFFFFFFull / ((uint64_t)pl.tpb * (uint64_t)ctx->N) / 2;   // thermalisation counts too
         if (max_meas < 1) max_meas = 1;
         const uint64_t max_any = ctx->opt_max_sweeps > 0 ? (uint64_t)ctx->opt_max_sweeps
-                                 : (pl.mode == MODE_WINDOW ? max_meas : total + 1);
+                                 : (pl.mode == MODE_WINDOW || pl.mode == MODE_WPAIR ? max_meas : total + 1);
         uint64_t s = 0;
         while (s < total) {
             uint64_t e = total;
@@ -528,7 +560,8 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
             if (e > meas_begin + max_meas) e = meas_begin + max_meas;
             if (e > s + max_any) e = s + max_any;
             prm.sweep_begin = (uint32_t)s; prm.sweep_end = (uint32_t)e;
-            const int rc = pl.mode == MODE_WINDOW ? launch_window(ctx, prm, pl.tpb, win) : launch_sweep(ctx, prm, pl);
+            const int rc = pl.mode == MODE_WINDOW ? launch_window(ctx, prm, pl.tpb, win)
+                           : pl.mode == MODE_WPAIR ? launch_wpair(ctx, prm, pl.tpb, win) : launch_sweep(ctx, prm, pl);
             if (rc != MUCA_OK) return rc;
             ++launches;
             s = e;
@@ -540,7 +573,7 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
         const int rc = run_sweeps(plan);
         if (rc != MUCA_OK) return rc;
     }
-    if (plan.mode == MODE_WINDOW && guarded) {
+    if ((plan.mode == MODE_WINDOW || plan.mode == MODE_WPAIR) && guarded) {
         CU(cudaMemcpyAsync(ctx->h_flag, ctx->d_flag, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
         CU(cudaStreamSynchronize(ctx->stream));
         if (ctx->h_flag[0]) {   // a walker left the window: repeat the iteration from the snapshot with the L1 kernel
@@ -794,7 +827,6 @@ int muca_unpack_spins_device(muca_ctx* ctx, void* d_out, size_t n) {
 int muca_get_spins(muca_ctx* ctx, int8_t* out, size_t n) {
     if (!ctx) return MUCA_EINVAL;
     if (!out || n != (size_t)ctx->W * ctx->N) return fail(ctx, MUCA_EINVAL, "get_spins: n must be %zu", (size_t)ctx->W * ctx->N);
-    if (!ctx->d_stage) CU(cudaMalloc(&ctx->d_stage, n));
     int rc = muca_unpack_spins_device(ctx, ctx->d_stage, n);
     if (rc == MUCA_OK) {
         cudaError_t e = cudaMemcpyAsync(out, ctx->d_stage, n, cudaMemcpyDeviceToHost, ctx->stream);
@@ -807,7 +839,6 @@ int muca_get_spins(muca_ctx* ctx, int8_t* out, size_t n) {
 int muca_set_spins(muca_ctx* ctx, const int8_t* spins, size_t n) {
     if (!ctx) return MUCA_EINVAL;
     if (!spins || n != (size_t)ctx->W * ctx->N) return fail(ctx, MUCA_EINVAL, "set_spins: n must be %zu", (size_t)ctx->W * ctx->N);
-    if (!ctx->d_stage) CU(cudaMalloc(&ctx->d_stage, n));
     void* d_tmp = ctx->d_stage;
     int rc = MUCA_OK;
     cudaError_t e = cudaMemcpyAsync(d_tmp, spins, n, cudaMemcpyHostToDevice, ctx->stream);

@@ -291,6 +291,33 @@ struct GroupLoop<QN, QN, L, MEAS, RS> {
                                                const uint32_t, const uint32_t, const uint32_t) {}
 };
 
+// Deviates handed over by a paired deviate warp through a double-buffered shared ring (muca_window.cuh,
+// sweep_kernel_wpair): ring[(buf * 8 + call) * slots], one uint4 per call and walker, one barrier per 32-site word.
+struct DeviateFeed {
+    const uint4* ring;   // + this walker's slot
+    int slots, buf, bar_id;
+};
+
+// as GroupLoop, with the deviates of the word in rnd[32] instead of a Philox call per group
+template <int Q, int QN, int L, bool MEAS, uint32_t RS>
+struct GroupLoopExt {
+    static __device__ __forceinline__ void run(uint32_t (&FWk)[4], uint32_t* FWlast3, const uint32_t patch, const bool first_word,
+                                               uint32_t& o, uint32_t& c, uint32_t& rp, uint32_t& tp, const uint32_t (&rndw)[32]) {
+        uint32_t t0;
+        const uint32_t rnd[4] = {rndw[4 * Q], rndw[4 * Q + 1], rndw[4 * Q + 2], rndw[4 * Q + 3]};
+        site_group_smem<Q, MEAS, RS>(FWk[0], FWk[1], FWk[2], FWk[3], o, c, rnd, rp, tp, t0);
+        if (Q == 0 && first_word) {
+            if (rnd[0] <= t0) *FWlast3 += patch;
+        }
+        GroupLoopExt<Q + 1, QN, L, MEAS, RS>::run(FWk, FWlast3, patch, first_word, o, c, rp, tp, rndw);
+    }
+};
+template <int QN, int L, bool MEAS, uint32_t RS>
+struct GroupLoopExt<QN, QN, L, MEAS, RS> {
+    static __device__ __forceinline__ void run(uint32_t (&)[4], uint32_t*, const uint32_t, const bool, uint32_t&, uint32_t&,
+                                               uint32_t&, uint32_t&, const uint32_t (&)[32]) {}
+};
+
 // One typewriter pass over row y of one walker.  up/dn: rows above/below (current values), cur: the row,
 // updated in place.  o: byte offset of the walker's energy row in the table (= j * row stride), updated.
 //
@@ -305,13 +332,13 @@ struct GroupLoop<QN, QN, L, MEAS, RS> {
 //   o   += D ? RS*(2 - a(fw)) : 0    RS*a(fw) comes from an 8-entry byte table in two registers (PRMT)
 //   s_x ^= D                         predicated XOR with an immediate
 //   H[row o] += 1                    shared-memory atomic, measured sweeps only
-template <int L, int MODE, bool MEAS>
+template <int L, int MODE, bool MEAS, bool EXT = false>
 __device__ __forceinline__ void process_row(const uint32_t (&up)[Geo<L>::WPR], uint32_t (&cur)[Geo<L>::WPR],
                                             const uint32_t (&dn)[Geo<L>::WPR], uint32_t& o,
                                             const uint32_t ctr0_row, const uint32_t sweep, const uint32_t iteration,
                                             const uint32_t walker, const uint32_t key0, const uint32_t key1,
                                             const char* __restrict__ tbl_smem, const char* __restrict__ tbl_glob,
-                                            uint32_t* __restrict__ hist) {
+                                            uint32_t* __restrict__ hist, DeviateFeed* feed = nullptr) {
     using G = Geo<L>;
     constexpr int WPR = G::WPR, BITS = G::BITS;
     constexpr uint32_t RS = (tbl_in_smem(MODE) ? ROW_SMEM_WORDS : ROW_L1_WORDS) * 4;  // row stride in bytes
@@ -358,8 +385,21 @@ __device__ __forceinline__ void process_row(const uint32_t (&up)[Geo<L>::WPR], u
 #pragma unroll
         for (int k = 0; k < WPR; ++k) {
             uint32_t c = cur[k];
-            GroupLoop<0, BITS / 4, L, MEAS, RS>::run(FW[k], &FW[WPR - 1][3], patch, k == 0, o, c, rp, tp,
-                                                     ctr0_row + (uint32_t)(k * 8), sweep, iteration, walker, key0, key1);
+            if constexpr (EXT) {
+                static_assert(BITS == 32, "external deviates: one ring hand-over per 32-site word");
+                asm volatile("bar.sync %0, 64;" ::"r"(feed->bar_id) : "memory");   // the deviates of this word are in ring[buf]
+                uint32_t rndw[32];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    const uint4 v = feed->ring[(feed->buf * 8 + q) * feed->slots];
+                    rndw[4 * q] = v.x; rndw[4 * q + 1] = v.y; rndw[4 * q + 2] = v.z; rndw[4 * q + 3] = v.w;
+                }
+                feed->buf ^= 1;
+                GroupLoopExt<0, BITS / 4, L, MEAS, RS>::run(FW[k], &FW[WPR - 1][3], patch, k == 0, o, c, rp, tp, rndw);
+            } else {
+                GroupLoop<0, BITS / 4, L, MEAS, RS>::run(FW[k], &FW[WPR - 1][3], patch, k == 0, o, c, rp, tp,
+                                                         ctr0_row + (uint32_t)(k * 8), sweep, iteration, walker, key0, key1);
+            }
             cur[k] = c;
         }
     } else {
@@ -708,10 +748,11 @@ __device__ __forceinline__ void resident_sweeps(uint32_t* __restrict__ lat, cons
     }
 }
 
-template <int L, int MODE, bool MEAS>
+template <int L, int MODE, bool MEAS, bool EXT = false>
 __device__ __forceinline__ void streamed_sweeps(uint32_t* __restrict__ rows, const size_t row_stride, uint32_t& o,
                                                 const uint32_t s0, const uint32_t s1, const SweepParams& prm,
-                                                const uint32_t walker, const char* tbl_glob, uint32_t* hist) {
+                                                const uint32_t walker, const char* tbl_glob, uint32_t* hist,
+                                                DeviateFeed* feed = nullptr, const bool store = true) {
     using G = Geo<L>;
     constexpr int WPR = G::WPR;
 #pragma unroll 1
@@ -727,9 +768,9 @@ __device__ __forceinline__ void streamed_sweeps(uint32_t* __restrict__ rows, con
 #pragma unroll
                 for (int k = 0; k < WPR; ++k) dn[k] = first[k];                     // row 0, already updated
             }
-            process_row<L, MODE, MEAS>(up, cur, dn, o, (uint32_t)(y * (L / 4)), s, prm.iteration, walker,
-                                                prm.key0, prm.key1, nullptr, tbl_glob, hist);
-            st_row<WPR>(rows + (size_t)y * row_stride, cur);
+            process_row<L, MODE, MEAS, EXT>(up, cur, dn, o, (uint32_t)(y * (L / 4)), s, prm.iteration, walker,
+                                            prm.key0, prm.key1, nullptr, tbl_glob, hist, feed);
+            if (store) st_row<WPR>(rows + (size_t)y * row_stride, cur);   // store == false: a lane without a walker (pair kernel)
 #pragma unroll
             for (int k = 0; k < WPR; ++k) {
                 if (y == 0) first[k] = cur[k];

@@ -162,6 +162,8 @@ def test_full_size_configs_sampled_walkers(name):
     (64, B.MUCA_KERNEL_RESIDENT, 32), (64, B.MUCA_KERNEL_RESIDENT, 224), (64, B.MUCA_KERNEL_STREAMED, 64),
     (128, B.MUCA_KERNEL_RESIDENT, 32), (128, B.MUCA_KERNEL_STREAMED, 64),
     (32, B.MUCA_KERNEL_STREAMED_SMEM, 96), (64, B.MUCA_KERNEL_STREAMED_SMEM, 64), (64, B.MUCA_KERNEL_STREAMED_SMEM, 256),
+    (32, B.MUCA_KERNEL_STREAMED_PAIRS, 96), (64, B.MUCA_KERNEL_STREAMED_PAIRS, 64), (64, B.MUCA_KERNEL_STREAMED_PAIRS, 256),
+    (128, B.MUCA_KERNEL_STREAMED_PAIRS, 32),
 ])
 def test_kernel_variants(L, kernel, tpb):
     W = 2 * tpb + 13
@@ -187,14 +189,15 @@ def test_resident_walkers_per_warp(L, W, tpb, wpw):
 
 # L = 128 default: a WINDOW of the threshold table in shared memory; an iteration in which a walker leaves the window is
 # repeated from a snapshot with the L1 kernel.  Small forced windows exercise that fallback; the chains must not change.
+@pytest.mark.parametrize("kernel", [B.MUCA_KERNEL_STREAMED_SMEM, B.MUCA_KERNEL_STREAMED_PAIRS])
 @pytest.mark.parametrize("L,W,rows,iters,therm,sweeps,expect_fallback", [
     (128, 70, 0, 3, 2, 5, False), (128, 70, 600, 4, 2, 6, None), (64, 150, 300, 6, 3, 12, None),
     (32, 200, 120, 8, 5, 40, True), (32, 100, 40, 3, 2, 10, None),
 ])
-def test_windowed_table_and_fallback(L, W, rows, iters, therm, sweeps, expect_fallback):
+def test_windowed_table_and_fallback(L, W, rows, iters, therm, sweeps, expect_fallback, kernel):
     g, o = mb.Muca(L, W, PRIMARY_SEED, walker_offset=4), mo.Oracle(L, W, PRIMARY_SEED, walker_offset=4)
     try:
-        g.set_option(B.MUCA_OPT_KERNEL, B.MUCA_KERNEL_STREAMED_SMEM)
+        g.set_option(B.MUCA_OPT_KERNEL, kernel)
         if rows:
             g.set_option(B.MUCA_OPT_TABLE_WINDOW_ROWS, rows)
         for it in range(iters):
