@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstring>
 #include <limits>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -328,6 +329,36 @@ int launch_sweep(muca_ctx* ctx, const SweepParams& prm, const Plan& p) {
     return fail(ctx, MUCA_EINVAL, "unsupported L=%d", ctx->L);
 }
 
+// Pinned host buffers are kept in a small process-wide pool instead of being freed with their context: a job that
+// creates a context per step (bench.py) otherwise pays cudaMallocHost / cudaFreeHost -- page locking under a driver
+// lock, 0.1 ms on a quiet host, hundreds of ms on a busy one -- inside its timed region.
+struct PinnedPool {
+    std::mutex m;
+    std::vector<std::pair<size_t, void*>> free_list;
+    void* get(size_t bytes) {
+        {
+            std::lock_guard<std::mutex> g(m);
+            for (size_t i = 0; i < free_list.size(); ++i)
+                if (free_list[i].first == bytes) {
+                    void* p = free_list[i].second;
+                    free_list.erase(free_list.begin() + i);
+                    return p;
+                }
+        }
+        void* p = nullptr;
+        return cudaMallocHost(&p, bytes) == cudaSuccess ? p : nullptr;
+    }
+    void put(size_t bytes, void* p) {
+        if (!p) return;
+        std::lock_guard<std::mutex> g(m);
+        if (free_list.size() < 16) free_list.emplace_back(bytes, p);
+        else cudaFreeHost(p);
+    }
+};
+PinnedPool& pinned_pool() { static PinnedPool* pool = new PinnedPool; return *pool; }   // never destroyed: contexts may outlive static destructors
+size_t pinned_table_bytes(int n_bins) { return (size_t)n_bins * 8 * 4; }
+size_t pinned_hist_bytes(int n_bins) { return (size_t)n_bins * 8 + 4 * sizeof(int); }
+
 int create_common(muca_ctx** out, int L, int W, uint64_t seed, uint32_t walker_offset, void* d_ws, size_t ws_bytes,
                   void* stream, bool own) {
     if (!out) return MUCA_EINVAL;
@@ -356,8 +387,9 @@ int create_common(muca_ctx** out, int L, int W, uint64_t seed, uint32_t walker_o
     ctx->d_snap = L >= 32 ? (void*)(base + c.snap) : nullptr;
     ctx->logw.assign(ctx->n_bins, 0.0);   // R2: omega == 0
     ctx->H.assign(ctx->n_bins, 0);
-    if (cudaMallocHost((void**)&ctx->h_table, (size_t)ctx->n_bins * 8 * 4) != cudaSuccess ||
-        cudaMallocHost((void**)&ctx->h_H, (size_t)ctx->n_bins * 8 + 4 * sizeof(int)) != cudaSuccess ||
+    ctx->h_table = (uint32_t*)pinned_pool().get(pinned_table_bytes(ctx->n_bins));
+    ctx->h_H = (unsigned long long*)pinned_pool().get(pinned_hist_bytes(ctx->n_bins));
+    if (!ctx->h_table || !ctx->h_H ||
         cudaEventCreate(&ctx->ev0) != cudaSuccess || cudaEventCreate(&ctx->ev1) != cudaSuccess)
         return bail(MUCA_ECUDA);
     ctx->h_flag = reinterpret_cast<int*>(ctx->h_H + ctx->n_bins);
@@ -420,8 +452,8 @@ int muca_create_in(muca_ctx** out, int L, int n_walkers, uint64_t seed, uint32_t
 void muca_destroy(muca_ctx* ctx) {
     if (!ctx) return;
     if (ctx->stream || ctx->d_workspace) cudaStreamSynchronize(ctx->stream);
-    if (ctx->h_table) cudaFreeHost(ctx->h_table);
-    if (ctx->h_H) cudaFreeHost(ctx->h_H);
+    pinned_pool().put(pinned_table_bytes(ctx->n_bins), ctx->h_table);
+    pinned_pool().put(pinned_hist_bytes(ctx->n_bins), ctx->h_H);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
 
