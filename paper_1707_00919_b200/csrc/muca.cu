@@ -578,7 +578,7 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
     prm.W = ctx->W; prm.walker_offset = ctx->walker_offset;
     prm.key0 = (uint32_t)(ctx->seed & 0xFFFFFFFFull); prm.key1 = (uint32_t)(ctx->seed >> 32);
     prm.iteration = ctx->iteration; prm.therm = (uint32_t)therm_sweeps;
-    int launches = 0;
+    int launches = windowed_plan ? 1 : 0;   // the slot-range kernel
     auto run_sweeps = [&](const Plan& pl) -> int {
         uint64_t max_meas = 0xFFFFFFFFull / ((uint64_t)pl.tpb * (uint64_t)ctx->N);
         if (pl.mode == MODE_WINDOW || pl.mode == MODE_WPAIR) max_meas = 0xFFFFFFFFull / ((uint64_t)pl.tpb * (uint64_t)ctx->N) / 2;   // thermalisation counts too
