@@ -266,6 +266,58 @@ __device__ __forceinline__ void site_group_smem(const uint32_t fw0, const uint32
     t0 = t_first;
 }
 
+// The same four sites with the decision consumed by SELs instead of predicated instructions (measured recorded
+// sweeps only; used by the paired streamed kernels, where a warp has a scheduler to itself or shares it with one other
+// chain and the length of the chain is what counts):
+//   pD -> SEL (carry 0/1) -> XOR (column) -> IMAD (address) -> ld.shared -> setp -> pD     and     pD -> SEL (state)
+// ISETP -> SEL -> next instruction costs 9 cycles, ISETP -> predicated instruction -> next one about 17
+// (profiles/r01_ubench_chain.txt).  The accept candidate oa passes through a LOP3 with a predicate output (true at run
+// time: oa is a non-zero address): without a second, unconditional consumer ptxas folds "sub/add + selp" into an add
+// predicated on the decision.
+#define MUCA_SITE_SEL(FWOP, ROP, MOP)                                              \
+    "shr.u32 f0, " FWOP ", %16;\n\t"                                             \
+    "and.b32 f0, f0, 7;\n\t"                                                       \
+    "selp.u32 cy, 1, 0, pD;\n\t"                                                   \
+    "xor.b32 f, f0, cy;\n\t"                                                       \
+    "mad.lo.u32 ad, f, 4, %0;\n\t"                                               \
+    "ld.shared.u32 t, [ad];\n\t"                                                   \
+    "prmt.b32 d, %14, %15, f;\n\t"                                     \
+    "sub.u32 oa, %0, d;\n\t"                                                     \
+    "add.u32 oa, oa, %17;\n\t"                                                  \
+    "lop3.and.b32 oa|pq, oa, oa, oa, 0xF0, pt;\n\t"                                \
+    "setp.le.and.u32 pD, " ROP ", t, pq;\n\t"                                      \
+    "selp.u32 %0, oa, %0, pD;\n\t"                                             \
+    "@pD xor.b32 %1, %1, " MOP ";\n\t"                                             \
+    "red.shared.add.u32 [%0+32], 1;\n\t"
+
+template <int Q, uint32_t RS>
+__device__ __forceinline__ void site_group_smem_sel(const uint32_t fw0, const uint32_t fw1, const uint32_t fw2,
+                                                    const uint32_t fw3, uint32_t& o, uint32_t& c,
+                                                    const uint32_t (&rnd)[4], uint32_t& rp, uint32_t& tp, uint32_t& t0) {
+    constexpr uint32_t LUT_LO = (RS * 0) | (RS * 1) << 8 | (RS * 1) << 16 | (RS * 2) << 24;
+    constexpr uint32_t LUT_HI = (RS * 2) | (RS * 3) << 8 | (RS * 3) << 16 | (RS * 4) << 24;
+    uint32_t t_first, t_last;
+    asm volatile(
+        "{\n\t.reg .pred pD, pq, pt;\n\t.reg .b32 f0, cy, f, ad, d, oa, t;\n\t"
+        "setp.eq.u32 pt, 0, 0;\n\t"
+        "setp.le.u32 pD, %12, %13;\n\t"
+        MUCA_SITE_SEL("%4", "%8", "%18")
+        "mov.u32 %2, t;\n\t"
+        MUCA_SITE_SEL("%5", "%9", "%19")
+        MUCA_SITE_SEL("%6", "%10", "%20")
+        MUCA_SITE_SEL("%7", "%11", "%21")
+        "mov.u32 %3, t;\n\t}"
+        : "+r"(o), "+r"(c), "=r"(t_first), "=r"(t_last)
+        : "r"(fw0), "r"(fw1), "r"(fw2), "r"(fw3), "r"(rnd[0]), "r"(rnd[1]),
+          "r"(rnd[2]), "r"(rnd[3]), "r"(rp), "r"(tp), "r"(LUT_LO), "r"(LUT_HI),
+          "n"(4 * Q), "n"(2 * RS), "n"(1u << (4 * Q)), "n"(1u << (4 * Q + 1)),
+          "n"(1u << (4 * Q + 2)), "n"(1u << (4 * Q + 3))
+        : "memory");
+    rp = rnd[3];
+    tp = t_last;
+    t0 = t_first;
+}
+
 template <int Q, int QN, int L, bool MEAS, uint32_t RS>
 struct GroupLoop {
     // groups Q .. QN-1 of word k of a row (compile-time recursion: the shifts and flip masks are immediates)
@@ -305,7 +357,10 @@ struct GroupLoopExt {
                                                uint32_t& o, uint32_t& c, uint32_t& rp, uint32_t& tp, const uint32_t (&rndw)[32]) {
         uint32_t t0;
         const uint32_t rnd[4] = {rndw[4 * Q], rndw[4 * Q + 1], rndw[4 * Q + 2], rndw[4 * Q + 3]};
-        site_group_smem<Q, MEAS, RS>(FWk[0], FWk[1], FWk[2], FWk[3], o, c, rnd, rp, tp, t0);
+        // SEL form where the chain length counts (L = 128: every warp has a scheduler to itself, c_flip 55.9 -> 53.2);
+        // at L = 64 (7 pairs per SM, ALU pipe 59 % busy) the predicate-carried form is 2 % faster
+        if constexpr (MEAS && L >= 128) site_group_smem_sel<Q, RS>(FWk[0], FWk[1], FWk[2], FWk[3], o, c, rnd, rp, tp, t0);
+        else site_group_smem<Q, MEAS, RS>(FWk[0], FWk[1], FWk[2], FWk[3], o, c, rnd, rp, tp, t0);
         if (Q == 0 && first_word) {
             if (rnd[0] <= t0) *FWlast3 += patch;
         }
