@@ -311,3 +311,42 @@ def test_error_paths():
     with pytest.raises(mb.MucaError):
         g.run_iteration(1, 1)
     g.close()
+
+
+def test_randomized_configurations():
+    # seeded random mix of lattice sizes, walker counts (ragged warps), global offsets, kernel variants, launch splits,
+    # table windows, walkers per warp, both update schemes and optional weight updates: every combination must give the
+    # oracle's chains bit for bit (3000 cases of this generator were run once during development)
+    import random
+    rng = random.Random(20260411)
+    for trial in range(80):
+        L = rng.choice([8, 16, 32, 32, 64, 128])
+        W = rng.choice([1, 3, 31, 32, 33, 64, 97, 130, 257])
+        if L == 128:
+            W = min(W, 97)
+        seed, off = rng.getrandbits(64), rng.choice([0, 0, 5, 1000, 2 ** 31])
+        kernel = rng.choice({8: [0, 1, 4], 16: [0, 1, 3, 4], 32: [0, 1, 2, 3, 4, 5, 6], 64: [0, 1, 2, 5, 6], 128: [0, 1, 2, 5, 6]}[L])
+        g, o = mb.Muca(L, W, seed, walker_offset=off), mo.Oracle(L, W, seed, walker_offset=off)
+        tag = [trial, L, W, kernel]
+        try:
+            g.set_option(B.MUCA_OPT_KERNEL, kernel)
+            if rng.random() < 0.3:
+                g.set_option(B.MUCA_OPT_MAX_SWEEPS_PER_LAUNCH, rng.choice([1, 2, 3])); tag.append("split")
+            if L >= 32 and kernel in (0, 5, 6) and rng.random() < 0.5:
+                rows = rng.choice([40, 60, 100, 300, 1000]); g.set_option(B.MUCA_OPT_TABLE_WINDOW_ROWS, rows); tag.append(("window", rows))
+            if L <= 32 and kernel in (0, 1) and rng.random() < 0.5:
+                wpw = rng.choice([1, 7, 16, 28, 32]); g.set_option(B.MUCA_OPT_WALKERS_PER_WARP, wpw); tag.append(("wpw", wpw))
+            for it in range(rng.choice([1, 2, 4])):
+                if rng.random() < 0.2:
+                    u0, u1 = rng.choice([0, 17, 100]), rng.choice([0, 1, 999, 4001])
+                    Hg, Ho = g.run_iteration_random_site(u0, u1), o.run_iteration_random_site(u0, u1, n_threads=mo.max_threads())
+                else:
+                    th, sw = rng.choice([0, 1, 3]), rng.choice([0, 1, 2, 5, 9] if L < 128 else [0, 1, 2])
+                    Hg, Ho = g.run_iteration(th, sw), o.run_iteration(th, sw, n_threads=mo.max_threads())
+                assert np.array_equal(Hg, Ho), (tag, it)
+                if rng.random() < 0.7:
+                    g.update_weights(); o.update_weights()
+            compare_state(g, o, str(tag))
+            assert np.max(np.abs(g.get_log_weights() - o.get_log_weights())) <= LOGW_TOL
+        finally:
+            g.close(); o.close()
