@@ -155,7 +155,8 @@ def test_full_size_configs_sampled_walkers(name):
 # every kernel variant / block size must give the same chains
 @pytest.mark.parametrize("L,kernel,tpb", [
     (8, B.MUCA_KERNEL_RESIDENT, 64), (16, B.MUCA_KERNEL_RESIDENT, 128),
-    (32, B.MUCA_KERNEL_RESIDENT, 64), (32, B.MUCA_KERNEL_RESIDENT, 128), (32, B.MUCA_KERNEL_STREAMED, 32),
+    (32, B.MUCA_KERNEL_RESIDENT, 64), (32, B.MUCA_KERNEL_RESIDENT, 128), (32, B.MUCA_KERNEL_RESIDENT, 96),
+    (16, B.MUCA_KERNEL_RESIDENT, 32), (32, B.MUCA_KERNEL_STREAMED, 32),
     (32, B.MUCA_KERNEL_STREAMED, 96),
     (8, B.MUCA_KERNEL_RESIDENT_V3, 32), (16, B.MUCA_KERNEL_RESIDENT_V3, 64), (32, B.MUCA_KERNEL_RESIDENT_V3, 128),
     (16, B.MUCA_KERNEL_RESIDENT_V2, 32), (32, B.MUCA_KERNEL_RESIDENT_V2, 64),
