@@ -29,7 +29,8 @@ def compare_state(g, o, tag=""):
     if not np.array_equal(sg, so):
         bad = np.nonzero((sg != so).reshape(sg.shape[0], -1).any(axis=1))[0]
         raise AssertionError(f"{tag}: spins differ for walkers {bad[:8]} ({bad.size} of {sg.shape[0]})")
-    assert np.array_equal(energy_numpy(sg), Eg), f"{tag}: tracked E != recomputed E"
+    for a in range(0, sg.shape[0], 4096):                      # chunked: 128 MiB of spins at configs 4 and 5
+        assert np.array_equal(energy_numpy(sg[a:a + 4096]), Eg[a:a + 4096]), f"{tag}: tracked E != recomputed E"
 
 
 def run_pair(L, W, seed, iterations, therm, sweeps, offset=0, options=(), threads=None, check_every=True):
@@ -100,10 +101,11 @@ def test_config1_L8_full(seed):
     run_pair(c.L, c.n_walkers, seed, c.iterations, c.therm_sweeps, c.sweeps)
 
 
-# config 2 in full (2.8e9 attempts on the oracle: tens of seconds on a few cores)
-def test_config2_L16_full():
+# config 2 in full, all three seeds (2.8e9 attempts on the oracle per seed: seconds on 16 threads)
+@pytest.mark.parametrize("seed", (PRIMARY_SEED,) + EXTRA_SEEDS)
+def test_config2_L16_full(seed):
     c = CONFIGS[1]
-    run_pair(c.L, c.n_walkers, c.seed, c.iterations, c.therm_sweeps, c.sweeps, check_every=False)
+    run_pair(c.L, c.n_walkers, seed, c.iterations, c.therm_sweeps, c.sweeps, check_every=False)
 
 
 # configs 3-5 at reduced walker count / sweeps, several tiles and a ragged tail, default launch configuration
@@ -113,7 +115,7 @@ def test_config2_L16_full():
     (128, 32 * 2 + 9, 3, 2, 5),
 ])
 def test_configs345_reduced(L, W, iters, therm, sweeps):
-    for seed in (PRIMARY_SEED, EXTRA_SEEDS[1]):
+    for seed in (PRIMARY_SEED,) + EXTRA_SEEDS:
         run_pair(L, W, seed, iters, therm, sweeps, offset=11)
 
 
@@ -150,6 +152,45 @@ def test_full_size_configs_sampled_walkers(name):
         g.close()
         for o in oracles:
             o.close()
+
+
+# configs 3-5 at FULL size, ALL walkers, in the launch configuration bench.py times: H is a sum over all walkers
+# (Fig. 1), so a merge error that keeps sum(H) -- a bin dropped in one block and counted twice in another,
+# a lane without a walker leaking into a real bin -- shows only when the whole histogram is compared.  The oracle needs
+# 10-35 s per full-size iteration, so it replays the first, a middle and the last iteration of the config from the
+# library's own state before that iteration (spins, omega, iteration counter) and must reproduce the full H, every
+# energy and every spin.  Chained with test_full_size_configs_sampled_walkers (sampled walkers followed through every
+# iteration from the initial state) this covers the whole run.
+@pytest.mark.parametrize("name", ["L32_w16384", "L64_w32768", "L128_w8192"])
+def test_full_size_configs_all_walkers_replayed(name):
+    c = next(x for x in CONFIGS if x.name == name)
+    W, N = c.n_walkers, c.N
+    replay = sorted({0, c.iterations // 2, c.iterations - 1})
+    g = mb.Muca(c.L, W, c.seed)
+    o = mo.Oracle(c.L, W, c.seed)
+    try:
+        compare_state(g, o, f"{name}: init")
+        for it in range(c.iterations):
+            if it in replay:
+                logw = g.get_log_weights()
+                o.set_spins(g.get_spins())
+                o.set_log_weights(logw)
+                o.iteration = g.iteration
+                assert np.array_equal(o.get_energies(), g.get_energies()), f"{name} it{it}: energies before the replay"
+                assert np.array_equal(g.get_thresholds(), mo.thresholds(logw)), f"{name} it{it}: thresholds"
+            Hg = g.run_iteration(c.therm_sweeps, c.sweeps)
+            assert int(Hg.sum()) == W * c.sweeps * N and Hg[1] == 0 and Hg[N - 1] == 0
+            if it in replay:
+                Ho = o.run_iteration(c.therm_sweeps, c.sweeps, n_threads=mo.max_threads())
+                assert np.array_equal(Hg, Ho), f"{name} it{it}: H differs in slots {np.nonzero(Hg != Ho)[0][:8]}"
+                compare_state(g, o, f"{name} it{it}")
+                o.update_weights()
+            g.update_weights()
+            if it in replay:
+                assert np.max(np.abs(g.get_log_weights() - o.get_log_weights())) <= LOGW_TOL
+    finally:
+        g.close()
+        o.close()
 
 
 # every kernel variant / block size must give the same chains
