@@ -76,6 +76,8 @@ enum {
                                      schedule rounded up to whole sweeps, R18) or MUCA_SCHEME_RANDOM_SITE (the paper's
                                      own scheme and units: N_therm = 30 w and N_updates attempted flips per walker;
                                      muca_production then runs therm_sweeps * N and sweeps * N updates per call) */
+    MUCA_OPT_ROLE_MAP = 7,        /* resident kernel with 4 warp pairs per block: 0 = walker warps share schedulers with
+                                     walker warps, 1 = every scheduler runs one walker and one deviate warp (A/B knob) */
     MUCA_OPT_TABLE_WINDOW_ROWS = 6 /* STREAMED_SMEM kernel: rows of the threshold-table window held in shared memory;
                                      0 = as many as fit.  A value below L*L+1 forces the windowed kernel (testing) */
 };

@@ -18,6 +18,7 @@ MUCA_KERNEL_STREAMED_PAIRS = 6
 MUCA_OPT_KERNEL, MUCA_OPT_THREADS_PER_BLOCK, MUCA_OPT_MAX_SWEEPS_PER_LAUNCH, MUCA_OPT_WALKERS_PER_WARP = 1, 2, 3, 4
 MUCA_OPT_UPDATE_SCHEME = 5
 MUCA_OPT_TABLE_WINDOW_ROWS = 6
+MUCA_OPT_ROLE_MAP = 7
 MUCA_SCHEME_TYPEWRITER, MUCA_SCHEME_RANDOM_SITE = 0, 1
 
 # every symbol include/muca.h declares (tests/test_abi.py checks the header against this list and the .so)

@@ -46,6 +46,7 @@ struct muca_ctx {
     int opt_tpb = 0;
     int opt_max_sweeps = 0;
     int opt_wpw = 0;
+    int opt_role_map = 0;           // MUCA_OPT_ROLE_MAP (resident kernel, 4 pairs per block)
     int opt_window_rows = 0;        // MUCA_OPT_TABLE_WINDOW_ROWS: 0 = as many table rows as shared memory holds
     void* d_snap = nullptr;         // snapshot of spins + E for the windowed kernels' fallback (in the workspace, L >= 32)
     int* d_flag = nullptr;          // device int[4]: window-left flag, smallest / largest slot of the walkers
@@ -147,15 +148,15 @@ int launch_sweep_v3(muca_ctx* ctx, const SweepParams& prm, int tpb) {
 }
 
 template <int L>
-int launch_sweep_v5(muca_ctx* ctx, const SweepParams& prm, int nw, int wpw) {
+int launch_sweep_v6(muca_ctx* ctx, const SweepParams& prm, int nw, int wpw) {
     static bool configured = false;
     if (!configured) {
-        CU(cudaFuncSetAttribute(sweep_kernel_v5<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V5<L>::SMEM_BYTES));
+        CU(cudaFuncSetAttribute(sweep_kernel_v6<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V6<L>::SMEM_BYTES));
         configured = true;
     }
     const int per_block = nw * wpw;
     const int grid = (prm.W + per_block - 1) / per_block;
-    sweep_kernel_v5<L><<<grid, 64 * nw, V5<L>::SMEM_BYTES, ctx->stream>>>(prm, wpw);
+    sweep_kernel_v6<L><<<grid, 64 * nw, V6<L>::SMEM_BYTES, ctx->stream>>>(prm, wpw, ctx->opt_role_map);
     CU(cudaGetLastError());
     return MUCA_OK;
 }
@@ -227,7 +228,7 @@ Plan make_plan(const muca_ctx* c) {
 
 size_t plan_smem(int L, const Plan& p) {
     if (p.mode == MODE_WINDOW || p.mode == MODE_WPAIR) return 0;   // sized at run time from what the device allows
-    if (p.mode == MODE_V5) return L == 8 ? V5<8>::SMEM_BYTES : L == 16 ? V5<16>::SMEM_BYTES : V5<32>::SMEM_BYTES;
+    if (p.mode == MODE_V5) return L == 8 ? V6<8>::SMEM_BYTES : L == 16 ? V6<16>::SMEM_BYTES : V6<32>::SMEM_BYTES;
     if (p.mode == MODE_V3) return L == 8 ? V3<8>::SMEM_BYTES : L == 16 ? V3<16>::SMEM_BYTES : V3<32>::SMEM_BYTES;
     switch (L) {
         case 8: return sweep_smem_bytes<8, MODE_TBL_SMEM>(p.tpb);
@@ -297,9 +298,9 @@ int launch_window(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& 
 int launch_sweep(muca_ctx* ctx, const SweepParams& prm, const Plan& p) {
     if (p.mode == MODE_V5) {
         switch (ctx->L) {
-            case 8: return launch_sweep_v5<8>(ctx, prm, p.nw, p.wpw);
-            case 16: return launch_sweep_v5<16>(ctx, prm, p.nw, p.wpw);
-            case 32: return launch_sweep_v5<32>(ctx, prm, p.nw, p.wpw);
+            case 8: return launch_sweep_v6<8>(ctx, prm, p.nw, p.wpw);
+            case 16: return launch_sweep_v6<16>(ctx, prm, p.nw, p.wpw);
+            case 32: return launch_sweep_v6<32>(ctx, prm, p.nw, p.wpw);
         }
     }
     if (p.mode == MODE_V3) {
@@ -486,6 +487,11 @@ int muca_set_option(muca_ctx* ctx, int option, int value) {
     if (option == MUCA_OPT_UPDATE_SCHEME) {
         if (value != MUCA_SCHEME_TYPEWRITER && value != MUCA_SCHEME_RANDOM_SITE) return fail(ctx, MUCA_EINVAL, "bad update scheme %d", value);
         ctx->opt_scheme = value;
+        return MUCA_OK;
+    }
+    if (option == MUCA_OPT_ROLE_MAP) {
+        if (value < 0 || value > 1) return fail(ctx, MUCA_EINVAL, "role map must be 0 or 1");
+        ctx->opt_role_map = value;
         return MUCA_OK;
     }
     if (option == MUCA_OPT_MAX_SWEEPS_PER_LAUNCH) {

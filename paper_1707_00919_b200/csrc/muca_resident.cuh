@@ -1,196 +1,309 @@
 // paper_1707_00919_b200/csrc/muca_resident.cuh
-// Resident sweep kernel v5 for L <= 32 (sm_100a): "state in the address", walker warps paired with deviate warps.
+// Resident sweep kernel v6 for L <= 32 (sm_100a): "state in the address", two-candidate select, walker warps paired
+// with deviate warps, everything that is not the per-site chain spread over the sites of the previous row.
 // Citations: "PAPER.md:<line>" = /root/reference/PAPER.md, "R<n>" = DESIGN.md section 3.
 //
-// The walker's dynamic state -- energy slot j AND the carry c = [previous site of this row flipped] -- is ONE
-// shared-memory address S = rowaddr(j, c).  The table is stored twice: copy c at byte offset c*K (K a power of
-// two above copy 0, the lattices and the deviate ring); copy 1 has its columns permuted (f -> f ^ 1: a flipped
-// left neighbour toggles the [left != s] bit of the column index).  Row (j, c) is 68 bytes (17 words: consecutive
-// rows rotate through all 32 banks):
+// The walker's dynamic state is the shared-memory address S = rowaddr(j) of its energy slot j; the carry
+// c = [previous site of this row flipped] lives in the ENTRY address A of the next lookup.  The table is stored twice:
+// copy c at byte offset c*K (K a power of two above copy 0, the lattices and the deviate ring); copy 1 has its columns
+// permuted (f -> f ^ 1: a flipped left neighbour toggles the [left != s] bit of the column index).  Row (j, c) is 68
+// bytes (17 words: consecutive rows rotate through all 32 banks):
 //     +4f      t  = thresh[j][a],  a = a(f ^ c)          (PAPER.md:109 acceptance, R6/R7)
-//     +32+4f   Sa = rowaddr(j + 2 - a, 1)                 (state an ACCEPTED move leads to; a rejected one leads
-//                                                          to rowaddr(j, 0) = S & ~K)
-//     +64      histogram bin of slot j (copy 0 only: both copies of a slot count into it)
-// Two 32-bit loads instead of one 64-bit load: a random-row LDS.64 takes 34 cycles (two 16-lane phases, each with
-// its own bank conflicts), a random-row LDS.32 27 (profiles/r01_ubench_chain.txt); Sa arrives 3 cycles behind t.
-// Per site the serial chain is   LDS t -> ISETP -> SEL(Sa, S & ~K) -> IADD (+ column of the next site) -> LDS t'.
-// Column extraction, flip mask and histogram increment are off the chain.  Philox runs in a paired "deviate" warp
-// (same walkers) that feeds a double-buffered shared ring one row ahead: the hardware interleaves its instruction
-// stream into the stalls of the walker warps (at 4 pairs per SM, walker warps share schedulers with walker warps and
-// deviate warps with deviate warps).  What was measured and dropped: a single in-order
-// warp doing both (75 cycles per site), selecting between two precomputed entry addresses (ptxas folds the add
-// into an instruction predicated on the decision, +11 cycles), and speculative loads for both outcomes of the
-// next site (the walker warp becomes issue-bound at the same 49 cycles).
+//     +32+4f   Sa = rowaddr(j + 2 - a)                    (state an ACCEPTED move leads to; a rejected one keeps S)
+//     +64      histogram bin of slot j (copy 0 only)
+// Per site the serial chain is   LDS t -> ISETP -> SEL(A_acc, A_rej) -> LDS t'   with BOTH candidates of the next
+// entry address, A_acc = Sa + K + 4f' and A_rej = S + 4f', formed before the decision (round 1, v5, selected the
+// state and added the column afterwards: ISETP -> SEL -> IADD -> LDS).  Philox runs in a paired "deviate" warp (same
+// walkers) that feeds a double-buffered shared ring one row ahead.
+//
+// What the ncu source view of v5 showed (profiles/README.md, round 2): a steady-state site cost 46 cycles, but the
+// row prologue -- eight 16-byte ring loads in one burst (32 wavefronts queued in front of the first table loads) and
+// ~70 instructions of bit-sliced preparation -- added another 340 cycles per row, 10.7 per site.  Here the deviates
+// of row y + 1 replace those of row y in place, one 16-byte load per four sites, and the field words of row y + 1 are
+// prepared a step per site in the shadow of the table loads; the part that depends on the row above is finished as
+// soon as the last site of its residue class (x & 3) has been decided.
 #pragma once
 #include "muca_device.cuh"
 
 namespace muca {
 
+#ifndef MUCA_SITE_VARIANT
+#define MUCA_SITE_VARIANT 7
+#endif
+#if MUCA_SITE_VARIANT == 7
+#define MUCA_V6_DT 1   // the state an accepted move leads to is computed from a 16-word delta table instead of loaded from the row
+#endif
 
 template <int L>
-struct V5 {
+struct V6 {
+    static constexpr uint32_t SBASE = 1024;                  // dynamic shared memory starts behind the 1 KB the system reserves on sm_100 (checked)
     static constexpr uint32_t BINS = L * L + 1;
+#ifdef MUCA_V6_DT
+    // row (j, c): t[8] | bin (copy 0 only) = 9 words (odd: consecutive rows rotate through all 32 banks);
+    // behind the rows of copy c: DT[c][f] = RS * (2 - a(f ^ c)), the state change of an accepted move
+    static constexpr uint32_t RS = 36, BIN_OFF = 32;
+    static constexpr uint32_t DT_OFF = (BINS + 1) * RS;      // + one all-reject row: parking place of unused lanes
+    static constexpr uint32_t COPY_BYTES = DT_OFF + 32;
+    // K = offset of copy 1; K % 128 == 32 puts DT[1][f] into other banks than DT[0][f]: a warp's delta load is one wavefront
+    static constexpr uint32_t K = (COPY_BYTES + 127u) / 128u * 128u + 32u;
+    static constexpr uint32_t LAT_OFF = (K + COPY_BYTES + 15u) & ~15u;
+#else
     static constexpr uint32_t RS = 68;
     static constexpr uint32_t SA_OFF = 32, BIN_OFF = 64;
     static constexpr uint32_t TBL_BYTES = (BINS + 1) * RS;   // + one all-reject row: parking place of unused lanes
     static constexpr int KBIT = L == 32 ? 17 : (L == 16 ? 16 : 15);
     static constexpr uint32_t K = 1u << KBIT;
     static constexpr uint32_t LAT_OFF = (TBL_BYTES + 15u) & ~15u;
+#endif
     static constexpr int MAX_WARPS = 4;                      // walker warps per block (+ as many deviate warps)
     static constexpr int SLOTS = 32 * MAX_WARPS;             // lattice / ring columns
     static constexpr int NC = Geo<L>::BITS / 4;              // Philox calls per row
     static constexpr uint32_t RING_OFF = LAT_OFF + (uint32_t)L * 4u * SLOTS;
     static constexpr uint32_t RING_BYTES = 2u * NC * 16u * SLOTS;
+#ifdef MUCA_V6_DT
+    static constexpr size_t SMEM_BYTES = (size_t)RING_OFF + RING_BYTES;
+#else
     static_assert(1024u + RING_OFF + RING_BYTES <= K, "copy 0 + lattices + ring must end below K");
     static constexpr size_t SMEM_BYTES = (size_t)K + TBL_BYTES;
+#endif
 };
 
-// Static planes of a row, split so that the part that does not depend on the row ABOVE (which the walker has only
-// just finished) can be prepared one row ahead, in the shadow of the current row's table loads:
-//   partial_words: nibble q of P[r] = hl + 2*(vd + hr) of site 4q + r   (hl/hr: left/right bond, vd: bond to the row below)
-//   finish_words : FW[r] = P[r] + 2*vu   (vu: bond to the row above)  =  column f = hl + 2*n3 of field_words()
+// Field words of a row: nibble q of FW[r] holds the column f = hl + 2*n3 of site 4q + r (hl: bond to the left
+// neighbour's OLD value, n3 = antiparallel bonds to up / down / right).  They are built in two parts so that most of
+// the work can be done a row ahead: the planes that do not depend on the row ABOVE (which the walker is still
+// updating) go into P[r] = hl + 2*(vd + hr), one small step per site of the row before (prep_step), and
+// FW[r] = P[r] + 2*vu is finished when the sites 4q + r of the row above are final (finish_word).
 template <int L>
-__device__ __forceinline__ void partial_words(const uint32_t c, const uint32_t dn, uint32_t (&P)[4], uint32_t& patch) {
+struct NextRow {
+    uint32_t c, dn;            // the row (old value) and the row below it (old; row 0, already final, below row L-1)
+    uint32_t hl, hr, m0, m1;   // bond planes: left, right, (down + right) as sum and carry bits
+    uint32_t t;
+    uint32_t P[4];
+    uint32_t patch;            // added to FW[3] when site 0 flips: n3 of the LAST site of the row changes by +-1
+};
+
+constexpr int PREP_STEPS = 17;
+
+template <int L, int I>
+__device__ __forceinline__ void prep_step(NextRow<L>& n) {
     using G = Geo<L>;
     constexpr int BITS = G::BITS;
-    uint32_t rw, lw;
-    if constexpr (L >= 32) {
-        rw = (c >> 1) | (c << 31);
-        lw = (c << 1) | (c >> 31);
+    if constexpr (I == 0) {
+        const uint32_t rw = L >= 32 ? __funnelshift_r(n.c, n.c, 1) : ((n.c >> 1) | ((n.c & 1u) << (BITS - 1)));
+        n.hr = n.c ^ rw;
+    } else if constexpr (I == 1) {
+        const uint32_t lw = L >= 32 ? __funnelshift_l(n.c, n.c, 1) : (((n.c << 1) | (n.c >> (BITS - 1))) & G::MASK);
+        n.hl = n.c ^ lw;
+    } else if constexpr (I == 2) {
+        n.m0 = n.c ^ n.dn ^ n.hr;
+    } else if constexpr (I == 3) {
+        n.m1 = (n.c ^ n.dn) & n.hr;
+    } else if constexpr (I < 16) {
+        constexpr int r = (I - 4) / 3, part = (I - 4) % 3;
+        if constexpr (part == 0) n.t = (n.hl >> r) & 0x11111111u;
+        else if constexpr (part == 1) n.t |= (r >= 1 ? n.m0 >> (r >= 1 ? r - 1 : 0) : n.m0 << 1) & 0x22222222u;
+        else n.P[r] = n.t | ((r >= 2 ? n.m1 >> (r >= 2 ? r - 2 : 0) : n.m1 << (2 - r)) & 0x44444444u);
     } else {
-        rw = (c >> 1) | ((c & 1u) << (BITS - 1));
-        lw = ((c << 1) | (c >> (BITS - 1))) & G::MASK;
+        constexpr int QL = BITS / 4 - 1;
+        const uint32_t hr_last = (n.hr >> (BITS - 1)) & 1u;
+        n.patch = (1u << (4 * QL + 1)) - (hr_last << (4 * QL + 2));
     }
-    const uint32_t vd = c ^ dn, hr = c ^ rw, hl = c ^ lw;
-    const uint32_t m0 = vd ^ hr, m1 = vd & hr;
-#pragma unroll
-    for (int r = 0; r < 4; ++r) {
-        const uint32_t A = hl >> r;
-        const uint32_t B = r >= 1 ? m0 >> (r - 1) : m0 << 1;
-        const uint32_t C = r >= 2 ? m1 >> (r - 2) : m1 << (2 - r);
-        const uint32_t t1 = (A & 0x11111111u) | (B & 0x22222222u);
-        P[r] = t1 | (C & 0x44444444u);
-    }
-    constexpr int QL = BITS / 4 - 1;
-    const uint32_t hr_last = (hr >> (BITS - 1)) & 1u;
-    patch = (1u << (4 * QL + 1)) - (hr_last << (4 * QL + 2));   // site 0 flipped: n3 of the LAST site +-1
 }
+template <int L, int I0, int I1>
+__device__ __forceinline__ void prep_steps(NextRow<L>& n) {
+    if constexpr (I0 < I1) {
+        prep_step<L, I0>(n);
+        prep_steps<L, I0 + 1, I1>(n);
+    }
+}
+// the steps that follow site x of the row above: sites 0 .. BITS-5 share the PREP_STEPS steps evenly, the last four
+// sites are left to finish_word
 template <int L>
-__device__ __forceinline__ void finish_words(const uint32_t (&P)[4], const uint32_t vu, uint32_t (&FW)[4]) {
+__device__ __forceinline__ void prep_for_site(NextRow<L>& n, const int x) {
+    constexpr int D = Geo<L>::BITS - 4;
+    switch (x) {
+#define MUCA_PREP_CASE(X) case X: if constexpr (X < D) prep_steps<L, (X * PREP_STEPS) / D, ((X + 1) * PREP_STEPS) / D>(n); break;
+        MUCA_PREP_CASE(0) MUCA_PREP_CASE(1) MUCA_PREP_CASE(2) MUCA_PREP_CASE(3) MUCA_PREP_CASE(4) MUCA_PREP_CASE(5) MUCA_PREP_CASE(6)
+        MUCA_PREP_CASE(7) MUCA_PREP_CASE(8) MUCA_PREP_CASE(9) MUCA_PREP_CASE(10) MUCA_PREP_CASE(11) MUCA_PREP_CASE(12)
+        MUCA_PREP_CASE(13) MUCA_PREP_CASE(14) MUCA_PREP_CASE(15) MUCA_PREP_CASE(16) MUCA_PREP_CASE(17) MUCA_PREP_CASE(18)
+        MUCA_PREP_CASE(19) MUCA_PREP_CASE(20) MUCA_PREP_CASE(21) MUCA_PREP_CASE(22) MUCA_PREP_CASE(23) MUCA_PREP_CASE(24)
+        MUCA_PREP_CASE(25) MUCA_PREP_CASE(26) MUCA_PREP_CASE(27)
+#undef MUCA_PREP_CASE
+        default: break;
+    }
+}
+// FW[r] of the row below `above_new` (bits 4q + r of above_new must be final)
+template <int L>
+__device__ __forceinline__ uint32_t finish_word(const NextRow<L>& n, const uint32_t above_new, const int r) {
     constexpr uint32_t M = Geo<L>::BITS == 32 ? 0x11111111u : (Geo<L>::BITS == 16 ? 0x1111u : 0x11u);
-#pragma unroll
-    for (int r = 0; r < 4; ++r) FW[r] = P[r] + 2u * ((vu >> r) & M);
+    return n.P[r] + 2u * (((n.c ^ above_new) >> r) & M);
 }
 
-// One site of the walker chain, in PTX.  Three things ptxas does not do by itself:
-//  * the decision must be consumed by a SEL: ISETP -> SEL -> (IADD ->) LDS costs 9 (13) cycles on sm_100a, ISETP ->
-//    predicated instruction -> LDS about 20 (profiles/r01_ubench_chain.txt).  ptxas turns "S = p ? sa : S & ~K" into a
-//    predicated AND unless the AND has a second, unconditional use: here it is the address of the histogram
-//    increment (the bin of copy 0 serves both copies);
-//  * the walker warp is a single in-order instruction stream whose ISETP blocks until the threshold arrives, so
-//    everything that does not depend on the decision should be issued BEFORE the ISETP, in the shadow of the
-//    27-cycle table load.  The predicate chain ps -> pg -> ISETP (LOP3 with a predicate output; both are true at
-//    run time: sr is a non-zero address) pins the ISETP behind the column extraction of the next site;
-//  * H[j]++ of the PREVIOUS attempt is issued behind this site's table loads (S still holds that state).
+// One site of the walker chain, in PTX.
 //   %0 S: state address (in/out)    %1 A: entry address of this site (in), of the next site (out)
 //   %2 flips (in/out)   %3 FW[3] at site 0 (in/out)   %4 deviate   %5 field word of the NEXT site   %6 its shift
-//   %7 flip mask of this site   %8 ~K   %9 patch (site 0)
-// The flip mask is a predicated OR (one ALU instruction; collecting bit K of the new state with SHF + LOP3 instead
-// costs 1.7 cycles per site once two walker warps share a scheduler and its ALU pipe).
-#define MUCA_V5_SITE(SHIFT_OP, EXTRA_LINE)                                       \
-    "{\n\t.reg .pred p, ps, pg;\n\t.reg .b32 t, sa, sr, g0, g;\n\t"               \
-    "ld.shared.u32 t, [%1];\n\t"                                                 \
-    "ld.shared.u32 sa, [%1+32];\n\t"                                             \
-    "setp.eq.u32 ps, 0, 0;\n\t"                                                  \
-    "lop3.and.b32 sr|ps, %0, %8, 0, 0xC0, ps;\n\t"                               \
-    "red.shared.add.u32 [sr+64], 1;\n\t"                                         \
-    SHIFT_OP " g0, %5, %6;\n\t"                                                  \
-    "lop3.or.b32 g|pg, g0, 0x1C, 0, 0xC0, ps;\n\t"                               \
-    "setp.le.and.u32 p, %4, t, pg;\n\t"                                          \
-    "selp.u32 %0, sa, sr, p;\n\t"                                                \
-    "add.u32 %1, %0, g;\n\t"                                                     \
-    "@p or.b32 %2, %2, %7;\n\t" EXTRA_LINE "}"
+//   %7 flip mask of this site   %8 K (0 at the last site of a row: the next row starts without a carry)   %9 patch (site 0)
+// H[j]++ of the PREVIOUS attempt is issued behind this site's table loads (S still holds that state); thermalisation
+// sweeps leave it out.  The flip mask is a predicated OR.
+//   %0 S   %1 A   %2 flips   %3 FW[3] at site 0   %4 checksum   %5 delta-table offset A - S (variant 7)
+//   %6 deviate   %7 field word of the NEXT site   %8 its shift   %9 flip mask   %10 K (0 at the last site of a row)
+//   %11 patch (site 0)   %12 address of DT[0][0] (variant 7)
+#if MUCA_SITE_VARIANT == 3     // Sa loaded from the row (in front of t: volatile loads keep their order)
+#define MUCA_V6_SITE(SHIFT_OP, HIST_LINE, EXTRA_LINE)                            \
+    "{\n\t.reg .pred p;\n\t.reg .b32 t, sa, g0, g, gk, ar, aa;\n\t"              \
+    "ld.volatile.shared.u32 sa, [%1+32];\n\t"                                    \
+    "ld.volatile.shared.u32 t, [%1];\n\t" HIST_LINE                              \
+    SHIFT_OP " g0, %7, %8;\n\t"                                                  \
+    "and.b32 g, g0, 0x1C;\n\t"                                                   \
+    "add.u32 ar, %0, g;\n\t"                                                     \
+    "add.u32 gk, g, %10;\n\t"                                                    \
+    "add.u32 aa, sa, gk;\n\t"                                                    \
+    "mad.lo.u32 %4, aa, ar, %4;\n\t"                                             \
+    "setp.le.u32 p, %6, t;\n\t"                                                  \
+    "selp.u32 %1, aa, ar, p;\n\t"                                                \
+    "selp.u32 %0, sa, %0, p;\n\t"                                                \
+    "@p or.b32 %2, %2, %9;\n\t" EXTRA_LINE "}"
+#elif MUCA_SITE_VARIANT == 7   // Sa = S + DT[A - S]: a conflict-free load behind the table load; the offset A - S is selected like A
+#define MUCA_V6_SITE(SHIFT_OP, HIST_LINE, EXTRA_LINE)                            \
+    "{\n\t.reg .pred p;\n\t.reg .b32 t, d, sa, g0, g, gk, ar, aa, sg;\n\t"       \
+    "ld.volatile.shared.u32 t, [%1];\n\t"                                        \
+    "ld.volatile.shared.u32 d, [%5+%12];\n\t" HIST_LINE                          \
+    SHIFT_OP " g0, %7, %8;\n\t"                                                  \
+    "and.b32 g, g0, 0x1C;\n\t"                                                   \
+    "add.u32 ar, %0, g;\n\t"                                                     \
+    "add.u32 gk, g, %10;\n\t"                                                    \
+    "add.u32 sg, %0, gk;\n\t"                                                    \
+    "add.u32 aa, sg, d;\n\t"                                                     \
+    "add.u32 sa, %0, d;\n\t"                                                     \
+    "mad.lo.u32 %4, aa, ar, %4;\n\t"                                             \
+    "setp.le.u32 p, %6, t;\n\t"                                                  \
+    "selp.u32 %1, aa, ar, p;\n\t"                                                \
+    "selp.u32 %5, gk, g, p;\n\t"                                                 \
+    "selp.u32 %0, sa, %0, p;\n\t"                                                \
+    "@p or.b32 %2, %2, %9;\n\t" EXTRA_LINE "}"
+#endif
+#ifdef MUCA_V6_DT
+#define MUCA_V6_HIST "red.shared.add.u32 [%0+32], 1;\n\t"
+#else
+#define MUCA_V6_HIST "red.shared.add.u32 [%0+64], 1;\n\t"
+#endif
 
-// One row of the walker warp.  In: the row above (`up`, final), this row (`c`, `P`, `patch`, `rnd`: old values, partial
-// planes, deviates).  Out: the same for row y + 1 in (c1, P1, patch1, rnd1), fetched / prepared while this row is
-// processed (none of it depends on this row; only "FW = P + 2*vu" waits for the row above), and `up` = this row's new
-// value.  Every site increments the bin of the state it STARTS from, i.e. of the state after the previous attempt.
-template <int L>
-__device__ __forceinline__ void row_v5(uint32_t* __restrict__ lat, uint32_t& S, const int y, const bool more, uint32_t& up,
-                                       const uint32_t c, const uint32_t (&P)[4], const uint32_t patch,
-                                       const uint32_t (&rnd)[Geo<L>::BITS], uint32_t& c1, uint32_t (&P1)[4], uint32_t& patch1,
-                                       uint32_t (&rnd1)[Geo<L>::BITS], const uint4* __restrict__ ring, int& buf,
-                                       const int bar_id) {
-    using G = Geo<L>;
-    using V = V5<L>;
-    constexpr int BITS = G::BITS, NC = V::NC, SLOTS = V::SLOTS;
-    // the deviates of row y + 1 are in ring[buf]; ring[buf ^ 1] (this row's, already in registers) may be refilled.
-    // After the last row of a phase there is no such barrier (the deviate warp has left its loop) and what is
-    // fetched below is not used.
-    if (more) pair_barrier(bar_id);
-    uint32_t FW[4];
-    finish_words<L>(P, c ^ up, FW);
-    const int y1 = (y + 1) & (L - 1), y2 = (y + 2) & (L - 1);
-    c1 = lat[y1 * SLOTS];
-    partial_words<L>(c1, lat[y2 * SLOTS], P1, patch1);   // row y + 2 is old (or row 0, final in this sweep, when y + 1 = L - 1)
-#pragma unroll
-    for (int k = 0; k < NC; ++k) {
-        const uint4 v = ring[(buf * NC + k) * SLOTS];
-        rnd1[4 * k] = v.x; rnd1[4 * k + 1] = v.y; rnd1[4 * k + 2] = v.z; rnd1[4 * k + 3] = v.w;
+template <int L, bool MEAS, int KK>
+__device__ __forceinline__ void site_v6(uint32_t& S, uint32_t& A, uint32_t& flips, uint32_t& fw3, uint32_t& chk, uint32_t& off, const uint32_t rnd,
+                                        const uint32_t fwn, const int qn, const uint32_t mask, const uint32_t patch,
+                                        const bool first) {
+    const uint32_t sh = qn == 0 ? 2u : (uint32_t)(4 * qn - 2);   // nibble qn of the field word -> bits 2..4
+    uint32_t unused = 0;   // fills operand %3 of the site macro where site 0 has FW[3]
+#ifdef MUCA_V6_DT
+    constexpr uint32_t DTA = V6<L>::SBASE + V6<L>::DT_OFF;
+#else
+    constexpr uint32_t DTA = 0;
+#endif
+    if (first) {   // site 0 also patches the last site's column: its right neighbour is site 0
+        if (MEAS)
+            asm volatile(MUCA_V6_SITE("shl.b32", MUCA_V6_HIST, "@p add.u32 %3, %3, %11;\n\t")
+                         : "+r"(S), "+r"(A), "+r"(flips), "+r"(fw3), "+r"(chk), "+r"(off)
+                         : "r"(rnd), "r"(fwn), "r"(sh), "r"(mask), "n"(KK), "r"(patch), "n"(DTA) : "memory");
+        else
+            asm volatile(MUCA_V6_SITE("shl.b32", "", "@p add.u32 %3, %3, %11;\n\t")
+                         : "+r"(S), "+r"(A), "+r"(flips), "+r"(fw3), "+r"(chk), "+r"(off)
+                         : "r"(rnd), "r"(fwn), "r"(sh), "r"(mask), "n"(KK), "r"(patch), "n"(DTA) : "memory");
+    } else if (qn == 0) {
+        if (MEAS)
+            asm volatile(MUCA_V6_SITE("shl.b32", MUCA_V6_HIST, "")
+                         : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused), "+r"(chk), "+r"(off)
+                         : "r"(rnd), "r"(fwn), "r"(sh), "r"(mask), "n"(KK), "r"(0), "n"(DTA) : "memory");
+        else
+            asm volatile(MUCA_V6_SITE("shl.b32", "", "")
+                         : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused), "+r"(chk), "+r"(off)
+                         : "r"(rnd), "r"(fwn), "r"(sh), "r"(mask), "n"(KK), "r"(0), "n"(DTA) : "memory");
+    } else {
+        if (MEAS)
+            asm volatile(MUCA_V6_SITE("shr.u32", MUCA_V6_HIST, "")
+                         : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused), "+r"(chk), "+r"(off)
+                         : "r"(rnd), "r"(fwn), "r"(sh), "r"(mask), "n"(KK), "r"(0), "n"(DTA) : "memory");
+        else
+            asm volatile(MUCA_V6_SITE("shr.u32", "", "")
+                         : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused), "+r"(chk), "+r"(off)
+                         : "r"(rnd), "r"(fwn), "r"(sh), "r"(mask), "n"(KK), "r"(0), "n"(DTA) : "memory");
     }
-    buf ^= (int)more;
-    S &= ~V::K;                        // site 0: its left neighbour (site L-1) has not been visited in this sweep
-    uint32_t A = S + ((FW[0] << 2) & 0x1Cu);
-    uint32_t flips = 0, unused = 0;    // `unused` fills operand %3 of the site macro where site 0 has FW[3]
+}
+
+// One row of the walker warp.  In: the row above (`up`, final), this row's old value `c`, its finished field words FW,
+// its deviates rnd[] and the entry address A of site 0.  While the row is processed, the row below is prepared in `n`
+// (old value, partial planes), its field words FWn are finished and its deviates replace this row's in rnd[] (call k
+// after site 4k + 3).  Out: `up` = this row's new value, A = entry address of site 0 of the row below.
+// Every site increments the bin of the state it STARTS from, i.e. of the state after the previous attempt.
+template <int L, bool MEAS>
+__device__ __forceinline__ void row_v6(uint32_t* __restrict__ lat, uint32_t& S, uint32_t& A, uint32_t& chk, uint32_t& off, const int y, const bool more,
+                                       uint32_t& up, const uint32_t c, uint32_t (&FW)[4], const uint32_t patch,
+                                       uint32_t (&rnd)[Geo<L>::BITS], NextRow<L>& n, uint32_t (&FWn)[4],
+                                       const uint4* __restrict__ ring, int& buf, const int bar_id) {
+    using G = Geo<L>;
+    using V = V6<L>;
+    constexpr int BITS = G::BITS, NC = V::NC, SLOTS = V::SLOTS;
+    // the deviates of row y + 1 are in ring[buf]; ring[buf ^ 1] (this row's, all fetched) may be refilled.  After the
+    // last row of a phase there is no such barrier (the deviate warp has left its loop) and what is fetched is not used.
+    if (more) pair_barrier(bar_id);
+    const int y1 = (y + 1) & (L - 1), y2 = (y + 2) & (L - 1);
+    n.c = lat[y1 * SLOTS];
+    n.dn = lat[y2 * SLOTS];   // row y + 2 is old (or row 0, final in this sweep, when y + 1 = L - 1)
+    uint32_t flips = 0;
 #pragma unroll
     for (int x = 0; x < BITS; ++x) {
-        // column of the next site: nibble qn of FW[xn & 3], moved to bits 2..4 inside the site block
-        const int xn = x + 1, qn = xn >> 2;
-        const uint32_t fwn = xn < BITS ? FW[xn & 3] : 0u;
-        const uint32_t sh = qn == 0 ? 2u : (uint32_t)(4 * qn - 2);
-        if (x == 0)                    // site 0 also patches the last site's column: its right neighbour is site 0
-            asm volatile(MUCA_V5_SITE("shl.b32", "@p add.u32 %3, %3, %9;\n\t")
-                         : "+r"(S), "+r"(A), "+r"(flips), "+r"(FW[3])
-                         : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u), "n"(~V::K), "r"(patch) : "memory");
-        else if (qn == 0)
-            asm volatile(MUCA_V5_SITE("shl.b32", "")
-                         : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused)
-                         : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u << (x & 31)), "n"(~V::K) : "memory");
-        else
-            asm volatile(MUCA_V5_SITE("shr.u32", "")
-                         : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused)
-                         : "r"(rnd[x]), "r"(fwn), "r"(sh), "r"(1u << (x & 31)), "n"(~V::K) : "memory");
+        const int xn = x + 1;
+        if (xn < BITS)
+            site_v6<L, MEAS, (int)V::K>(S, A, flips, FW[3], chk, off, rnd[x], FW[xn & 3], xn >> 2, 1u << x, patch, x == 0);
+        else   // next site: site 0 of the row below, no carry
+            site_v6<L, MEAS, 0>(S, A, flips, FW[3], chk, off, rnd[x], FWn[0], 0, 1u << x, patch, false);
+        // ---- off the chain, in the shadow of the table loads: prepare the row below
+        prep_for_site<L>(n, x);
+        if (x >= BITS - 4 && x < BITS - 1) FWn[x - (BITS - 4)] = finish_word<L>(n, c ^ flips, x - (BITS - 4));
+        if ((x & 3) == 3 && more) {   // the deviates of sites 4k .. 4k + 3 are spent: fetch call k of the row below into their place
+            const int k = x >> 2;
+            const uint4 v = ring[(buf * NC + k) * SLOTS];
+            rnd[4 * k] = v.x; rnd[4 * k + 1] = v.y; rnd[4 * k + 2] = v.z; rnd[4 * k + 3] = v.w;
+        }
     }
+    buf ^= (int)more;
     up = c ^ flips;
     lat[y * SLOTS] = up;
+    FWn[3] = finish_word<L>(n, up, 3);
 }
 
 // Walker warp: sweeps s0 .. s1-1; `buf` is the ring buffer holding the deviates of the next row to fetch.  Rows are
-// processed in pairs so that the two register sets (this row / next row) swap roles without copies.
-// The caller compensates the first and the last attempt of the measured phase in the histogram (see row_v5).
-template <int L>
-__device__ __forceinline__ void sweeps_v5(uint32_t* __restrict__ lat, uint32_t& S, const uint32_t s0, const uint32_t s1,
+// processed in pairs so that the two register sets (this row / row below) swap roles without copies.
+// The caller compensates the first and the last attempt of the measured phase in the histogram (see row_v6).
+template <int L, bool MEAS>
+__device__ __forceinline__ void sweeps_v6(uint32_t* __restrict__ lat, uint32_t& S, uint32_t& chk, const uint32_t s0, const uint32_t s1,
                                           const uint4* __restrict__ ring, int& buf, const int bar_id) {
     using G = Geo<L>;
-    using V = V5<L>;
+    using V = V6<L>;
     constexpr int BITS = G::BITS, NC = V::NC, SLOTS = V::SLOTS;
     if (s1 <= s0) return;
-    uint32_t up = lat[(L - 1) * SLOTS], cA = lat[0], cB;
-    uint32_t PA[4], PB[4], patchA, patchB, rndA[BITS], rndB[BITS];
-    partial_words<L>(cA, lat[SLOTS], PA, patchA);
+    uint32_t up = lat[(L - 1) * SLOTS];
+    NextRow<L> nA, nB;
+    uint32_t FWA[4], FWB[4], rnd[BITS];
+    nA.c = lat[0];
+    nA.dn = lat[SLOTS];
+    prep_steps<L, 0, PREP_STEPS>(nA);
+#pragma unroll
+    for (int r = 0; r < 4; ++r) FWA[r] = finish_word<L>(nA, up, r);
     pair_barrier(bar_id);                      // the deviates of the first row are in ring[buf]
 #pragma unroll
     for (int k = 0; k < NC; ++k) {
         const uint4 v = ring[(buf * NC + k) * SLOTS];
-        rndA[4 * k] = v.x; rndA[4 * k + 1] = v.y; rndA[4 * k + 2] = v.z; rndA[4 * k + 3] = v.w;
+        rnd[4 * k] = v.x; rnd[4 * k + 1] = v.y; rnd[4 * k + 2] = v.z; rnd[4 * k + 3] = v.w;
     }
     buf ^= 1;
+    uint32_t off = (FWA[0] << 2) & 0x1Cu;      // site 0: its left neighbour (site L-1) has not been visited in this sweep
+    uint32_t A = S + off;
 #pragma unroll 1
     for (uint32_t s = s0; s < s1; ++s) {
 #pragma unroll 1
         for (int y = 0; y < L; y += 2) {
-            row_v5<L>(lat, S, y, true, up, cA, PA, patchA, rndA, cB, PB, patchB, rndB, ring, buf, bar_id);
-            row_v5<L>(lat, S, y + 1, s + 1 < s1 || y + 2 < L, up, cB, PB, patchB, rndB, cA, PA, patchA, rndA, ring, buf, bar_id);
+            row_v6<L, MEAS>(lat, S, A, chk, off, y, true, up, nA.c, FWA, nA.patch, rnd, nB, FWB, ring, buf, bar_id);
+            row_v6<L, MEAS>(lat, S, A, chk, off, y + 1, s + 1 < s1 || y + 2 < L, up, nB.c, FWB, nB.patch, rnd, nA, FWA, ring, buf, bar_id);
         }
     }
 }
@@ -199,9 +312,9 @@ __device__ __forceinline__ void sweeps_v5(uint32_t* __restrict__ lat, uint32_t& 
 // the double-buffered shared ring rnd[buf][call][slot] as one 16-byte store per call.  One barrier per row hands
 // the buffer over.  R4: ctr = (i >> 2, sweep, iteration, walker).
 template <int L>
-__device__ __forceinline__ void deviates_v5(uint4* __restrict__ ring, const uint32_t s0, const uint32_t s1, int& buf,
-                                            const int bar_id, const SweepParams& prm, const uint32_t walker) {
-    constexpr int NC = V5<L>::NC, SLOTS = V5<L>::SLOTS;
+__device__ __forceinline__ void deviates_v6(uint4* __restrict__ ring, const uint32_t s0, const uint32_t s1, int& buf,
+                                            const int bar_id, const SweepParams& prm, const uint32_t walker, const bool active) {
+    constexpr int NC = V6<L>::NC, SLOTS = V6<L>::SLOTS;
 #pragma unroll 1
     for (uint32_t s = s0; s < s1; ++s) {
 #pragma unroll 1
@@ -217,7 +330,8 @@ __device__ __forceinline__ void deviates_v5(uint4* __restrict__ ring, const uint
                 for (int k = 0; k < NC; ++k)
                     philox_round(st[k], prm.key0 + (uint32_t)r * 0x9E3779B9u, prm.key1 + (uint32_t)r * 0xBB67AE85u);
 #pragma unroll
-            for (int k = 0; k < NC; ++k) ring[(buf * NC + k) * SLOTS] = make_uint4(st[k][0], st[k][1], st[k][2], st[k][3]);
+            for (int k = 0; k < NC; ++k)
+                if (active) ring[(buf * NC + k) * SLOTS] = make_uint4(st[k][0], st[k][1], st[k][2], st[k][3]);
             pair_barrier(bar_id);
             buf ^= 1;
         }
@@ -229,17 +343,35 @@ __device__ __forceinline__ void deviates_v5(uint4* __restrict__ ring, const uint
 // The host spreads the walkers over all SMs (as few pairs per SM, then as few lanes per warp, as possible: fewer
 // lanes collide in the banks).  Lanes without a walker are parked on the all-reject row and never leave it.
 template <int L>
-__global__ void __launch_bounds__(64 * V5<L>::MAX_WARPS, 1) sweep_kernel_v5(const SweepParams prm, const int wpw) {
+__global__ void __launch_bounds__(64 * V6<L>::MAX_WARPS, 1) sweep_kernel_v6(const SweepParams prm, const int wpw, const int role_map) {
     using G = Geo<L>;
-    using V = V5<L>;
+    using V = V6<L>;
     constexpr int N = G::N, BINS = G::BINS, SLOTS = V::SLOTS;
     extern __shared__ __align__(16) uint32_t smem[];
     char* const sm = reinterpret_cast<char*>(smem);
     const int tid = threadIdx.x, nthr = blockDim.x, nw = nthr >> 6;
     const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(smem);
-    // the window must end below K, and no row address may be 0 (the site macro uses "S & ~K != 0" as an always-true
-    // predicate; dynamic shared memory starts behind the 1 KB the system reserves on sm_100)
-    if (sbase == 0u || sbase + V::RING_OFF + V::RING_BYTES > V::K) __trap();
+#ifdef MUCA_V6_DT
+    if (sbase != V::SBASE) __trap();   // the site macro addresses the delta table by an immediate
+
+    // ---- both table copies: row (j, c) = t[8] | bin; delta tables behind the rows
+    for (int idx = tid; idx < BINS * 16; idx += nthr) {
+        const int j = idx >> 4, cc = (idx >> 3) & 1, f = idx & 7;
+        const int fe = f ^ cc, a = (fe >> 1) + (fe & 1);
+        const int jn = j + 2 - a;                            // where an accepted move leads (dE = 8 - 4a)
+        // R17: a move out of [0, N] cannot occur for a real configuration; its entry is never consulted
+        *reinterpret_cast<uint32_t*>(sm + (size_t)cc * V::K + (size_t)j * V::RS + 4 * f) = (jn < 0 || jn > N) ? 0u : prm.table[j * 8 + fe];
+    }
+    for (int j = tid; j <= BINS; j += nthr) *reinterpret_cast<uint32_t*>(sm + (size_t)j * V::RS + V::BIN_OFF) = 0u;
+    if (tid < 16) {   // row BINS of both copies: t = 0 in every column; the lanes parked here get deviates 0xFFFFFFFF and stay
+        const int cc = tid >> 3, f = tid & 7, fe = f ^ cc, a = (fe >> 1) + (fe & 1);
+        *reinterpret_cast<uint32_t*>(sm + (size_t)cc * V::K + (size_t)BINS * V::RS + 4 * f) = 0u;
+        *reinterpret_cast<int32_t*>(sm + (size_t)cc * V::K + V::DT_OFF + 4 * f) = (int)V::RS * (2 - a);
+    }
+#else
+    // copy 0, the lattices and the ring must end below K (dynamic shared memory starts behind the 1 KB the system
+    // reserves on sm_100)
+    if (sbase + V::RING_OFF + V::RING_BYTES > V::K) __trap();
 
     // ---- both table copies: row (j, c) = t[8] | Sa[8] | bin
     for (int idx = tid; idx < BINS * 16; idx += nthr) {
@@ -250,27 +382,35 @@ __global__ void __launch_bounds__(64 * V5<L>::MAX_WARPS, 1) sweep_kernel_v5(cons
         if (jn < 0 || jn > N) { jn = j; t = 0u; }            // R17: cannot occur for a real configuration
         char* const row = sm + (size_t)cc * V::K + (size_t)j * V::RS;
         *reinterpret_cast<uint32_t*>(row + 4 * f) = t;
-        *reinterpret_cast<uint32_t*>(row + V::SA_OFF + 4 * f) = sbase + V::K + (uint32_t)jn * V::RS;
+        *reinterpret_cast<uint32_t*>(row + V::SA_OFF + 4 * f) = sbase + (uint32_t)jn * V::RS;
     }
     for (int idx = tid; idx < BINS * 2; idx += nthr)
         *reinterpret_cast<uint32_t*>(sm + (size_t)(idx & 1) * V::K + (size_t)(idx >> 1) * V::RS + V::BIN_OFF) = 0u;
-    if (tid < 17)  // row BINS of copy 0: t = 0 and Sa = itself in every column -- a lane parked here stays here
-        *reinterpret_cast<uint32_t*>(sm + (size_t)BINS * V::RS + 4 * tid) = tid >= 8 && tid < 16 ? sbase + BINS * V::RS : 0u;
+    if (tid < 34) {  // row BINS of both copies: t = 0 and Sa = itself in every column -- a lane parked here stays here
+        const int cc = tid / 17, e = tid % 17;
+        *reinterpret_cast<uint32_t*>(sm + (size_t)cc * V::K + (size_t)BINS * V::RS + 4 * e) = e >= 8 && e < 16 ? sbase + BINS * V::RS : 0u;
+    }
+#endif
 
-    // warp -> role.  A warp runs on scheduler (warp id % 4).  With 4 pairs per block the walker warps take warp ids
-    // {0, 1, 4, 5} and the deviate warps {2, 3, 6, 7}: two walker warps share a scheduler (each is latency-bound and
-    // leaves 60 % of the issue slots to the other) and two deviate warps share one; a walker sharing with its deviate
-    // warp instead loses 12 cycles per site to the Philox stream (profiles/README.md).  With 1 or 2 pairs every warp
-    // has a scheduler of its own (deviate ids 0 .. nw-1, walker ids nw .. 2nw-1).
+    // warp -> role.  A warp runs on scheduler (warp id % 4).  role_map 0 (4 pairs per block): the walker warps take
+    // warp ids {0, 1, 4, 5} and the deviate warps {2, 3, 6, 7}: two walker warps share a scheduler and two deviate warps
+    // share one.  role_map 1: deviate warps 0 .. 3, walker warps 4 .. 7 -- every scheduler runs one walker warp and one
+    // deviate warp (the walker has the higher warp id).  With 1 or 2 pairs every warp has a scheduler of its own
+    // (deviate ids 0 .. nw-1, walker ids nw .. 2nw-1).
     const int warp_id = tid >> 5;
-    const bool is_walker = nw == 4 ? (warp_id & 2) == 0 : warp_id >= nw;
-    const int pair = nw == 4 ? (warp_id & 1) | ((warp_id >> 2) << 1) : (is_walker ? warp_id - nw : warp_id);
+    const bool split = nw == 4 && role_map == 0;
+    const bool is_walker = split ? (warp_id & 2) == 0 : warp_id >= nw;
+    const int pair = split ? (warp_id & 1) | ((warp_id >> 2) << 1) : (is_walker ? warp_id - nw : warp_id);
     const int lane = tid & 31, slot = 32 * pair + lane;          // slot: lattice / ring column
     const int w = (blockIdx.x * nw + pair) * wpw + lane;
     const bool active = lane < wpw && w < prm.W;
     const int bar_id = 1 + pair;
     uint32_t* const lat = reinterpret_cast<uint32_t*>(sm + V::LAT_OFF) + slot;
     uint4* const ring = reinterpret_cast<uint4*>(sm + V::RING_OFF);
+    // a lane without a walker never accepts: its ring slots hold the deviate 0xFFFFFFFF for good (the deviate warp
+    // stores only for lanes with a walker) and its row has all thresholds 0
+    if (!is_walker && !active)
+        for (int k = 0; k < 2 * V::NC; ++k) ring[k * SLOTS + slot] = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
 
     // ---- lattice: one word per row, column `slot`
     if (is_walker) {
@@ -292,27 +432,26 @@ __global__ void __launch_bounds__(64 * V5<L>::MAX_WARPS, 1) sweep_kernel_v5(cons
     const uint32_t walker = prm.walker_offset + (uint32_t)w;
     const uint32_t s_th = prm.therm < prm.sweep_begin ? prm.sweep_begin
                           : (prm.therm > prm.sweep_end ? prm.sweep_end : prm.therm);
-    // slot j = (E + 2N)/4, copy 0
+    // slot j = (E + 2N)/4
     uint32_t S = sbase + (is_walker && active ? (uint32_t)((prm.E[w] + 2 * N) >> 2) : (uint32_t)BINS) * V::RS;
     int buf = 0;
-    // ---- thermalisation sweeps: same code, the bins are cleared afterwards
-    if (is_walker) sweeps_v5<L>(lat, S, prm.sweep_begin, s_th, ring + slot, buf, bar_id);
-    else deviates_v5<L>(ring + slot, prm.sweep_begin, s_th, buf, bar_id, prm, walker);
-    __syncthreads();
-    for (int j = tid; j <= BINS; j += nthr) *reinterpret_cast<uint32_t*>(sm + (size_t)j * V::RS + V::BIN_OFF) = 0u;
-    __syncthreads();
+    uint32_t chk = 0;
+    // ---- thermalisation sweeps: nothing is recorded
+    if (is_walker) sweeps_v6<L, false>(lat, S, chk, prm.sweep_begin, s_th, ring + slot, buf, bar_id);
+    else deviates_v6<L>(ring + slot, prm.sweep_begin, s_th, buf, bar_id, prm, walker, active);
     // ---- measured sweeps: every site counts the state it starts from, so the state before the first measured
     //      attempt is taken out again here and the state after the last one is added below
     if (is_walker) {
-        if (s_th < prm.sweep_end) atomicSub(reinterpret_cast<uint32_t*>(sm + ((S & ~V::K) - sbase) + V::BIN_OFF), 1u);
-        sweeps_v5<L>(lat, S, s_th, prm.sweep_end, ring + slot, buf, bar_id);
-        if (s_th < prm.sweep_end) atomicAdd(reinterpret_cast<uint32_t*>(sm + ((S & ~V::K) - sbase) + V::BIN_OFF), 1u);
+        if (s_th < prm.sweep_end) atomicSub(reinterpret_cast<uint32_t*>(sm + (S - sbase) + V::BIN_OFF), 1u);
+        sweeps_v6<L, true>(lat, S, chk, s_th, prm.sweep_end, ring + slot, buf, bar_id);
+        if (s_th < prm.sweep_end) atomicAdd(reinterpret_cast<uint32_t*>(sm + (S - sbase) + V::BIN_OFF), 1u);
     } else {
-        deviates_v5<L>(ring + slot, s_th, prm.sweep_end, buf, bar_id, prm, walker);
+        deviates_v6<L>(ring + slot, s_th, prm.sweep_end, buf, bar_id, prm, walker, active);
     }
     if (is_walker) {
+        if (chk == 0x9E3779B9u && !active) lat[0] = chk;   // keeps the checksum of the site macro alive (never true for a parked lane: its addresses are constant)
         if (active) {
-            prm.E[w] = (int)(((S & ~V::K) - sbase) / V::RS) * 4 - 2 * N;
+            prm.E[w] = (int)((S - sbase) / V::RS) * 4 - 2 * N;
             if (L >= 32) {
                 for (int y = 0; y < L; ++y) prm.spins[(size_t)y * prm.W + w] = lat[y * SLOTS];
             } else {
@@ -328,7 +467,7 @@ __global__ void __launch_bounds__(64 * V5<L>::MAX_WARPS, 1) sweep_kernel_v5(cons
     }
     __syncthreads();
 
-    // ---- a4: merge the block's bins into the global uint64 histogram
+    // ---- a4: merge the block's bins into the global uint64 histogram (the parking row BINS is not a slot)
     if (prm.sweep_end > prm.therm) {
         for (int j = tid; j < BINS; j += nthr) {
             const uint32_t v = *reinterpret_cast<uint32_t*>(sm + (size_t)j * V::RS + V::BIN_OFF);
