@@ -3,18 +3,20 @@
 // with deviate warps, everything that is not the per-site chain spread over the sites of the previous row.
 // Citations: "PAPER.md:<line>" = /root/reference/PAPER.md, "R<n>" = DESIGN.md section 3.
 //
-// The walker's dynamic state is the shared-memory address S = rowaddr(j) of its energy slot j; the carry
-// c = [previous site of this row flipped] lives in the ENTRY address A of the next lookup.  The table is stored twice:
-// copy c at byte offset c*K (K a power of two above copy 0, the lattices and the deviate ring); copy 1 has its columns
-// permuted (f -> f ^ 1: a flipped left neighbour toggles the [left != s] bit of the column index).  Row (j, c) is 68
-// bytes (17 words: consecutive rows rotate through all 32 banks):
-//     +4f      t  = thresh[j][a],  a = a(f ^ c)          (PAPER.md:109 acceptance, R6/R7)
-//     +32+4f   Sa = rowaddr(j + 2 - a)                    (state an ACCEPTED move leads to; a rejected one keeps S)
-//     +64      histogram bin of slot j (copy 0 only)
+// The walker's dynamic state is the shared-memory address S = rowaddr(j) of its energy slot j.  Row j is 36 bytes (9
+// words: consecutive rows rotate through all 32 banks):
+//     +4f      t = thresh[j][a(f)],  f = hl + 2*n3 the column of the site: n3 antiparallel bonds to up / down / right,
+//              hl = [left neighbour != s]                                  (PAPER.md:109 acceptance, R6/R7)
+//     +32      histogram bin of slot j
+// and behind the rows the delta table DT[f] = RS * (2 - a(f)): an accepted move leads to S + DT[f].  The carry
+// c = [previous site of this row flipped] toggles the hl bit of the column, f -> f ^ 1; it lives in the ENTRY address
+// A = S + 4 (f ^ c) of the lookup, never in S.
 // Per site the serial chain is   LDS t -> ISETP -> SEL(A_acc, A_rej) -> LDS t'   with BOTH candidates of the next
-// entry address, A_acc = Sa + K + 4f' and A_rej = S + 4f', formed before the decision (round 1, v5, selected the
-// state and added the column afterwards: ISETP -> SEL -> IADD -> LDS).  Philox runs in a paired "deviate" warp (same
-// walkers) that feeds a double-buffered shared ring one row ahead.
+// entry address, A_acc = S + DT[f ^ c] + 4 (f' ^ 1) and A_rej = S + 4 f', formed before the decision (round 1, v5,
+// selected the state and added the column afterwards, ISETP -> SEL -> IADD -> LDS, kept two copies of the table for
+// the two values of the carry and loaded the next state from the row: a second load with ~3.3 bank-conflict
+// wavefronts).  Philox runs in a paired "deviate" warp (same walkers) that feeds a double-buffered shared ring one
+// row ahead.
 //
 // What the ncu source view of v5 showed (profiles/README.md, round 2): a steady-state site cost 46 cycles, but the
 // row prologue -- eight 16-byte ring loads in one burst (32 wavefronts queued in front of the first table loads) and
@@ -27,45 +29,19 @@
 
 namespace muca {
 
-#ifndef MUCA_SITE_VARIANT
-#define MUCA_SITE_VARIANT 7
-#endif
-#if MUCA_SITE_VARIANT == 7
-#define MUCA_V6_DT 1   // the state an accepted move leads to is computed from a 16-word delta table instead of loaded from the row
-#endif
-
 template <int L>
 struct V6 {
     static constexpr uint32_t SBASE = 1024;                  // dynamic shared memory starts behind the 1 KB the system reserves on sm_100 (checked)
     static constexpr uint32_t BINS = L * L + 1;
-#ifdef MUCA_V6_DT
-    // row (j, c): t[8] | bin (copy 0 only) = 9 words (odd: consecutive rows rotate through all 32 banks);
-    // behind the rows of copy c: DT[c][f] = RS * (2 - a(f ^ c)), the state change of an accepted move
-    static constexpr uint32_t RS = 36, BIN_OFF = 32;
+    static constexpr uint32_t RS = 36, BIN_OFF = 32;         // row j: t[8] | bin
     static constexpr uint32_t DT_OFF = (BINS + 1) * RS;      // + one all-reject row: parking place of unused lanes
-    static constexpr uint32_t COPY_BYTES = DT_OFF + 32;
-    // K = offset of copy 1; K % 128 == 32 puts DT[1][f] into other banks than DT[0][f]: a warp's delta load is one wavefront
-    static constexpr uint32_t K = (COPY_BYTES + 127u) / 128u * 128u + 32u;
-    static constexpr uint32_t LAT_OFF = (K + COPY_BYTES + 15u) & ~15u;
-#else
-    static constexpr uint32_t RS = 68;
-    static constexpr uint32_t SA_OFF = 32, BIN_OFF = 64;
-    static constexpr uint32_t TBL_BYTES = (BINS + 1) * RS;   // + one all-reject row: parking place of unused lanes
-    static constexpr int KBIT = L == 32 ? 17 : (L == 16 ? 16 : 15);
-    static constexpr uint32_t K = 1u << KBIT;
-    static constexpr uint32_t LAT_OFF = (TBL_BYTES + 15u) & ~15u;
-#endif
+    static constexpr uint32_t LAT_OFF = (DT_OFF + 32u + 15u) & ~15u;
     static constexpr int MAX_WARPS = 4;                      // walker warps per block (+ as many deviate warps)
     static constexpr int SLOTS = 32 * MAX_WARPS;             // lattice / ring columns
     static constexpr int NC = Geo<L>::BITS / 4;              // Philox calls per row
     static constexpr uint32_t RING_OFF = LAT_OFF + (uint32_t)L * 4u * SLOTS;
     static constexpr uint32_t RING_BYTES = 2u * NC * 16u * SLOTS;
-#ifdef MUCA_V6_DT
     static constexpr size_t SMEM_BYTES = (size_t)RING_OFF + RING_BYTES;
-#else
-    static_assert(1024u + RING_OFF + RING_BYTES <= K, "copy 0 + lattices + ring must end below K");
-    static constexpr size_t SMEM_BYTES = (size_t)K + TBL_BYTES;
-#endif
 };
 
 // Field words of a row: nibble q of FW[r] holds the column f = hl + 2*n3 of site 4q + r (hl: bond to the left
@@ -116,22 +92,6 @@ __device__ __forceinline__ void prep_steps(NextRow<L>& n) {
         prep_steps<L, I0 + 1, I1>(n);
     }
 }
-// the steps that follow site x of the row above: sites 0 .. BITS-5 share the PREP_STEPS steps evenly, the last four
-// sites are left to finish_word
-template <int L>
-__device__ __forceinline__ void prep_for_site(NextRow<L>& n, const int x) {
-    constexpr int D = Geo<L>::BITS - 4;
-    switch (x) {
-#define MUCA_PREP_CASE(X) case X: if constexpr (X < D) prep_steps<L, (X * PREP_STEPS) / D, ((X + 1) * PREP_STEPS) / D>(n); break;
-        MUCA_PREP_CASE(0) MUCA_PREP_CASE(1) MUCA_PREP_CASE(2) MUCA_PREP_CASE(3) MUCA_PREP_CASE(4) MUCA_PREP_CASE(5) MUCA_PREP_CASE(6)
-        MUCA_PREP_CASE(7) MUCA_PREP_CASE(8) MUCA_PREP_CASE(9) MUCA_PREP_CASE(10) MUCA_PREP_CASE(11) MUCA_PREP_CASE(12)
-        MUCA_PREP_CASE(13) MUCA_PREP_CASE(14) MUCA_PREP_CASE(15) MUCA_PREP_CASE(16) MUCA_PREP_CASE(17) MUCA_PREP_CASE(18)
-        MUCA_PREP_CASE(19) MUCA_PREP_CASE(20) MUCA_PREP_CASE(21) MUCA_PREP_CASE(22) MUCA_PREP_CASE(23) MUCA_PREP_CASE(24)
-        MUCA_PREP_CASE(25) MUCA_PREP_CASE(26) MUCA_PREP_CASE(27)
-#undef MUCA_PREP_CASE
-        default: break;
-    }
-}
 // FW[r] of the row below `above_new` (bits 4q + r of above_new must be final)
 template <int L>
 __device__ __forceinline__ uint32_t finish_word(const NextRow<L>& n, const uint32_t above_new, const int r) {
@@ -139,132 +99,124 @@ __device__ __forceinline__ uint32_t finish_word(const NextRow<L>& n, const uint3
     return n.P[r] + 2u * (((n.c ^ above_new) >> r) & M);
 }
 
-// One site of the walker chain, in PTX.
-//   %0 S: state address (in/out)    %1 A: entry address of this site (in), of the next site (out)
-//   %2 flips (in/out)   %3 FW[3] at site 0 (in/out)   %4 deviate   %5 field word of the NEXT site   %6 its shift
-//   %7 flip mask of this site   %8 K (0 at the last site of a row: the next row starts without a carry)   %9 patch (site 0)
-// H[j]++ of the PREVIOUS attempt is issued behind this site's table loads (S still holds that state); thermalisation
-// sweeps leave it out.  The flip mask is a predicated OR.
-//   %0 S   %1 A   %2 flips   %3 FW[3] at site 0   %4 checksum   %5 delta-table offset A - S (variant 7)
-//   %6 deviate   %7 field word of the NEXT site   %8 its shift   %9 flip mask   %10 K (0 at the last site of a row)
-//   %11 patch (site 0)   %12 address of DT[0][0] (variant 7)
-#if MUCA_SITE_VARIANT == 3     // Sa loaded from the row (in front of t: volatile loads keep their order)
-#define MUCA_V6_SITE(SHIFT_OP, HIST_LINE, EXTRA_LINE)                            \
-    "{\n\t.reg .pred p;\n\t.reg .b32 t, sa, g0, g, gk, ar, aa;\n\t"              \
-    "ld.volatile.shared.u32 sa, [%1+32];\n\t"                                    \
-    "ld.volatile.shared.u32 t, [%1];\n\t" HIST_LINE                              \
-    SHIFT_OP " g0, %7, %8;\n\t"                                                  \
-    "and.b32 g, g0, 0x1C;\n\t"                                                   \
-    "add.u32 ar, %0, g;\n\t"                                                     \
-    "add.u32 gk, g, %10;\n\t"                                                    \
-    "add.u32 aa, sa, gk;\n\t"                                                    \
-    "mad.lo.u32 %4, aa, ar, %4;\n\t"                                             \
-    "setp.le.u32 p, %6, t;\n\t"                                                  \
-    "selp.u32 %1, aa, ar, p;\n\t"                                                \
-    "selp.u32 %0, sa, %0, p;\n\t"                                                \
-    "@p or.b32 %2, %2, %9;\n\t" EXTRA_LINE "}"
-#elif MUCA_SITE_VARIANT == 7   // Sa = S + DT[A - S]: a conflict-free load behind the table load; the offset A - S is selected like A
-#define MUCA_V6_SITE(SHIFT_OP, HIST_LINE, EXTRA_LINE)                            \
-    "{\n\t.reg .pred p;\n\t.reg .b32 t, d, sa, g0, g, gk, ar, aa, sg;\n\t"       \
+// One site of the walker chain, in PTX.  Operands:
+//   %0 S: state address (in/out)      %1 A: entry address of this site (in), of the next site (out)
+//   %2 flips (in/out)                 %3 FW[3] at site 0 (in/out)          %4 checksum (in/out, see below)
+//   %5 off = A - S = 4 (f ^ c): offset into the delta table (in: this site, out: next site)
+//   %6 g1 = 4f of the NEXT site (in), of the site after it (out)           %7 gx1 = g1 ^ 4 (same; g1 where a row starts)
+//   %8 deviate   %9 field word of the site AFTER the next   %10 its shift   %11 flip mask of this site
+//   %12 the constant 4 in a register   %13 patch (site 0)   %14 address of DT[0]
+// What ptxas does not do by itself (profiles/README.md, round 2; SASS checked with cuobjdump):
+//  * the decision must be consumed by SELs: ISETP -> SEL -> LDS costs ~9 cycles, ISETP -> predicated instruction ->
+//    LDS about 20.  ptxas turns "A = p ? aa : ar" into "A = aa; @!p A = S + g" unless BOTH candidates have a second,
+//    unconditional use: the multiply-add into the checksum %4 (FMA pipe, idle in a walker warp; the checksum is kept
+//    alive by a store that never executes).  The state itself may be a predicated add: it is off the chain.
+//  * the table load is issued in front of the (conflict-free, one-wavefront) delta load: volatile loads keep their order.
+// The column of the site after the next is extracted here, a site early, so that both candidates can be formed as soon
+// as the delta arrives.  H[j]++ of the PREVIOUS attempt is issued behind this site's loads (S still holds that state);
+// thermalisation sweeps leave it out.  The flip mask is a predicated OR.
+#define MUCA_V6_SITE(SHIFT_OP, HIST_LINE, GX_LINE, EXTRA_LINE)                   \
+    "{\n\t.reg .pred p;\n\t.reg .b32 t, d, sa, gs, g2, gx2, ar, aa, sg;\n\t"     \
     "ld.volatile.shared.u32 t, [%1];\n\t"                                        \
-    "ld.volatile.shared.u32 d, [%5+%12];\n\t" HIST_LINE                          \
-    SHIFT_OP " g0, %7, %8;\n\t"                                                  \
-    "and.b32 g, g0, 0x1C;\n\t"                                                   \
-    "add.u32 ar, %0, g;\n\t"                                                     \
-    "add.u32 gk, g, %10;\n\t"                                                    \
-    "add.u32 sg, %0, gk;\n\t"                                                    \
+    "ld.volatile.shared.u32 d, [%5+%14];\n\t" HIST_LINE                          \
+    SHIFT_OP " gs, %9, %10;\n\t"                                                 \
+    "add.u32 ar, %0, %6;\n\t"                                                    \
+    "add.u32 sg, %0, %7;\n\t"                                                    \
+    "and.b32 g2, gs, 0x1C;\n\t" GX_LINE                                          \
     "add.u32 aa, sg, d;\n\t"                                                     \
     "add.u32 sa, %0, d;\n\t"                                                     \
     "mad.lo.u32 %4, aa, ar, %4;\n\t"                                             \
-    "setp.le.u32 p, %6, t;\n\t"                                                  \
+    "setp.le.u32 p, %8, t;\n\t"                                                  \
     "selp.u32 %1, aa, ar, p;\n\t"                                                \
-    "selp.u32 %5, gk, g, p;\n\t"                                                 \
+    "selp.u32 %5, %7, %6, p;\n\t"                                                \
     "selp.u32 %0, sa, %0, p;\n\t"                                                \
-    "@p or.b32 %2, %2, %9;\n\t" EXTRA_LINE "}"
-#endif
-#ifdef MUCA_V6_DT
+    "@p or.b32 %2, %2, %11;\n\t" EXTRA_LINE                                      \
+    "mov.u32 %6, g2;\n\tmov.u32 %7, gx2;\n\t}"
 #define MUCA_V6_HIST "red.shared.add.u32 [%0+32], 1;\n\t"
-#else
-#define MUCA_V6_HIST "red.shared.add.u32 [%0+64], 1;\n\t"
-#endif
+#define MUCA_V6_GX_CARRY "lop3.b32 gx2, gs, 0x1C, %12, 0x6A;\n\t"   /* (gs & 0x1C) ^ 4: the column if this site's left neighbour has flipped */
+#define MUCA_V6_GX_ROWSTART "mov.u32 gx2, g2;\n\t"                  /* site 0 of a row: its left neighbour has not been visited in this sweep */
+#define MUCA_V6_PATCH "@p add.u32 %3, %3, %13;\n\t"
 
-template <int L, bool MEAS, int KK>
-__device__ __forceinline__ void site_v6(uint32_t& S, uint32_t& A, uint32_t& flips, uint32_t& fw3, uint32_t& chk, uint32_t& off, const uint32_t rnd,
-                                        const uint32_t fwn, const int qn, const uint32_t mask, const uint32_t patch,
-                                        const bool first) {
-    const uint32_t sh = qn == 0 ? 2u : (uint32_t)(4 * qn - 2);   // nibble qn of the field word -> bits 2..4
-    uint32_t unused = 0;   // fills operand %3 of the site macro where site 0 has FW[3]
-#ifdef MUCA_V6_DT
+enum { SITE_FIRST = 0, SITE_SHL = 1, SITE_SHR = 2, SITE_ROWSTART = 3 };   // flavour of the site macro
+
+template <int L, bool MEAS, int FLAVOUR>
+__device__ __forceinline__ void site_v6(uint32_t& S, uint32_t& A, uint32_t& flips, uint32_t& fw3, uint32_t& chk, uint32_t& off,
+                                        uint32_t& g1, uint32_t& gx1, const uint32_t rnd, const uint32_t fw2, const uint32_t sh2,
+                                        const uint32_t mask, const uint32_t patch) {
     constexpr uint32_t DTA = V6<L>::SBASE + V6<L>::DT_OFF;
-#else
-    constexpr uint32_t DTA = 0;
-#endif
-    if (first) {   // site 0 also patches the last site's column: its right neighbour is site 0
-        if (MEAS)
-            asm volatile(MUCA_V6_SITE("shl.b32", MUCA_V6_HIST, "@p add.u32 %3, %3, %11;\n\t")
-                         : "+r"(S), "+r"(A), "+r"(flips), "+r"(fw3), "+r"(chk), "+r"(off)
-                         : "r"(rnd), "r"(fwn), "r"(sh), "r"(mask), "n"(KK), "r"(patch), "n"(DTA) : "memory");
-        else
-            asm volatile(MUCA_V6_SITE("shl.b32", "", "@p add.u32 %3, %3, %11;\n\t")
-                         : "+r"(S), "+r"(A), "+r"(flips), "+r"(fw3), "+r"(chk), "+r"(off)
-                         : "r"(rnd), "r"(fwn), "r"(sh), "r"(mask), "n"(KK), "r"(patch), "n"(DTA) : "memory");
-    } else if (qn == 0) {
-        if (MEAS)
-            asm volatile(MUCA_V6_SITE("shl.b32", MUCA_V6_HIST, "")
-                         : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused), "+r"(chk), "+r"(off)
-                         : "r"(rnd), "r"(fwn), "r"(sh), "r"(mask), "n"(KK), "r"(0), "n"(DTA) : "memory");
-        else
-            asm volatile(MUCA_V6_SITE("shl.b32", "", "")
-                         : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused), "+r"(chk), "+r"(off)
-                         : "r"(rnd), "r"(fwn), "r"(sh), "r"(mask), "n"(KK), "r"(0), "n"(DTA) : "memory");
+    uint32_t unused = 0;   // fills operand %3 of the site macro where site 0 has FW[3]
+#define MUCA_V6_ASM(SHIFT_OP, HIST, GX, EXTRA, FW3)                                                                    \
+    asm volatile(MUCA_V6_SITE(SHIFT_OP, HIST, GX, EXTRA)                                                               \
+                 : "+r"(S), "+r"(A), "+r"(flips), "+r"(FW3), "+r"(chk), "+r"(off), "+r"(g1), "+r"(gx1)                 \
+                 : "r"(rnd), "r"(fw2), "r"(sh2), "r"(mask), "r"(4u), "r"(patch), "n"(DTA) : "memory")
+    if constexpr (FLAVOUR == SITE_FIRST) {   // site 0 also patches the last site's column: its right neighbour is site 0
+        if constexpr (MEAS) MUCA_V6_ASM("shl.b32", MUCA_V6_HIST, MUCA_V6_GX_CARRY, MUCA_V6_PATCH, fw3);
+        else MUCA_V6_ASM("shl.b32", "", MUCA_V6_GX_CARRY, MUCA_V6_PATCH, fw3);
+    } else if constexpr (FLAVOUR == SITE_SHL) {
+        if constexpr (MEAS) MUCA_V6_ASM("shl.b32", MUCA_V6_HIST, MUCA_V6_GX_CARRY, "", unused);
+        else MUCA_V6_ASM("shl.b32", "", MUCA_V6_GX_CARRY, "", unused);
+    } else if constexpr (FLAVOUR == SITE_SHR) {
+        if constexpr (MEAS) MUCA_V6_ASM("shr.u32", MUCA_V6_HIST, MUCA_V6_GX_CARRY, "", unused);
+        else MUCA_V6_ASM("shr.u32", "", MUCA_V6_GX_CARRY, "", unused);
     } else {
-        if (MEAS)
-            asm volatile(MUCA_V6_SITE("shr.u32", MUCA_V6_HIST, "")
-                         : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused), "+r"(chk), "+r"(off)
-                         : "r"(rnd), "r"(fwn), "r"(sh), "r"(mask), "n"(KK), "r"(0), "n"(DTA) : "memory");
-        else
-            asm volatile(MUCA_V6_SITE("shr.u32", "", "")
-                         : "+r"(S), "+r"(A), "+r"(flips), "+r"(unused), "+r"(chk), "+r"(off)
-                         : "r"(rnd), "r"(fwn), "r"(sh), "r"(mask), "n"(KK), "r"(0), "n"(DTA) : "memory");
+        if constexpr (MEAS) MUCA_V6_ASM("shl.b32", MUCA_V6_HIST, MUCA_V6_GX_ROWSTART, "", unused);
+        else MUCA_V6_ASM("shl.b32", "", MUCA_V6_GX_ROWSTART, "", unused);
     }
+#undef MUCA_V6_ASM
 }
 
+// site x of a row (compile-time recursion: flavour, shifts and masks are constants)
+template <int L, bool MEAS, int X>
+struct RowSites {
+    static __device__ __forceinline__ void run(uint32_t& S, uint32_t& A, uint32_t& flips, uint32_t& chk, uint32_t& off, uint32_t& g1,
+                                               uint32_t& gx1, const uint32_t c, uint32_t (&FW)[4], const uint32_t patch,
+                                               uint32_t (&rnd)[Geo<L>::BITS], NextRow<L>& n, uint32_t (&FWn)[4],
+                                               const uint4* __restrict__ ring, const int buf, const bool more) {
+        constexpr int BITS = Geo<L>::BITS, NC = V6<L>::NC, SLOTS = V6<L>::SLOTS;
+        constexpr int X2 = X + 2;                              // the site whose column is extracted now
+        constexpr bool below = X2 >= BITS;                     // it belongs to the row below
+        constexpr int q2 = below ? 0 : X2 >> 2;
+        constexpr uint32_t sh2 = q2 == 0 ? 2u : (uint32_t)(4 * q2 - 2);   // nibble q2 of the field word -> bits 2..4
+        constexpr int FLAVOUR = X == 0 ? SITE_FIRST : (X2 == BITS ? SITE_ROWSTART : (q2 == 0 ? SITE_SHL : SITE_SHR));
+        site_v6<L, MEAS, FLAVOUR>(S, A, flips, FW[3], chk, off, g1, gx1, rnd[X], below ? FWn[X2 - BITS] : FW[X2 & 3], sh2,
+                                  1u << X, patch);
+        // ---- off the chain, in the shadow of the table loads: prepare the row below
+        constexpr int D = BITS - 4;
+        if constexpr (X < D) prep_steps<L, (X * PREP_STEPS) / D, ((X + 1) * PREP_STEPS) / D>(n);
+        if constexpr (X >= BITS - 4 && X < BITS - 1) FWn[X - (BITS - 4)] = finish_word<L>(n, c ^ flips, X - (BITS - 4));
+        if constexpr ((X & 3) == 3) {
+            if (more) {   // the deviates of sites 4k .. 4k + 3 are spent: fetch call k of the row below into their place
+                constexpr int k = X >> 2;
+                const uint4 v = ring[(buf * NC + k) * SLOTS];
+                rnd[4 * k] = v.x; rnd[4 * k + 1] = v.y; rnd[4 * k + 2] = v.z; rnd[4 * k + 3] = v.w;
+            }
+        }
+        if constexpr (X + 1 < BITS)
+            RowSites<L, MEAS, X + 1>::run(S, A, flips, chk, off, g1, gx1, c, FW, patch, rnd, n, FWn, ring, buf, more);
+    }
+};
+
 // One row of the walker warp.  In: the row above (`up`, final), this row's old value `c`, its finished field words FW,
-// its deviates rnd[] and the entry address A of site 0.  While the row is processed, the row below is prepared in `n`
-// (old value, partial planes), its field words FWn are finished and its deviates replace this row's in rnd[] (call k
-// after site 4k + 3).  Out: `up` = this row's new value, A = entry address of site 0 of the row below.
+// its deviates rnd[], the entry address A of site 0 (with off = A - S) and the column offsets g1, gx1 of site 1.  While
+// the row is processed, the row below is prepared in `n` (old value, partial planes), its field words FWn are finished
+// (FWn[r] as soon as the sites 4q + r of this row are final) and its deviates replace this row's in rnd[] (call k after
+// site 4k + 3).  Out: `up` = this row's new value, A / off / g1 / gx1 for the row below.
 // Every site increments the bin of the state it STARTS from, i.e. of the state after the previous attempt.
 template <int L, bool MEAS>
-__device__ __forceinline__ void row_v6(uint32_t* __restrict__ lat, uint32_t& S, uint32_t& A, uint32_t& chk, uint32_t& off, const int y, const bool more,
-                                       uint32_t& up, const uint32_t c, uint32_t (&FW)[4], const uint32_t patch,
-                                       uint32_t (&rnd)[Geo<L>::BITS], NextRow<L>& n, uint32_t (&FWn)[4],
+__device__ __forceinline__ void row_v6(uint32_t* __restrict__ lat, uint32_t& S, uint32_t& A, uint32_t& chk, uint32_t& off, uint32_t& g1,
+                                       uint32_t& gx1, const int y, const bool more, uint32_t& up, const uint32_t c, uint32_t (&FW)[4],
+                                       const uint32_t patch, uint32_t (&rnd)[Geo<L>::BITS], NextRow<L>& n, uint32_t (&FWn)[4],
                                        const uint4* __restrict__ ring, int& buf, const int bar_id) {
-    using G = Geo<L>;
     using V = V6<L>;
-    constexpr int BITS = G::BITS, NC = V::NC, SLOTS = V::SLOTS;
+    constexpr int SLOTS = V::SLOTS;
     // the deviates of row y + 1 are in ring[buf]; ring[buf ^ 1] (this row's, all fetched) may be refilled.  After the
-    // last row of a phase there is no such barrier (the deviate warp has left its loop) and what is fetched is not used.
+    // last row of a phase there is no such barrier (the deviate warp has left its loop) and nothing is fetched.
     if (more) pair_barrier(bar_id);
     const int y1 = (y + 1) & (L - 1), y2 = (y + 2) & (L - 1);
     n.c = lat[y1 * SLOTS];
     n.dn = lat[y2 * SLOTS];   // row y + 2 is old (or row 0, final in this sweep, when y + 1 = L - 1)
     uint32_t flips = 0;
-#pragma unroll
-    for (int x = 0; x < BITS; ++x) {
-        const int xn = x + 1;
-        if (xn < BITS)
-            site_v6<L, MEAS, (int)V::K>(S, A, flips, FW[3], chk, off, rnd[x], FW[xn & 3], xn >> 2, 1u << x, patch, x == 0);
-        else   // next site: site 0 of the row below, no carry
-            site_v6<L, MEAS, 0>(S, A, flips, FW[3], chk, off, rnd[x], FWn[0], 0, 1u << x, patch, false);
-        // ---- off the chain, in the shadow of the table loads: prepare the row below
-        prep_for_site<L>(n, x);
-        if (x >= BITS - 4 && x < BITS - 1) FWn[x - (BITS - 4)] = finish_word<L>(n, c ^ flips, x - (BITS - 4));
-        if ((x & 3) == 3 && more) {   // the deviates of sites 4k .. 4k + 3 are spent: fetch call k of the row below into their place
-            const int k = x >> 2;
-            const uint4 v = ring[(buf * NC + k) * SLOTS];
-            rnd[4 * k] = v.x; rnd[4 * k + 1] = v.y; rnd[4 * k + 2] = v.z; rnd[4 * k + 3] = v.w;
-        }
-    }
+    RowSites<L, MEAS, 0>::run(S, A, flips, chk, off, g1, gx1, c, FW, patch, rnd, n, FWn, ring, buf, more);
     buf ^= (int)more;
     up = c ^ flips;
     lat[y * SLOTS] = up;
@@ -298,12 +250,14 @@ __device__ __forceinline__ void sweeps_v6(uint32_t* __restrict__ lat, uint32_t& 
     buf ^= 1;
     uint32_t off = (FWA[0] << 2) & 0x1Cu;      // site 0: its left neighbour (site L-1) has not been visited in this sweep
     uint32_t A = S + off;
+    uint32_t g1 = (FWA[1] << 2) & 0x1Cu, gx1 = g1 ^ 4u;
 #pragma unroll 1
     for (uint32_t s = s0; s < s1; ++s) {
 #pragma unroll 1
         for (int y = 0; y < L; y += 2) {
-            row_v6<L, MEAS>(lat, S, A, chk, off, y, true, up, nA.c, FWA, nA.patch, rnd, nB, FWB, ring, buf, bar_id);
-            row_v6<L, MEAS>(lat, S, A, chk, off, y + 1, s + 1 < s1 || y + 2 < L, up, nB.c, FWB, nB.patch, rnd, nA, FWA, ring, buf, bar_id);
+            row_v6<L, MEAS>(lat, S, A, chk, off, g1, gx1, y, true, up, nA.c, FWA, nA.patch, rnd, nB, FWB, ring, buf, bar_id);
+            row_v6<L, MEAS>(lat, S, A, chk, off, g1, gx1, y + 1, s + 1 < s1 || y + 2 < L, up, nB.c, FWB, nB.patch, rnd, nA, FWA, ring, buf,
+                            bar_id);
         }
     }
 }
@@ -351,46 +305,21 @@ __global__ void __launch_bounds__(64 * V6<L>::MAX_WARPS, 1) sweep_kernel_v6(cons
     char* const sm = reinterpret_cast<char*>(smem);
     const int tid = threadIdx.x, nthr = blockDim.x, nw = nthr >> 6;
     const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(smem);
-#ifdef MUCA_V6_DT
     if (sbase != V::SBASE) __trap();   // the site macro addresses the delta table by an immediate
 
-    // ---- both table copies: row (j, c) = t[8] | bin; delta tables behind the rows
-    for (int idx = tid; idx < BINS * 16; idx += nthr) {
-        const int j = idx >> 4, cc = (idx >> 3) & 1, f = idx & 7;
-        const int fe = f ^ cc, a = (fe >> 1) + (fe & 1);
+    // ---- table: row j = t[8] | bin; delta table behind the rows
+    for (int idx = tid; idx < BINS * 8; idx += nthr) {
+        const int j = idx >> 3, f = idx & 7, a = (f >> 1) + (f & 1);
         const int jn = j + 2 - a;                            // where an accepted move leads (dE = 8 - 4a)
         // R17: a move out of [0, N] cannot occur for a real configuration; its entry is never consulted
-        *reinterpret_cast<uint32_t*>(sm + (size_t)cc * V::K + (size_t)j * V::RS + 4 * f) = (jn < 0 || jn > N) ? 0u : prm.table[j * 8 + fe];
+        *reinterpret_cast<uint32_t*>(sm + (size_t)j * V::RS + 4 * f) = (jn < 0 || jn > N) ? 0u : prm.table[idx];
     }
     for (int j = tid; j <= BINS; j += nthr) *reinterpret_cast<uint32_t*>(sm + (size_t)j * V::RS + V::BIN_OFF) = 0u;
-    if (tid < 16) {   // row BINS of both copies: t = 0 in every column; the lanes parked here get deviates 0xFFFFFFFF and stay
-        const int cc = tid >> 3, f = tid & 7, fe = f ^ cc, a = (fe >> 1) + (fe & 1);
-        *reinterpret_cast<uint32_t*>(sm + (size_t)cc * V::K + (size_t)BINS * V::RS + 4 * f) = 0u;
-        *reinterpret_cast<int32_t*>(sm + (size_t)cc * V::K + V::DT_OFF + 4 * f) = (int)V::RS * (2 - a);
+    if (tid < 8) {   // row BINS: t = 0 in every column; the lanes parked here get deviates 0xFFFFFFFF and stay
+        const int f = tid, a = (f >> 1) + (f & 1);
+        *reinterpret_cast<uint32_t*>(sm + (size_t)BINS * V::RS + 4 * f) = 0u;
+        *reinterpret_cast<int32_t*>(sm + V::DT_OFF + 4 * f) = (int)V::RS * (2 - a);
     }
-#else
-    // copy 0, the lattices and the ring must end below K (dynamic shared memory starts behind the 1 KB the system
-    // reserves on sm_100)
-    if (sbase + V::RING_OFF + V::RING_BYTES > V::K) __trap();
-
-    // ---- both table copies: row (j, c) = t[8] | Sa[8] | bin
-    for (int idx = tid; idx < BINS * 16; idx += nthr) {
-        const int j = idx >> 4, cc = (idx >> 3) & 1, f = idx & 7;
-        const int fe = f ^ cc, a = (fe >> 1) + (fe & 1);
-        int jn = j + 2 - a;                                  // where an accepted move leads (dE = 8 - 4a)
-        uint32_t t = prm.table[j * 8 + fe];
-        if (jn < 0 || jn > N) { jn = j; t = 0u; }            // R17: cannot occur for a real configuration
-        char* const row = sm + (size_t)cc * V::K + (size_t)j * V::RS;
-        *reinterpret_cast<uint32_t*>(row + 4 * f) = t;
-        *reinterpret_cast<uint32_t*>(row + V::SA_OFF + 4 * f) = sbase + (uint32_t)jn * V::RS;
-    }
-    for (int idx = tid; idx < BINS * 2; idx += nthr)
-        *reinterpret_cast<uint32_t*>(sm + (size_t)(idx & 1) * V::K + (size_t)(idx >> 1) * V::RS + V::BIN_OFF) = 0u;
-    if (tid < 34) {  // row BINS of both copies: t = 0 and Sa = itself in every column -- a lane parked here stays here
-        const int cc = tid / 17, e = tid % 17;
-        *reinterpret_cast<uint32_t*>(sm + (size_t)cc * V::K + (size_t)BINS * V::RS + 4 * e) = e >= 8 && e < 16 ? sbase + BINS * V::RS : 0u;
-    }
-#endif
 
     // warp -> role.  A warp runs on scheduler (warp id % 4).  role_map 0 (4 pairs per block): the walker warps take
     // warp ids {0, 1, 4, 5} and the deviate warps {2, 3, 6, 7}: two walker warps share a scheduler and two deviate warps
