@@ -16,6 +16,7 @@
 #include "muca_resident.cuh"
 #include "muca_random_site.cuh"
 #include "muca_window.cuh"
+#include "muca_streamed.cuh"
 
 using namespace muca;
 
@@ -175,7 +176,8 @@ int launch_sweep_t(muca_ctx* ctx, const SweepParams& prm, int tpb) {
     return MUCA_OK;
 }
 
-constexpr int MODE_WPAIR = 7;    // sweep_kernel_wpair: the same with Philox in paired deviate warps
+constexpr int MODE_WPAIR = 7;    // sweep_kernel_wpair: the same with Philox in paired deviate warps (round 1)
+constexpr int MODE_S6 = 8;       // sweep_kernel_s6 (muca_streamed.cuh): streamed lattices, v6 site chain, paired deviate warps
 constexpr int MODE_WINDOW = 6;   // sweep_kernel_window (muca_window.cuh): streamed lattices + a window of the table in shared memory
 struct Plan { int mode; int tpb; int nw; int wpw; };   // tpb = walkers per block; v5: nw warp pairs x wpw walkers per warp
 
@@ -190,7 +192,7 @@ Plan make_plan(const muca_ctx* c) {
     if (kern == MUCA_KERNEL_RESIDENT) p.mode = L <= 32 ? MODE_V5 : MODE_TBL_L1;
     else if (kern == MUCA_KERNEL_RESIDENT_V3) p.mode = MODE_V3;
     else if (kern == MUCA_KERNEL_RESIDENT_V2) p.mode = MODE_TBL_SMEM;
-    else if (kern == MUCA_KERNEL_STREAMED_PAIRS) p.mode = L < 32 ? MODE_V5 : MODE_WPAIR;
+    else if (kern == MUCA_KERNEL_STREAMED_PAIRS) p.mode = L < 32 ? MODE_V5 : MODE_S6;
     else if (kern == MUCA_KERNEL_STREAMED_SMEM)
         p.mode = L < 32 ? MODE_V5 : (L == 128 || c->opt_window_rows > 0) ? MODE_WINDOW : MODE_STREAMED_SMEM;
     else p.mode = MODE_STREAMED;
@@ -213,12 +215,13 @@ Plan make_plan(const muca_ctx* c) {
         if (p.mode == MODE_V3) tpb = L == 32 ? 128 : 32;
         else if (p.mode == MODE_TBL_SMEM) tpb = 32;
         else if (p.mode == MODE_TBL_L1) tpb = L == 64 ? 64 : 32;
-        else if (p.mode == MODE_STREAMED_SMEM || p.mode == MODE_WINDOW || p.mode == MODE_WPAIR) {
+        else if (p.mode == MODE_STREAMED_SMEM || p.mode == MODE_WINDOW || p.mode == MODE_WPAIR || p.mode == MODE_S6) {
             // one block per SM (164 KB of table at L = 64): spread the walkers over all SMs
             const int n_sm = c->n_sm > 0 ? c->n_sm : 148;
             tpb = ((c->W + n_sm - 1) / n_sm + 31) / 32 * 32;
             if (tpb > 512) tpb = 512;
             if (p.mode == MODE_WPAIR && tpb > 32 * WPAIR_MAX_PAIRS) tpb = 32 * WPAIR_MAX_PAIRS;
+            if (p.mode == MODE_S6 && tpb > 32 * s6_max_pairs(L)) tpb = 32 * s6_max_pairs(L);
         }
         else tpb = 32;
     }
@@ -227,7 +230,7 @@ Plan make_plan(const muca_ctx* c) {
 }
 
 size_t plan_smem(int L, const Plan& p) {
-    if (p.mode == MODE_WINDOW || p.mode == MODE_WPAIR) return 0;   // sized at run time from what the device allows
+    if (p.mode == MODE_WINDOW || p.mode == MODE_WPAIR || p.mode == MODE_S6) return 0;   // sized at run time from what the device allows
     if (p.mode == MODE_V5) return L == 8 ? V6<8>::SMEM_BYTES : L == 16 ? V6<16>::SMEM_BYTES : V6<32>::SMEM_BYTES;
     if (p.mode == MODE_V3) return L == 8 ? V3<8>::SMEM_BYTES : L == 16 ? V3<16>::SMEM_BYTES : V3<32>::SMEM_BYTES;
     switch (L) {
@@ -275,6 +278,31 @@ int launch_wpair_t(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window&
                                                                                   win.sent_hi, ctx->d_flag);
     CU(cudaGetLastError());
     return MUCA_OK;
+}
+
+template <int L>
+int launch_s6_t(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& win) {
+    const int npairs = tpb / 32;
+    if (npairs < 1 || npairs > s6_max_pairs(L)) return fail(ctx, MUCA_EINVAL, "paired streamed kernel: 1 to %d warp pairs per block at L = %d", s6_max_pairs(L), L);
+    const size_t smem = s6_smem_bytes(win.n_rows, npairs);
+    static size_t configured = 0;
+    if (smem > configured) {
+        CU(cudaFuncSetAttribute(sweep_kernel_s6<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured = smem;
+    }
+    sweep_kernel_s6<L><<<(prm.W + tpb - 1) / tpb, 2 * tpb, smem, ctx->stream>>>(prm, win.j_lo, win.n_rows, win.sent_lo, win.sent_hi,
+                                                                               ctx->opt_role_map, ctx->d_flag);
+    CU(cudaGetLastError());
+    return MUCA_OK;
+}
+
+int launch_s6(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& win) {
+    switch (ctx->L) {
+        case 32: return launch_s6_t<32>(ctx, prm, tpb, win);
+        case 64: return launch_s6_t<64>(ctx, prm, tpb, win);
+        case 128: return launch_s6_t<128>(ctx, prm, tpb, win);
+    }
+    return fail(ctx, MUCA_EINVAL, "paired streamed kernel: L must be 32, 64 or 128");
 }
 
 int launch_wpair(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& win) {
@@ -546,7 +574,7 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
     fallback.mode = MODE_STREAMED; fallback.tpb = 32; fallback.nw = fallback.wpw = 0;
     Window win;
     bool guarded = false;   // the window has sentinel rows: the result counts only if no walker entered one
-    const bool windowed_plan = plan.mode == MODE_WINDOW || plan.mode == MODE_WPAIR;
+    const bool windowed_plan = plan.mode == MODE_WINDOW || plan.mode == MODE_WPAIR || plan.mode == MODE_S6;
     if (windowed_plan) {
         const size_t spin_bytes = (size_t)ctx->W * (ctx->N / 8);
         ctx->h_flag[0] = 0; ctx->h_flag[1] = 0x7FFFFFFF; ctx->h_flag[2] = -1;
@@ -556,8 +584,9 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
         CU(cudaMemcpyAsync(ctx->h_flag, ctx->d_flag, 3 * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
         CU(cudaStreamSynchronize(ctx->stream));
         const int lo = ctx->h_flag[1], hi = ctx->h_flag[2];
-        const size_t ring = plan.mode == MODE_WPAIR ? wpair_ring_bytes(plan.tpb / 32) : 0;
-        int cap = (int)(((size_t)max_smem - 1024 - ring) / (ROW_SMEM_WORDS * 4)) - 2 * WINDOW_PAD_ROWS;
+        const size_t ring = plan.mode == MODE_WPAIR ? wpair_ring_bytes(plan.tpb / 32) : plan.mode == MODE_S6 ? s6_ring_bytes(plan.tpb / 32) + 32 : 0;
+        int cap = plan.mode == MODE_S6 ? (int)(((size_t)max_smem - ring) / S6_RS) - 2 * S6_PAD_ROWS
+                                       : (int)(((size_t)max_smem - 1024 - ring) / (ROW_SMEM_WORDS * 4)) - 2 * WINDOW_PAD_ROWS;
         if (ctx->opt_window_rows > 0 && ctx->opt_window_rows < cap) cap = ctx->opt_window_rows;
         const int margin = 8;   // rows between the outermost walker and a sentinel at the start of the iteration
         if (cap >= ctx->n_bins) {
@@ -599,7 +628,8 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
             if (e > s + max_any) e = s + max_any;
             prm.sweep_begin = (uint32_t)s; prm.sweep_end = (uint32_t)e;
             const int rc = pl.mode == MODE_WINDOW ? launch_window(ctx, prm, pl.tpb, win)
-                           : pl.mode == MODE_WPAIR ? launch_wpair(ctx, prm, pl.tpb, win) : launch_sweep(ctx, prm, pl);
+                           : pl.mode == MODE_WPAIR ? launch_wpair(ctx, prm, pl.tpb, win)
+                           : pl.mode == MODE_S6 ? launch_s6(ctx, prm, pl.tpb, win) : launch_sweep(ctx, prm, pl);
             if (rc != MUCA_OK) return rc;
             ++launches;
             s = e;
@@ -611,7 +641,7 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
         const int rc = run_sweeps(plan);
         if (rc != MUCA_OK) return rc;
     }
-    if ((plan.mode == MODE_WINDOW || plan.mode == MODE_WPAIR) && guarded) {
+    if ((plan.mode == MODE_WINDOW || plan.mode == MODE_WPAIR || plan.mode == MODE_S6) && guarded) {
         CU(cudaMemcpyAsync(ctx->h_flag, ctx->d_flag, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
         CU(cudaStreamSynchronize(ctx->stream));
         if (ctx->h_flag[0]) {   // a walker left the window: repeat the iteration from the snapshot with the L1 kernel

@@ -52,6 +52,7 @@ struct V6 {
 template <int L>
 struct NextRow {
     uint32_t c, dn;            // the row (old value) and the row below it (old; row 0, already final, below row L-1)
+    uint32_t left, right;      // L >= 64: the words of the same row to the left / right of c (old values, periodic)
     uint32_t hl, hr, m0, m1;   // bond planes: left, right, (down + right) as sum and carry bits
     uint32_t t;
     uint32_t P[4];
@@ -65,10 +66,12 @@ __device__ __forceinline__ void prep_step(NextRow<L>& n) {
     using G = Geo<L>;
     constexpr int BITS = G::BITS;
     if constexpr (I == 0) {
-        const uint32_t rw = L >= 32 ? __funnelshift_r(n.c, n.c, 1) : ((n.c >> 1) | ((n.c & 1u) << (BITS - 1)));
+        const uint32_t rw = G::WPR > 1 ? __funnelshift_r(n.c, n.right, 1)
+                            : L >= 32 ? __funnelshift_r(n.c, n.c, 1) : ((n.c >> 1) | ((n.c & 1u) << (BITS - 1)));
         n.hr = n.c ^ rw;
     } else if constexpr (I == 1) {
-        const uint32_t lw = L >= 32 ? __funnelshift_l(n.c, n.c, 1) : (((n.c << 1) | (n.c >> (BITS - 1))) & G::MASK);
+        const uint32_t lw = G::WPR > 1 ? __funnelshift_l(n.left, n.c, 1)
+                            : L >= 32 ? __funnelshift_l(n.c, n.c, 1) : (((n.c << 1) | (n.c >> (BITS - 1))) & G::MASK);
         n.hl = n.c ^ lw;
     } else if constexpr (I == 2) {
         n.m0 = n.c ^ n.dn ^ n.hr;
@@ -139,11 +142,10 @@ __device__ __forceinline__ uint32_t finish_word(const NextRow<L>& n, const uint3
 
 enum { SITE_FIRST = 0, SITE_SHL = 1, SITE_SHR = 2, SITE_ROWSTART = 3 };   // flavour of the site macro
 
-template <int L, bool MEAS, int FLAVOUR>
+template <int L, bool MEAS, int FLAVOUR, uint32_t DTA>
 __device__ __forceinline__ void site_v6(uint32_t& S, uint32_t& A, uint32_t& flips, uint32_t& fw3, uint32_t& chk, uint32_t& off,
                                         uint32_t& g1, uint32_t& gx1, const uint32_t rnd, const uint32_t fw2, const uint32_t sh2,
                                         const uint32_t mask, const uint32_t patch) {
-    constexpr uint32_t DTA = V6<L>::SBASE + V6<L>::DT_OFF;
     uint32_t unused = 0;   // fills operand %3 of the site macro where site 0 has FW[3]
 #define MUCA_V6_ASM(SHIFT_OP, HIST, GX, EXTRA, FW3)                                                                    \
     asm volatile(MUCA_V6_SITE(SHIFT_OP, HIST, GX, EXTRA)                                                               \
@@ -165,34 +167,43 @@ __device__ __forceinline__ void site_v6(uint32_t& S, uint32_t& A, uint32_t& flip
 #undef MUCA_V6_ASM
 }
 
-// site x of a row (compile-time recursion: flavour, shifts and masks are constants)
-template <int L, bool MEAS, int X>
+// The deviate ring is written by another warp between two pair barriers: its pointers are NOT __restrict__ (with
+// __restrict__ the compiler reused the values of an earlier load of the same ring slot across the barrier).
+// Site X of a 32-site unit (a row for L <= 32, one word of a row for L >= 64); compile-time recursion: flavour, shifts
+// and masks are constants.  FIRST / LASTW: the unit is the first / last one of its lattice row.  FW: the unit's
+// field words; fw3t: FW[3] of the LAST unit of the row (site 0 of the row patches it); FWseq: the field words of the
+// next unit in typewriter order (the columns of its sites 0 and 1 are extracted at the end of this unit); (n, FWp):
+// the unit one lattice row below, prepared here.  DTA: address of the delta table; stride: uint4 elements between two
+// calls in the ring.
+template <int L, bool MEAS, int X, bool FIRST, bool LASTW, uint32_t DTA>
 struct RowSites {
     static __device__ __forceinline__ void run(uint32_t& S, uint32_t& A, uint32_t& flips, uint32_t& chk, uint32_t& off, uint32_t& g1,
-                                               uint32_t& gx1, const uint32_t c, uint32_t (&FW)[4], const uint32_t patch,
-                                               uint32_t (&rnd)[Geo<L>::BITS], NextRow<L>& n, uint32_t (&FWn)[4],
-                                               const uint4* __restrict__ ring, const int buf, const bool more) {
-        constexpr int BITS = Geo<L>::BITS, NC = V6<L>::NC, SLOTS = V6<L>::SLOTS;
+                                               uint32_t& gx1, const uint32_t c, uint32_t (&FW)[4], uint32_t& fw3t, const uint32_t patch,
+                                               uint32_t (&rnd)[Geo<L>::BITS], NextRow<L>& n, uint32_t (&FWp)[4],
+                                               const uint32_t (&FWseq)[4], const uint4* ring, const int stride,
+                                               const int buf, const bool more) {
+        constexpr int BITS = Geo<L>::BITS, NC = BITS / 4;
         constexpr int X2 = X + 2;                              // the site whose column is extracted now
-        constexpr bool below = X2 >= BITS;                     // it belongs to the row below
+        constexpr bool below = X2 >= BITS;                     // it belongs to the next unit
         constexpr int q2 = below ? 0 : X2 >> 2;
         constexpr uint32_t sh2 = q2 == 0 ? 2u : (uint32_t)(4 * q2 - 2);   // nibble q2 of the field word -> bits 2..4
-        constexpr int FLAVOUR = X == 0 ? SITE_FIRST : (X2 == BITS ? SITE_ROWSTART : (q2 == 0 ? SITE_SHL : SITE_SHR));
-        site_v6<L, MEAS, FLAVOUR>(S, A, flips, FW[3], chk, off, g1, gx1, rnd[X], below ? FWn[X2 - BITS] : FW[X2 & 3], sh2,
-                                  1u << X, patch);
-        // ---- off the chain, in the shadow of the table loads: prepare the row below
+        constexpr int FLAVOUR = (X == 0 && FIRST) ? SITE_FIRST : ((X2 == BITS && LASTW) ? SITE_ROWSTART : (q2 == 0 ? SITE_SHL : SITE_SHR));
+        site_v6<L, MEAS, FLAVOUR, DTA>(S, A, flips, fw3t, chk, off, g1, gx1, rnd[X], below ? FWseq[X2 - BITS] : FW[X2 & 3], sh2,
+                                       1u << X, patch);
+        // ---- off the chain, in the shadow of the table loads: prepare the unit below
         constexpr int D = BITS - 4;
         if constexpr (X < D) prep_steps<L, (X * PREP_STEPS) / D, ((X + 1) * PREP_STEPS) / D>(n);
-        if constexpr (X >= BITS - 4 && X < BITS - 1) FWn[X - (BITS - 4)] = finish_word<L>(n, c ^ flips, X - (BITS - 4));
+        if constexpr (X >= BITS - 4 && X < BITS - 1) FWp[X - (BITS - 4)] = finish_word<L>(n, c ^ flips, X - (BITS - 4));
         if constexpr ((X & 3) == 3) {
-            if (more) {   // the deviates of sites 4k .. 4k + 3 are spent: fetch call k of the row below into their place
+            if (more) {   // the deviates of sites 4k .. 4k + 3 are spent: fetch call k of the next unit into their place
                 constexpr int k = X >> 2;
-                const uint4 v = ring[(buf * NC + k) * SLOTS];
+                const uint4 v = ring[(buf * NC + k) * stride];
                 rnd[4 * k] = v.x; rnd[4 * k + 1] = v.y; rnd[4 * k + 2] = v.z; rnd[4 * k + 3] = v.w;
             }
         }
         if constexpr (X + 1 < BITS)
-            RowSites<L, MEAS, X + 1>::run(S, A, flips, chk, off, g1, gx1, c, FW, patch, rnd, n, FWn, ring, buf, more);
+            RowSites<L, MEAS, X + 1, FIRST, LASTW, DTA>::run(S, A, flips, chk, off, g1, gx1, c, FW, fw3t, patch, rnd, n, FWp, FWseq, ring,
+                                                            stride, buf, more);
     }
 };
 
@@ -206,7 +217,7 @@ template <int L, bool MEAS>
 __device__ __forceinline__ void row_v6(uint32_t* __restrict__ lat, uint32_t& S, uint32_t& A, uint32_t& chk, uint32_t& off, uint32_t& g1,
                                        uint32_t& gx1, const int y, const bool more, uint32_t& up, const uint32_t c, uint32_t (&FW)[4],
                                        const uint32_t patch, uint32_t (&rnd)[Geo<L>::BITS], NextRow<L>& n, uint32_t (&FWn)[4],
-                                       const uint4* __restrict__ ring, int& buf, const int bar_id) {
+                                       const uint4* ring, int& buf, const int bar_id) {
     using V = V6<L>;
     constexpr int SLOTS = V::SLOTS;
     // the deviates of row y + 1 are in ring[buf]; ring[buf ^ 1] (this row's, all fetched) may be refilled.  After the
@@ -216,7 +227,8 @@ __device__ __forceinline__ void row_v6(uint32_t* __restrict__ lat, uint32_t& S, 
     n.c = lat[y1 * SLOTS];
     n.dn = lat[y2 * SLOTS];   // row y + 2 is old (or row 0, final in this sweep, when y + 1 = L - 1)
     uint32_t flips = 0;
-    RowSites<L, MEAS, 0>::run(S, A, flips, chk, off, g1, gx1, c, FW, patch, rnd, n, FWn, ring, buf, more);
+    RowSites<L, MEAS, 0, true, true, V::SBASE + V::DT_OFF>::run(S, A, flips, chk, off, g1, gx1, c, FW, FW[3], patch, rnd, n, FWn, FWn, ring,
+                                                                SLOTS, buf, more);
     buf ^= (int)more;
     up = c ^ flips;
     lat[y * SLOTS] = up;
@@ -228,7 +240,7 @@ __device__ __forceinline__ void row_v6(uint32_t* __restrict__ lat, uint32_t& S, 
 // The caller compensates the first and the last attempt of the measured phase in the histogram (see row_v6).
 template <int L, bool MEAS>
 __device__ __forceinline__ void sweeps_v6(uint32_t* __restrict__ lat, uint32_t& S, uint32_t& chk, const uint32_t s0, const uint32_t s1,
-                                          const uint4* __restrict__ ring, int& buf, const int bar_id) {
+                                          const uint4* ring, int& buf, const int bar_id) {
     using G = Geo<L>;
     using V = V6<L>;
     constexpr int BITS = G::BITS, NC = V::NC, SLOTS = V::SLOTS;
@@ -266,7 +278,7 @@ __device__ __forceinline__ void sweeps_v6(uint32_t* __restrict__ lat, uint32_t& 
 // the double-buffered shared ring rnd[buf][call][slot] as one 16-byte store per call.  One barrier per row hands
 // the buffer over.  R4: ctr = (i >> 2, sweep, iteration, walker).
 template <int L>
-__device__ __forceinline__ void deviates_v6(uint4* __restrict__ ring, const uint32_t s0, const uint32_t s1, int& buf,
+__device__ __forceinline__ void deviates_v6(uint4* ring, const uint32_t s0, const uint32_t s1, int& buf,
                                             const int bar_id, const SweepParams& prm, const uint32_t walker, const bool active) {
     constexpr int NC = V6<L>::NC, SLOTS = V6<L>::SLOTS;
 #pragma unroll 1
