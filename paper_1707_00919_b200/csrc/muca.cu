@@ -584,7 +584,7 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
         CU(cudaMemcpyAsync(ctx->h_flag, ctx->d_flag, 3 * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
         CU(cudaStreamSynchronize(ctx->stream));
         const int lo = ctx->h_flag[1], hi = ctx->h_flag[2];
-        const size_t ring = plan.mode == MODE_WPAIR ? wpair_ring_bytes(plan.tpb / 32) : plan.mode == MODE_S6 ? s6_ring_bytes(plan.tpb / 32) + 32 : 0;
+        const size_t ring = plan.mode == MODE_WPAIR ? wpair_ring_bytes(plan.tpb / 32) : plan.mode == MODE_S6 ? s6_ring_bytes(plan.tpb / 32) + S6_RING_OFF : 0;
         int cap = plan.mode == MODE_S6 ? (int)(((size_t)max_smem - ring) / S6_RS) - 2 * S6_PAD_ROWS
                                        : (int)(((size_t)max_smem - 1024 - ring) / (ROW_SMEM_WORDS * 4)) - 2 * WINDOW_PAD_ROWS;
         if (ctx->opt_window_rows > 0 && ctx->opt_window_rows < cap) cap = ctx->opt_window_rows;

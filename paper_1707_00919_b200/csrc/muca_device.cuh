@@ -560,6 +560,80 @@ __device__ __forceinline__ void philox_round(uint32_t (&c)[4], const uint32_t k0
     c[2] = n2;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Philox4x32-10 for the deviate warps, with everything that does not depend on the walker taken out of the lanes.
+// R4: ctr = (c0 = i >> 2, sweep, iteration, walker): only ctr.w differs between the lanes of a warp, so round 0 needs no
+// per-lane multiply at all, rounds 1 and 2 need one each, rounds 3 .. 9 two each: 16 of the 20 wide multiplies of a call
+// (nvcc, left to itself, keeps 18 in the lanes).  The four others give values that are the same for all walkers:
+//   per kernel : (hi1, lo1) = M1 * iteration;                 Y2 = lo1 ^ K0[1]
+//   per sweep  : (hi_s, lo_s) = M0 * (hi1 ^ sweep ^ K0[0]);   W3 = lo_s ^ K1[2]
+//   per call   : (hi0, lo0) = M0 * c0,  (hi3, lo3) = M1 * (hi_s ^ lo0 ^ K1[1]):
+//                U1 = hi0 ^ K1[0],  X3 = hi3 ^ K0[2],  L3k = lo3 ^ K0[3]
+// (K0[r], K1[r]: the round keys key + r * Weyl constant).  The per-call values of the NC calls of a unit are computed by
+// the lanes 0 .. NC-1 of the deviate warp (lane q: call q) into a warp-private scratch of 16 bytes per call and read back
+// by all lanes with one broadcast load per call.
+// ------------------------------------------------------------------------------------------------
+struct PhiloxSweep { uint32_t hi_s, W3, Y2, k0, k1; };   // per-sweep / per-kernel values and the key
+
+__device__ __forceinline__ PhiloxSweep philox_sweep_consts(const uint32_t sweep, const uint32_t iteration, const uint32_t k0, const uint32_t k1) {
+    const uint64_t p1 = (uint64_t)0xCD9E8D57u * iteration;
+    const uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+    const uint64_t ps = (uint64_t)0xD2511F53u * (hi1 ^ sweep ^ k0);
+    PhiloxSweep c;
+    c.hi_s = (uint32_t)(ps >> 32);
+    c.W3 = (uint32_t)ps ^ (k1 + 2u * 0xBB67AE85u);
+    c.Y2 = lo1 ^ (k0 + 0x9E3779B9u);
+    c.k0 = k0; c.k1 = k1;
+    return c;
+}
+// lane q < ncalls: the walker-independent values of call c0_base + q -> scratch[q]
+__device__ __forceinline__ void philox_call_consts(uint4* scratch, const int ncalls, const uint32_t c0_base, const PhiloxSweep& c, const int lane) {
+    if (lane < ncalls) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * (c0_base + (uint32_t)lane);
+        const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+        const uint64_t p3 = (uint64_t)0xCD9E8D57u * (c.hi_s ^ lo0 ^ (c.k1 + 0xBB67AE85u));
+        scratch[lane] = make_uint4(hi0 ^ c.k1, (uint32_t)(p3 >> 32) ^ (c.k0 + 2u * 0x9E3779B9u), (uint32_t)p3 ^ (c.k0 + 3u * 0x9E3779B9u), 0u);
+    }
+    __syncwarp();
+}
+// rounds 0 .. 2 of one call for this lane's walker, from the values above; the state is ready for round 3
+__device__ __forceinline__ void philox_head(uint32_t (&st)[4], const uint4 u, const PhiloxSweep& c, const uint32_t walker) {
+    const uint32_t c2 = u.x ^ walker;                                   // round 0: c2 = hi0 ^ walker ^ K1[0]
+    const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;                     // round 1: the only per-lane product
+    const uint32_t c0 = (uint32_t)(p1 >> 32) ^ c.Y2, c1 = (uint32_t)p1;
+    const uint64_t p0 = (uint64_t)0xD2511F53u * c0;                     // round 2: the only per-lane product
+    st[0] = u.y ^ c1;                                                   // hi3 ^ c1 ^ K0[2]
+    st[1] = u.z;                                                        // lo3 ^ K0[3]: round 3 uses it as (c1 ^ K0[3])
+    st[2] = (uint32_t)(p0 >> 32) ^ c.W3;                                // hi(p0) ^ lo_s ^ K1[2]
+    st[3] = (uint32_t)p0;
+}
+// round 3: as philox_round, with c1 ^ K0[3] already folded into st[1]
+__device__ __forceinline__ void philox_round3(uint32_t (&st)[4], const uint32_t k1_3) {
+    const uint64_t p0 = (uint64_t)0xD2511F53u * st[0];
+    const uint64_t p1 = (uint64_t)0xCD9E8D57u * st[2];
+    const uint32_t n0 = (uint32_t)(p1 >> 32) ^ st[1];
+    const uint32_t n2 = (uint32_t)(p0 >> 32) ^ st[3] ^ k1_3;
+    st[1] = (uint32_t)p1;
+    st[3] = (uint32_t)p0;
+    st[0] = n0;
+    st[2] = n2;
+}
+// the NC calls c0_base .. c0_base + NC - 1 of one unit, round-major (NC independent multiply chains)
+template <int NC>
+__device__ __forceinline__ void philox_unit(uint32_t (&st)[NC][4], uint4* scratch, const uint32_t c0_base, const PhiloxSweep& c,
+                                            const uint32_t walker, const int lane) {
+    philox_call_consts(scratch, NC, c0_base, c, lane);
+#pragma unroll
+    for (int q = 0; q < NC; ++q) philox_head(st[q], scratch[q], c, walker);
+    __syncwarp();   // the scratch may be rewritten for the next unit
+#pragma unroll
+    for (int q = 0; q < NC; ++q) philox_round3(st[q], c.k1 + 3u * 0xBB67AE85u);
+#pragma unroll
+    for (int r = 4; r < 10; ++r)
+#pragma unroll
+        for (int q = 0; q < NC; ++q) philox_round(st[q], c.k0 + (uint32_t)r * 0x9E3779B9u, c.k1 + (uint32_t)r * 0xBB67AE85u);
+}
+
 __device__ __forceinline__ void pair_barrier(const int id) {   // named barrier of one walker warp + its deviate warp
     asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory");
 }

@@ -41,7 +41,8 @@ struct V6 {
     static constexpr int NC = Geo<L>::BITS / 4;              // Philox calls per row
     static constexpr uint32_t RING_OFF = LAT_OFF + (uint32_t)L * 4u * SLOTS;
     static constexpr uint32_t RING_BYTES = 2u * NC * 16u * SLOTS;
-    static constexpr size_t SMEM_BYTES = (size_t)RING_OFF + RING_BYTES;
+    static constexpr uint32_t SCRATCH_OFF = RING_OFF + RING_BYTES;          // 16 bytes per call and deviate warp (philox_unit)
+    static constexpr size_t SMEM_BYTES = (size_t)SCRATCH_OFF + 16u * NC * MAX_WARPS;
 };
 
 // Field words of a row: nibble q of FW[r] holds the column f = hl + 2*n3 of site 4q + r (hl: bond to the left
@@ -274,27 +275,21 @@ __device__ __forceinline__ void sweeps_v6(uint32_t* __restrict__ lat, uint32_t& 
     }
 }
 
-// Deviate warp: the NC Philox calls of one row advance round-major (NC independent IMAD.WIDE chains), results go to
-// the double-buffered shared ring rnd[buf][call][slot] as one 16-byte store per call.  One barrier per row hands
-// the buffer over.  R4: ctr = (i >> 2, sweep, iteration, walker).
+// Deviate warp: the NC Philox calls of one row advance round-major (NC independent IMAD.WIDE chains, philox_unit), results
+// go to the double-buffered shared ring rnd[buf][call][slot] as one 16-byte store per call (lanes without a walker
+// store nothing: their slots hold 0xFFFFFFFF for good).  One barrier per row hands the buffer over.
+// R4: ctr = (i >> 2, sweep, iteration, walker).
 template <int L>
-__device__ __forceinline__ void deviates_v6(uint4* ring, const uint32_t s0, const uint32_t s1, int& buf,
-                                            const int bar_id, const SweepParams& prm, const uint32_t walker, const bool active) {
+__device__ __forceinline__ void deviates_v6(uint4* ring, uint4* scratch, const uint32_t s0, const uint32_t s1, int& buf,
+                                            const int bar_id, const SweepParams& prm, const uint32_t walker, const bool active, const int lane) {
     constexpr int NC = V6<L>::NC, SLOTS = V6<L>::SLOTS;
 #pragma unroll 1
     for (uint32_t s = s0; s < s1; ++s) {
+        const PhiloxSweep pc = philox_sweep_consts(s, prm.iteration, prm.key0, prm.key1);
 #pragma unroll 1
         for (int y = 0; y < L; ++y) {
             uint32_t st[NC][4];
-#pragma unroll
-            for (int k = 0; k < NC; ++k) {
-                st[k][0] = (uint32_t)(y * (L / 4) + k); st[k][1] = s; st[k][2] = prm.iteration; st[k][3] = walker;
-            }
-#pragma unroll
-            for (int r = 0; r < 10; ++r)
-#pragma unroll
-                for (int k = 0; k < NC; ++k)
-                    philox_round(st[k], prm.key0 + (uint32_t)r * 0x9E3779B9u, prm.key1 + (uint32_t)r * 0xBB67AE85u);
+            philox_unit<NC>(st, scratch, (uint32_t)(y * (L / 4)), pc, walker, lane);
 #pragma unroll
             for (int k = 0; k < NC; ++k)
                 if (active) ring[(buf * NC + k) * SLOTS] = make_uint4(st[k][0], st[k][1], st[k][2], st[k][3]);
@@ -348,6 +343,7 @@ __global__ void __launch_bounds__(64 * V6<L>::MAX_WARPS, 1) sweep_kernel_v6(cons
     const int bar_id = 1 + pair;
     uint32_t* const lat = reinterpret_cast<uint32_t*>(sm + V::LAT_OFF) + slot;
     uint4* const ring = reinterpret_cast<uint4*>(sm + V::RING_OFF);
+    uint4* const scratch = reinterpret_cast<uint4*>(sm + V::SCRATCH_OFF) + pair * V::NC;
     // a lane without a walker never accepts: its ring slots hold the deviate 0xFFFFFFFF for good (the deviate warp
     // stores only for lanes with a walker) and its row has all thresholds 0
     if (!is_walker && !active)
@@ -379,7 +375,7 @@ __global__ void __launch_bounds__(64 * V6<L>::MAX_WARPS, 1) sweep_kernel_v6(cons
     uint32_t chk = 0;
     // ---- thermalisation sweeps: nothing is recorded
     if (is_walker) sweeps_v6<L, false>(lat, S, chk, prm.sweep_begin, s_th, ring + slot, buf, bar_id);
-    else deviates_v6<L>(ring + slot, prm.sweep_begin, s_th, buf, bar_id, prm, walker, active);
+    else deviates_v6<L>(ring + slot, scratch, prm.sweep_begin, s_th, buf, bar_id, prm, walker, active, lane);
     // ---- measured sweeps: every site counts the state it starts from, so the state before the first measured
     //      attempt is taken out again here and the state after the last one is added below
     if (is_walker) {
@@ -387,7 +383,7 @@ __global__ void __launch_bounds__(64 * V6<L>::MAX_WARPS, 1) sweep_kernel_v6(cons
         sweeps_v6<L, true>(lat, S, chk, s_th, prm.sweep_end, ring + slot, buf, bar_id);
         if (s_th < prm.sweep_end) atomicAdd(reinterpret_cast<uint32_t*>(sm + (S - sbase) + V::BIN_OFF), 1u);
     } else {
-        deviates_v6<L>(ring + slot, s_th, prm.sweep_end, buf, bar_id, prm, walker, active);
+        deviates_v6<L>(ring + slot, scratch, s_th, prm.sweep_end, buf, bar_id, prm, walker, active, lane);
     }
     if (is_walker) {
         if (chk == 0x9E3779B9u && !active) lat[0] = chk;   // keeps the checksum of the site macro alive (never true for a parked lane: its addresses are constant)

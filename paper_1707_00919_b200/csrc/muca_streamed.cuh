@@ -5,7 +5,7 @@
 // the shadow of the table loads.  A "unit" is one 32-site word of a row (L / 32 words per row).
 // Citations: "PAPER.md:<line>" = /root/reference/PAPER.md, "R<n>" = DESIGN.md section 3.
 //
-// Shared memory: DT[8] | deviate ring (8 KB per pair) | threshold table, rows of 36 bytes (t[8] | bin).  The table
+// Shared memory: DT[8] | Philox scratch (1 KB) | deviate ring (8 KB per pair) | threshold table, rows of 36 bytes (t[8] | bin).  The table
 // holds rows [j_lo, j_lo + n_rows) of the N + 1 slots: all of them at L <= 64 (4097 rows = 147 KB), a WINDOW around the
 // walkers' energies at L = 128 (16385 rows do not fit).  A walker may leave the window during the iteration.  That
 // cannot be excluded beforehand, so it is DETECTED and the host repeats the iteration with the L1 kernel from a
@@ -27,8 +27,10 @@ constexpr uint32_t S6_SBASE = 1024;   // dynamic shared memory starts behind the
 constexpr uint32_t S6_DTA = S6_SBASE; // the delta table sits first: the site macro addresses it by an immediate
 
 __host__ __device__ constexpr size_t s6_ring_bytes(int npairs) { return (size_t)npairs * 2 * 8 * 32 * 16; }
+constexpr uint32_t S6_SCRATCH_OFF = 32, S6_SCRATCH_BYTES = 8 * 8 * 16;   // behind DT: 16 bytes per call and deviate warp (philox_unit)
+constexpr uint32_t S6_RING_OFF = S6_SCRATCH_OFF + S6_SCRATCH_BYTES;
 __host__ __device__ constexpr size_t s6_smem_bytes(int n_rows, int npairs) {
-    return 32 + s6_ring_bytes(npairs) + (size_t)(n_rows + 2 * S6_PAD_ROWS) * S6_RS;
+    return S6_RING_OFF + s6_ring_bytes(npairs) + (size_t)(n_rows + 2 * S6_PAD_ROWS) * S6_RS;
 }
 
 // Walker warp: sweeps s0 .. s1-1 over the streamed rows of one walker.
@@ -112,27 +114,20 @@ __device__ __forceinline__ void sweeps_s6(uint32_t* __restrict__ rows, const siz
     }
 }
 
-// Deviate warp: the 8 Philox calls of a 32-site word advance round-major, results go to the double-buffered ring
-// rnd[buf][call][slot] as one 16-byte store per call (lanes without a walker store nothing: their slots hold
+// Deviate warp: the 8 Philox calls of a 32-site word advance round-major (philox_unit), results go to the double-buffered
+// ring rnd[buf][call][slot] as one 16-byte store per call (lanes without a walker store nothing: their slots hold
 // 0xFFFFFFFF for good).  One barrier per word hands the buffer over.  R4: ctr = (i >> 2, sweep, iteration, walker).
 template <int L>
-__device__ __forceinline__ void deviates_s6(uint4* ring, const int slots, int& buf, const int bar_id, const uint32_t s0,
-                                            const uint32_t s1, const SweepParams& prm, const uint32_t walker, const bool active) {
+__device__ __forceinline__ void deviates_s6(uint4* ring, uint4* scratch, const int slots, int& buf, const int bar_id, const uint32_t s0,
+                                            const uint32_t s1, const SweepParams& prm, const uint32_t walker, const bool active, const int lane) {
     constexpr int WPR = Geo<L>::WPR;
 #pragma unroll 1
     for (uint32_t s = s0; s < s1; ++s) {
+        const PhiloxSweep pc = philox_sweep_consts(s, prm.iteration, prm.key0, prm.key1);
 #pragma unroll 1
         for (int word = 0; word < L * WPR; ++word) {      // typewriter word: sites 32 word .. 32 word + 31, calls 8 word .. + 7
             uint32_t st[8][4];
-#pragma unroll
-            for (int q = 0; q < 8; ++q) {
-                st[q][0] = (uint32_t)(word * 8 + q); st[q][1] = s; st[q][2] = prm.iteration; st[q][3] = walker;
-            }
-#pragma unroll
-            for (int r = 0; r < 10; ++r)
-#pragma unroll
-                for (int q = 0; q < 8; ++q)
-                    philox_round(st[q], prm.key0 + (uint32_t)r * 0x9E3779B9u, prm.key1 + (uint32_t)r * 0xBB67AE85u);
+            philox_unit<8>(st, scratch, (uint32_t)(word * 8), pc, walker, lane);
 #pragma unroll
             for (int q = 0; q < 8; ++q)
                 if (active) ring[(buf * 8 + q) * slots] = make_uint4(st[q][0], st[q][1], st[q][2], st[q][3]);
@@ -163,8 +158,9 @@ sweep_kernel_s6(const SweepParams prm, const int j_lo, const int n_rows, const i
     const int w = blockIdx.x * slots + slot;
     const bool active = w < prm.W;
     if ((uint32_t)__cvta_generic_to_shared(smem) != S6_SBASE) __trap();   // the site macro addresses the delta table by an immediate
-    uint4* const ring = reinterpret_cast<uint4*>(sm + 32) + slot;
-    char* const win = sm + 32 + s6_ring_bytes(npairs);
+    uint4* const ring = reinterpret_cast<uint4*>(sm + S6_RING_OFF) + slot;
+    uint4* const scratch = reinterpret_cast<uint4*>(sm + S6_SCRATCH_OFF) + pair * 8;
+    char* const win = sm + S6_RING_OFF + s6_ring_bytes(npairs);
     char* const tbl = win + S6_PAD_ROWS * S6_RS;                        // row 0 of the window
     // ---- table window: row jl = t[8] | bin; pad and sentinel rows: all thresholds 0
     for (int idx = tid; idx < (n_rows + 2 * S6_PAD_ROWS) * 9; idx += nthr) {
@@ -184,7 +180,7 @@ sweep_kernel_s6(const SweepParams prm, const int j_lo, const int n_rows, const i
         for (int q = 0; q < 16; ++q) ring[q * slots] = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
     __syncthreads();
 
-    const uint32_t o_base = S6_SBASE + 32u + (uint32_t)s6_ring_bytes(npairs) + S6_PAD_ROWS * S6_RS;   // address of window row 0
+    const uint32_t o_base = S6_SBASE + S6_RING_OFF + (uint32_t)s6_ring_bytes(npairs) + S6_PAD_ROWS * S6_RS;   // address of window row 0
     const uint32_t win_lo = o_base + (uint32_t)sent_lo * S6_RS, win_span = (uint32_t)(n_rows - sent_lo - sent_hi) * S6_RS;
     const uint32_t s_th = prm.therm < prm.sweep_begin ? prm.sweep_begin
                           : (prm.therm > prm.sweep_end ? prm.sweep_end : prm.therm);
@@ -213,8 +209,8 @@ sweep_kernel_s6(const SweepParams prm, const int j_lo, const int n_rows, const i
             if (left) atomicOr(overflow, 1);
         }
     } else {
-        deviates_s6<L>(ring, slots, buf, bar_id, prm.sweep_begin, s_th, prm, walker, active);
-        deviates_s6<L>(ring, slots, buf, bar_id, s_th, prm.sweep_end, prm, walker, active);
+        deviates_s6<L>(ring, scratch, slots, buf, bar_id, prm.sweep_begin, s_th, prm, walker, active, lane);
+        deviates_s6<L>(ring, scratch, slots, buf, bar_id, s_th, prm.sweep_end, prm, walker, active, lane);
     }
     __syncthreads();
     // ---- a4: merge the bins of the real rows into the global uint64 histogram
