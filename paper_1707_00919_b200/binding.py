@@ -62,11 +62,10 @@ def lib():
         return _lib
     try:
         path = _build.build()
-    except Exception as e:  # no nvcc / compile error: fail loudly, never fall back
-        if os.path.exists(_build.LIB):
-            path = _build.LIB
-        else:
+    except _build.NvccMissing as e:   # no compiler here: a library built elsewhere is used as it is; a compile ERROR propagates
+        if not os.path.exists(_build.LIB):
             raise MucaError(f"libmuca_b200.so is not built and cannot be built here: {e}") from e
+        path = _build.LIB
     L = C.CDLL(path)
     vp, u32p, u64p = C.c_void_p, C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)
     f64p, i8p, i32p = C.POINTER(C.c_double), C.POINTER(C.c_int8), C.POINTER(C.c_int32)

@@ -11,12 +11,12 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SOURCES = [os.path.join(CSRC, "muca.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "muca_device.cuh"), os.path.join(CSRC, "muca_resident.cuh"), os.path.join(CSRC, "muca_random_site.cuh"), os.path.join(CSRC, "muca_window.cuh"),
-                  os.path.join(os.path.dirname(HERE), "include", "muca.h")]
+DEPS = SOURCES + sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith(".cuh")) + \
+    [os.path.join(os.path.dirname(HERE), "include", "muca.h")]
 LIB = os.path.join(HERE, "libmuca_b200.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
-              "--use_fast_math", "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
+              "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
 
 
 def nvcc() -> str:
@@ -32,11 +32,18 @@ def stale() -> bool:
     return any(os.path.getmtime(d) > t for d in DEPS)
 
 
+class NvccMissing(RuntimeError):
+    """No nvcc on this machine (the only case in which an existing library may be used as it is)."""
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not stale():
         return LIB
     cmd = [nvcc()] + NVCC_FLAGS + ["-o", LIB + ".tmp"] + SOURCES
-    res = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
+    try:
+        res = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
+    except FileNotFoundError as e:
+        raise NvccMissing(str(e)) from e
     if verbose or res.returncode != 0:
         sys.stderr.write(res.stdout)
     if res.returncode != 0:

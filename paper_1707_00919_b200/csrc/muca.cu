@@ -8,7 +8,9 @@
 #include <cstdio>
 #include <cstring>
 #include <limits>
+#include <map>
 #include <mutex>
+#include <utility>
 #include <new>
 #include <vector>
 
@@ -57,7 +59,9 @@ struct muca_ctx {
     double conv_n_updates = 0.0;    // N_updates (flips per walker) of the previous iteration of muca_converge
     int opt_scheme = MUCA_SCHEME_TYPEWRITER;   // update scheme used by muca_converge / muca_production
     int conv_full = 0;              // the previous iteration already worked on the whole energy range
+    int device = 0;                 // CUDA device the context lives on: every entry point selects it (DeviceGuard)
     int n_sm = 0;
+    int max_smem_optin = 0;         // cudaDevAttrMaxSharedMemoryPerBlockOptin of that device
     char err[512] = {0};
 };
 
@@ -102,6 +106,38 @@ int fail(muca_ctx* c, int code, const char* fmt, ...) {
                         __FILE__, __LINE__);                                                         \
     } while (0)
 
+// Every entry point that touches the device runs with the context's device current and restores the caller's.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const muca_ctx* c) {
+        if (c && cudaGetDevice(&prev) == cudaSuccess && prev != c->device) switched = cudaSetDevice(c->device) == cudaSuccess;
+    }
+    ~DeviceGuard() {
+        if (switched) cudaSetDevice(prev);
+    }
+    DeviceGuard(const DeviceGuard&) = delete;
+    DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a property of (device, kernel): remembered per device, only ever raised.
+int ensure_dynamic_smem(muca_ctx* ctx, const void* kernel, size_t bytes) {
+    static std::mutex m;
+    static std::map<std::pair<int, const void*>, size_t> configured;
+    std::lock_guard<std::mutex> g(m);
+    size_t& have = configured[std::make_pair(ctx->device, kernel)];
+    if (bytes > have) {
+        CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+        have = bytes;
+    }
+    return MUCA_OK;
+}
+#define SMEM(kernel, bytes)                                                             \
+    do {                                                                                \
+        const int rc_ = ensure_dynamic_smem(ctx, (const void*)(kernel), (bytes));       \
+        if (rc_ != MUCA_OK) return rc_;                                                 \
+    } while (0)
+
 // Acceptance thresholds thresh[j][a], a = 0..4 (include/muca.h, muca_run_iteration step 1, R6/R7/R9).
 void build_thresholds5(const std::vector<double>& omega, std::vector<uint32_t>& t5) {
     const int bins = (int)omega.size();
@@ -137,11 +173,7 @@ void expand_table8(const std::vector<uint32_t>& t5, int bins, uint32_t* t8) {
 
 template <int L>
 int launch_sweep_v3(muca_ctx* ctx, const SweepParams& prm, int tpb) {
-    static bool configured = false;
-    if (!configured) {
-        CU(cudaFuncSetAttribute(sweep_kernel_v3<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V3<L>::SMEM_BYTES));
-        configured = true;
-    }
+    SMEM(sweep_kernel_v3<L>, V3<L>::SMEM_BYTES);
     const int grid = (prm.W + tpb - 1) / tpb;
     sweep_kernel_v3<L><<<grid, 2 * tpb, V3<L>::SMEM_BYTES, ctx->stream>>>(prm);   // tpb walker + tpb deviate threads
     CU(cudaGetLastError());
@@ -150,11 +182,7 @@ int launch_sweep_v3(muca_ctx* ctx, const SweepParams& prm, int tpb) {
 
 template <int L>
 int launch_sweep_v6(muca_ctx* ctx, const SweepParams& prm, int nw, int wpw) {
-    static bool configured = false;
-    if (!configured) {
-        CU(cudaFuncSetAttribute(sweep_kernel_v6<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V6<L>::SMEM_BYTES));
-        configured = true;
-    }
+    SMEM(sweep_kernel_v6<L>, V6<L>::SMEM_BYTES);
     const int per_block = nw * wpw;
     const int grid = (prm.W + per_block - 1) / per_block;
     sweep_kernel_v6<L><<<grid, 64 * nw, V6<L>::SMEM_BYTES, ctx->stream>>>(prm, wpw, ctx->opt_role_map);
@@ -165,11 +193,7 @@ int launch_sweep_v6(muca_ctx* ctx, const SweepParams& prm, int nw, int wpw) {
 template <int L, int MODE>
 int launch_sweep_t(muca_ctx* ctx, const SweepParams& prm, int tpb) {
     const size_t smem = sweep_smem_bytes<L, MODE>(tpb);
-    static size_t configured = 0;
-    if (smem > configured) {
-        CU(cudaFuncSetAttribute(sweep_kernel<L, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = smem;
-    }
+    SMEM((sweep_kernel<L, MODE>), smem);
     const int grid = (prm.W + tpb - 1) / tpb;
     sweep_kernel<L, MODE><<<grid, tpb, smem, ctx->stream>>>(prm);
     CU(cudaGetLastError());
@@ -254,11 +278,7 @@ struct Window { int j_lo = 0, n_rows = 0, sent_lo = 0, sent_hi = 0; };
 template <int L>
 int launch_window_t(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& win) {
     const size_t smem = window_smem_bytes(win.n_rows);
-    static size_t configured = 0;
-    if (smem > configured) {
-        CU(cudaFuncSetAttribute(sweep_kernel_window<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = smem;
-    }
+    SMEM((sweep_kernel_window<L>), smem);
     sweep_kernel_window<L><<<(prm.W + tpb - 1) / tpb, tpb, smem, ctx->stream>>>(prm, win.j_lo, win.n_rows, win.sent_lo,
                                                                                win.sent_hi, ctx->d_flag);
     CU(cudaGetLastError());
@@ -269,11 +289,7 @@ template <int L>
 int launch_wpair_t(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& win) {
     const int npairs = tpb / 32;
     const size_t smem = wpair_smem_bytes(win.n_rows, npairs);
-    static size_t configured = 0;
-    if (smem > configured) {
-        CU(cudaFuncSetAttribute(sweep_kernel_wpair<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = smem;
-    }
+    SMEM((sweep_kernel_wpair<L>), smem);
     sweep_kernel_wpair<L><<<(prm.W + tpb - 1) / tpb, 2 * tpb, smem, ctx->stream>>>(prm, win.j_lo, win.n_rows, win.sent_lo,
                                                                                   win.sent_hi, ctx->d_flag);
     CU(cudaGetLastError());
@@ -285,11 +301,7 @@ int launch_s6_t(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& wi
     const int npairs = tpb / 32;
     if (npairs < 1 || npairs > s6_max_pairs(L)) return fail(ctx, MUCA_EINVAL, "paired streamed kernel: 1 to %d warp pairs per block at L = %d", s6_max_pairs(L), L);
     const size_t smem = s6_smem_bytes(win.n_rows, npairs);
-    static size_t configured = 0;
-    if (smem > configured) {
-        CU(cudaFuncSetAttribute(sweep_kernel_s6<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = smem;
-    }
+    SMEM((sweep_kernel_s6<L>), smem);
     sweep_kernel_s6<L><<<(prm.W + tpb - 1) / tpb, 2 * tpb, smem, ctx->stream>>>(prm, win.j_lo, win.n_rows, win.sent_lo, win.sent_hi,
                                                                                ctx->opt_role_map, ctx->d_flag);
     CU(cudaGetLastError());
@@ -422,12 +434,11 @@ int create_common(muca_ctx** out, int L, int W, uint64_t seed, uint32_t walker_o
         cudaEventCreate(&ctx->ev0) != cudaSuccess || cudaEventCreate(&ctx->ev1) != cudaSuccess)
         return bail(MUCA_ECUDA);
     ctx->h_flag = reinterpret_cast<int*>(ctx->h_H + ctx->n_bins);
-    {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess ||
-            cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-            return bail(MUCA_ECUDA);
-    }
+    // the context lives on the device that is current at creation (the workspace and the stream are that device's)
+    if (cudaGetDevice(&ctx->device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, ctx->device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&ctx->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, ctx->device) != cudaSuccess)
+        return bail(MUCA_ECUDA);
     const int tpb = 128;
     init_kernel<<<(W + tpb - 1) / tpb, tpb, 0, ctx->stream>>>(ctx->d_spins, ctx->d_E, L, W, walker_offset,
                                                              (uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32));
@@ -443,11 +454,7 @@ namespace {
 template <int L>
 int launch_random_site(muca_ctx* ctx, const RandomSiteParams& prm, int tpb) {
     const size_t smem = random_site_smem_bytes<L>(tpb);
-    static size_t configured = 0;
-    if (smem > configured) {
-        CU(cudaFuncSetAttribute(random_site_kernel<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = smem;
-    }
+    SMEM((random_site_kernel<L>), smem);
     random_site_kernel<L><<<(prm.W + tpb - 1) / tpb, tpb, smem, ctx->stream>>>(prm);
     CU(cudaGetLastError());
     return MUCA_OK;
@@ -480,6 +487,7 @@ int muca_create_in(muca_ctx** out, int L, int n_walkers, uint64_t seed, uint32_t
 
 void muca_destroy(muca_ctx* ctx) {
     if (!ctx) return;
+    const DeviceGuard guard(ctx);
     if (ctx->stream || ctx->d_workspace) cudaStreamSynchronize(ctx->stream);
     pinned_pool().put(pinned_table_bytes(ctx->n_bins), ctx->h_table);
     pinned_pool().put(pinned_hist_bytes(ctx->n_bins), ctx->h_H);
@@ -549,16 +557,12 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
     if (n_bins != ctx->n_bins || therm_sweeps < 0 || sweeps < 0)
         return fail(ctx, MUCA_EINVAL, "run_iteration: n_bins must be %d, sweeps >= 0", ctx->n_bins);
     if (ctx->iteration == 0xFFFFFFFFu) return fail(ctx, MUCA_ERANGE, "iteration counter exhausted");
+    const DeviceGuard guard(ctx);
     Plan plan = make_plan(ctx);
-    int max_smem = 0;
-    {
-        int dev = 0;
-        CU(cudaGetDevice(&dev));
-        CU(cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
-        if (plan_smem(ctx->L, plan) > (size_t)max_smem)
-            return fail(ctx, MUCA_EINVAL, "kernel variant needs %zu B of shared memory per block, device allows %d",
-                        plan_smem(ctx->L, plan), max_smem);
-    }
+    const int max_smem = ctx->max_smem_optin;
+    if (plan_smem(ctx->L, plan) > (size_t)max_smem)
+        return fail(ctx, MUCA_EINVAL, "kernel variant needs %zu B of shared memory per block, device allows %d",
+                    plan_smem(ctx->L, plan), max_smem);
     // a1: thresholds from omega (host, double)
     std::vector<uint32_t> t5;
     build_thresholds5(ctx->logw, t5);
@@ -579,7 +583,7 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
         const size_t spin_bytes = (size_t)ctx->W * (ctx->N / 8);
         ctx->h_flag[0] = 0; ctx->h_flag[1] = 0x7FFFFFFF; ctx->h_flag[2] = -1;
         CU(cudaMemcpyAsync(ctx->d_flag, ctx->h_flag, 3 * sizeof(int), cudaMemcpyHostToDevice, ctx->stream));
-        slot_range_kernel<<<148, 256, 0, ctx->stream>>>(ctx->d_E, ctx->W, ctx->N, ctx->d_flag + 1);
+        slot_range_kernel<<<ctx->n_sm, 256, 0, ctx->stream>>>(ctx->d_E, ctx->W, ctx->N, ctx->d_flag + 1);
         CU(cudaGetLastError());
         CU(cudaMemcpyAsync(ctx->h_flag, ctx->d_flag, 3 * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
         CU(cudaStreamSynchronize(ctx->stream));
@@ -673,6 +677,7 @@ int muca_run_iteration_random_site(muca_ctx* ctx, uint64_t therm_updates, uint64
     if (n_bins != ctx->n_bins) return fail(ctx, MUCA_EINVAL, "run_iteration_random_site: n_bins must be %d", ctx->n_bins);
     if (ctx->iteration == 0xFFFFFFFFu) return fail(ctx, MUCA_ERANGE, "iteration counter exhausted");
     if (therm_updates > (1ull << 60) || updates > (1ull << 60)) return fail(ctx, MUCA_EINVAL, "too many updates");
+    const DeviceGuard guard(ctx);
     std::vector<uint32_t> t5;
     build_thresholds5(ctx->logw, t5);                                           // a1, as in muca_run_iteration
     expand_table8(t5, ctx->n_bins, ctx->h_table);
@@ -876,6 +881,7 @@ int muca_production(muca_ctx* ctx, int n_calls, int therm_sweeps, int sweeps, do
 int muca_get_energies(muca_ctx* ctx, int32_t* E_out, int n_walkers) {
     if (!ctx) return MUCA_EINVAL;
     if (!E_out || n_walkers != ctx->W) return fail(ctx, MUCA_EINVAL, "get_energies: n_walkers must be %d", ctx->W);
+    const DeviceGuard guard(ctx);
     CU(cudaMemcpyAsync(E_out, ctx->d_E, sizeof(int32_t) * (size_t)ctx->W, cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     return MUCA_OK;
@@ -884,6 +890,7 @@ int muca_get_energies(muca_ctx* ctx, int32_t* E_out, int n_walkers) {
 int muca_unpack_spins_device(muca_ctx* ctx, void* d_out, size_t n) {
     if (!ctx) return MUCA_EINVAL;
     if (!d_out || n != (size_t)ctx->W * ctx->N) return fail(ctx, MUCA_EINVAL, "unpack: n must be %zu", (size_t)ctx->W * ctx->N);
+    const DeviceGuard guard(ctx);
     if (((uintptr_t)d_out % 16) != 0) return fail(ctx, MUCA_EINVAL, "unpack: device buffer must be 16-byte aligned");
     const size_t threads = (size_t)ctx->W * (ctx->N / 32);
     const int tpb = 256;
@@ -895,6 +902,7 @@ int muca_unpack_spins_device(muca_ctx* ctx, void* d_out, size_t n) {
 int muca_get_spins(muca_ctx* ctx, int8_t* out, size_t n) {
     if (!ctx) return MUCA_EINVAL;
     if (!out || n != (size_t)ctx->W * ctx->N) return fail(ctx, MUCA_EINVAL, "get_spins: n must be %zu", (size_t)ctx->W * ctx->N);
+    const DeviceGuard guard(ctx);
     int rc = muca_unpack_spins_device(ctx, ctx->d_stage, n);
     if (rc == MUCA_OK) {
         cudaError_t e = cudaMemcpyAsync(out, ctx->d_stage, n, cudaMemcpyDeviceToHost, ctx->stream);
@@ -907,6 +915,7 @@ int muca_get_spins(muca_ctx* ctx, int8_t* out, size_t n) {
 int muca_set_spins(muca_ctx* ctx, const int8_t* spins, size_t n) {
     if (!ctx) return MUCA_EINVAL;
     if (!spins || n != (size_t)ctx->W * ctx->N) return fail(ctx, MUCA_EINVAL, "set_spins: n must be %zu", (size_t)ctx->W * ctx->N);
+    const DeviceGuard guard(ctx);
     void* d_tmp = ctx->d_stage;
     int rc = MUCA_OK;
     cudaError_t e = cudaMemcpyAsync(d_tmp, spins, n, cudaMemcpyHostToDevice, ctx->stream);
