@@ -1,6 +1,7 @@
 // paper_1707_00919_b200/csrc/muca_resident.cuh
 // Resident sweep kernel v6 for L <= 32 (sm_100a): "state in the address", two-candidate select, walker warps paired
-// with deviate warps, everything that is not the per-site chain spread over the sites of the previous row.
+// with deviate warps, everything that is not the per-site chain spread over the sites of the previous row; the site
+// macro in its PIPELINED form (the table load of the next site closes the macro, round 2).
 // Citations: "PAPER.md:<line>" = /root/reference/PAPER.md, "R<n>" = DESIGN.md section 3.
 //
 // The walker's dynamic state is the shared-memory address S = rowaddr(j) of its energy slot j.  Row j is 36 bytes (9
@@ -96,6 +97,16 @@ __device__ __forceinline__ void prep_steps(NextRow<L>& n) {
         prep_steps<L, I0 + 1, I1>(n);
     }
 }
+// the value written by preparation step I (scheduling dependency of the pipelined site macro)
+template <int L, int I>
+__device__ __forceinline__ uint32_t prep_last(const NextRow<L>& n) {
+    if constexpr (I == 0) return n.hr;
+    else if constexpr (I == 1) return n.hl;
+    else if constexpr (I == 2) return n.m0;
+    else if constexpr (I == 3) return n.m1;
+    else if constexpr (I < 16) return ((I - 4) % 3 == 2) ? n.P[(I - 4) / 3] : n.t;
+    else return n.patch;
+}
 // FW[r] of the row below `above_new` (bits 4q + r of above_new must be final)
 template <int L>
 __device__ __forceinline__ uint32_t finish_word(const NextRow<L>& n, const uint32_t above_new, const int r) {
@@ -141,13 +152,72 @@ __device__ __forceinline__ uint32_t finish_word(const NextRow<L>& n, const uint3
 #define MUCA_V6_GX_ROWSTART "mov.u32 gx2, g2;\n\t"                  /* site 0 of a row: its left neighbour has not been visited in this sweep */
 #define MUCA_V6_PATCH "@p add.u32 %3, %3, %13;\n\t"
 
+// The PIPELINED form of the site (resident kernel; profiles/README.md, round 2).  Threshold t and delta d of THIS site
+// were loaded by the previous macro (operands %8, %9); this one decides, selects and at once issues the loads of the
+// NEXT site, directly behind the two selects:
+//     ISETP -> SEL A' -> LDS t'         is all that is left between two table loads of the chain.
+// In the form above the new state was "selp S, S + d, S", which ptxas turns into an add predicated on the decision; a
+// predicate is consumed by a predicated instruction ~13 cycles after its ISETP, the warp issues in order, and the
+// next table load sat behind it.  Here S' = A' - off' (both selected, no predicate), H[j]++ counts the state after
+// the attempt where it is known, and the column extraction is a funnel shift whose other half (%16, shifted out of
+// the bits kept by the mask) is the last value written by the preparation steps scheduled at this site: without
+// that dependency ptxas sinks the ~35 preparation instructions of a row to its end, where no table load hides them.
+//   %0 S  %1 A  %2 flips  %3 FW[3] (site 0)  %4 checksum  %5 off  %6 g1  %7 gx1  %8 t  %9 d       (all in/out)
+//   %10 deviate  %11 field word of the site after the next  %12 its shift  %13 flip mask  %14 the constant 4
+//   %15 patch  %16 scheduling dependency  %17 address of DT[0]
+#define MUCA_V6P_SITE(SHIFT_LINE, HIST_LINE, GX_LINE, EXTRA_LINE)                \
+    "{\n\t.reg .pred p;\n\t.reg .b32 gs, g2, gx2, ar, aa, sg;\n\t"               \
+    SHIFT_LINE                                                                   \
+    "add.u32 ar, %0, %6;\n\t"                                                    \
+    "add.u32 sg, %0, %7;\n\t"                                                    \
+    "and.b32 g2, gs, 0x1C;\n\t" GX_LINE                                          \
+    "add.u32 aa, sg, %9;\n\t"                                                    \
+    "mad.lo.u32 %4, aa, ar, %4;\n\t"                                             \
+    "setp.le.u32 p, %10, %8;\n\t"                                                \
+    "selp.u32 %1, aa, ar, p;\n\t"                                                \
+    "selp.u32 %5, %7, %6, p;\n\t"                                                \
+    "ld.volatile.shared.u32 %8, [%1];\n\t"                                       \
+    "ld.volatile.shared.u32 %9, [%5+%17];\n\t"                                   \
+    "sub.u32 %0, %1, %5;\n\t"                                                    \
+    HIST_LINE                                                                    \
+    "@p or.b32 %2, %2, %13;\n\t" EXTRA_LINE                                      \
+    "mov.u32 %6, g2;\n\tmov.u32 %7, gx2;\n\t}"
+#define MUCA_V6P_SHL "shf.l.clamp.b32 gs, %16, %11, %12;\n\t"       /* (fw << s) | (dep >> (32 - s)): s = 2, the mask keeps bits 2..4 */
+#define MUCA_V6P_SHR "shf.r.clamp.b32 gs, %11, %16, %12;\n\t"       /* (fw >> s) | (dep << (32 - s)): s <= 26 */
+#define MUCA_V6P_GX_CARRY "lop3.b32 gx2, gs, 0x1C, %14, 0x6A;\n\t"
+#define MUCA_V6P_PATCH "@p add.u32 %3, %3, %15;\n\t"
+
+// threshold and delta of the next site (pipelined form) and the scheduling dependency of its macro
+struct SitePipe { uint32_t t, d, dep; };
+
 enum { SITE_FIRST = 0, SITE_SHL = 1, SITE_SHR = 2, SITE_ROWSTART = 3 };   // flavour of the site macro
 
-template <int L, bool MEAS, int FLAVOUR, uint32_t DTA>
+template <int L, bool MEAS, int FLAVOUR, uint32_t DTA, bool PIPE>
 __device__ __forceinline__ void site_v6(uint32_t& S, uint32_t& A, uint32_t& flips, uint32_t& fw3, uint32_t& chk, uint32_t& off,
                                         uint32_t& g1, uint32_t& gx1, const uint32_t rnd, const uint32_t fw2, const uint32_t sh2,
-                                        const uint32_t mask, const uint32_t patch) {
+                                        const uint32_t mask, const uint32_t patch, SitePipe& pp) {
     uint32_t unused = 0;   // fills operand %3 of the site macro where site 0 has FW[3]
+    if constexpr (PIPE) {
+#define MUCA_V6P_ASM(SHIFT, HIST, GX, EXTRA, FW3)                                                                      \
+    asm volatile(MUCA_V6P_SITE(SHIFT, HIST, GX, EXTRA)                                                                 \
+                 : "+r"(S), "+r"(A), "+r"(flips), "+r"(FW3), "+r"(chk), "+r"(off), "+r"(g1), "+r"(gx1), "+r"(pp.t), "+r"(pp.d) \
+                 : "r"(rnd), "r"(fw2), "r"(sh2), "r"(mask), "r"(4u), "r"(patch), "r"(pp.dep), "n"(DTA) : "memory")
+        if constexpr (FLAVOUR == SITE_FIRST) {
+            if constexpr (MEAS) MUCA_V6P_ASM(MUCA_V6P_SHL, MUCA_V6_HIST, MUCA_V6P_GX_CARRY, MUCA_V6P_PATCH, fw3);
+            else MUCA_V6P_ASM(MUCA_V6P_SHL, "", MUCA_V6P_GX_CARRY, MUCA_V6P_PATCH, fw3);
+        } else if constexpr (FLAVOUR == SITE_SHL) {
+            if constexpr (MEAS) MUCA_V6P_ASM(MUCA_V6P_SHL, MUCA_V6_HIST, MUCA_V6P_GX_CARRY, "", unused);
+            else MUCA_V6P_ASM(MUCA_V6P_SHL, "", MUCA_V6P_GX_CARRY, "", unused);
+        } else if constexpr (FLAVOUR == SITE_SHR) {
+            if constexpr (MEAS) MUCA_V6P_ASM(MUCA_V6P_SHR, MUCA_V6_HIST, MUCA_V6P_GX_CARRY, "", unused);
+            else MUCA_V6P_ASM(MUCA_V6P_SHR, "", MUCA_V6P_GX_CARRY, "", unused);
+        } else {
+            if constexpr (MEAS) MUCA_V6P_ASM(MUCA_V6P_SHL, MUCA_V6_HIST, MUCA_V6_GX_ROWSTART, "", unused);
+            else MUCA_V6P_ASM(MUCA_V6P_SHL, "", MUCA_V6_GX_ROWSTART, "", unused);
+        }
+#undef MUCA_V6P_ASM
+        return;
+    }
 #define MUCA_V6_ASM(SHIFT_OP, HIST, GX, EXTRA, FW3)                                                                    \
     asm volatile(MUCA_V6_SITE(SHIFT_OP, HIST, GX, EXTRA)                                                               \
                  : "+r"(S), "+r"(A), "+r"(flips), "+r"(FW3), "+r"(chk), "+r"(off), "+r"(g1), "+r"(gx1)                 \
@@ -176,35 +246,45 @@ __device__ __forceinline__ void site_v6(uint32_t& S, uint32_t& A, uint32_t& flip
 // next unit in typewriter order (the columns of its sites 0 and 1 are extracted at the end of this unit); (n, FWp):
 // the unit one lattice row below, prepared here.  DTA: address of the delta table; stride: uint4 elements between two
 // calls in the ring.
-template <int L, bool MEAS, int X, bool FIRST, bool LASTW, uint32_t DTA>
+template <int L, bool MEAS, int X, bool FIRST, bool LASTW, uint32_t DTA, bool PIPE>
 struct RowSites {
     static __device__ __forceinline__ void run(uint32_t& S, uint32_t& A, uint32_t& flips, uint32_t& chk, uint32_t& off, uint32_t& g1,
                                                uint32_t& gx1, const uint32_t c, uint32_t (&FW)[4], uint32_t& fw3t, const uint32_t patch,
                                                uint32_t (&rnd)[Geo<L>::BITS], NextRow<L>& n, uint32_t (&FWp)[4],
                                                const uint32_t (&FWseq)[4], const uint4* ring, const int stride,
-                                               const int buf, const bool more) {
+                                               const int buf, const bool more, SitePipe& pp) {
         constexpr int BITS = Geo<L>::BITS, NC = BITS / 4;
         constexpr int X2 = X + 2;                              // the site whose column is extracted now
         constexpr bool below = X2 >= BITS;                     // it belongs to the next unit
         constexpr int q2 = below ? 0 : X2 >> 2;
         constexpr uint32_t sh2 = q2 == 0 ? 2u : (uint32_t)(4 * q2 - 2);   // nibble q2 of the field word -> bits 2..4
         constexpr int FLAVOUR = (X == 0 && FIRST) ? SITE_FIRST : ((X2 == BITS && LASTW) ? SITE_ROWSTART : (q2 == 0 ? SITE_SHL : SITE_SHR));
-        site_v6<L, MEAS, FLAVOUR, DTA>(S, A, flips, fw3t, chk, off, g1, gx1, rnd[X], below ? FWseq[X2 - BITS] : FW[X2 & 3], sh2,
-                                       1u << X, patch);
+        site_v6<L, MEAS, FLAVOUR, DTA, PIPE>(S, A, flips, fw3t, chk, off, g1, gx1, rnd[X], below ? FWseq[X2 - BITS] : FW[X2 & 3], sh2,
+                                             1u << X, patch, pp);
         // ---- off the chain, in the shadow of the table loads: prepare the unit below
         constexpr int D = BITS - 4;
-        if constexpr (X < D) prep_steps<L, (X * PREP_STEPS) / D, ((X + 1) * PREP_STEPS) / D>(n);
+        if constexpr (X < D) {
+            constexpr int I0 = (X * PREP_STEPS) / D, I1 = ((X + 1) * PREP_STEPS) / D;
+            prep_steps<L, I0, I1>(n);
+            if constexpr (PIPE && I1 > I0) pp.dep = prep_last<L, I1 - 1>(n);   // pins these steps in front of the next site
+        }
         if constexpr (X >= BITS - 4 && X < BITS - 1) FWp[X - (BITS - 4)] = finish_word<L>(n, c ^ flips, X - (BITS - 4));
         if constexpr ((X & 3) == 3) {
             if (more) {   // the deviates of sites 4k .. 4k + 3 are spent: fetch call k of the next unit into their place
                 constexpr int k = X >> 2;
-                const uint4 v = ring[(buf * NC + k) * stride];
-                rnd[4 * k] = v.x; rnd[4 * k + 1] = v.y; rnd[4 * k + 2] = v.z; rnd[4 * k + 3] = v.w;
+                if constexpr (PIPE) {   // volatile: stays between the table loads of this site and of the next one
+                    asm volatile("ld.volatile.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                                 : "=r"(rnd[4 * k]), "=r"(rnd[4 * k + 1]), "=r"(rnd[4 * k + 2]), "=r"(rnd[4 * k + 3])
+                                 : "r"((uint32_t)__cvta_generic_to_shared(ring + (buf * NC + k) * stride)) : "memory");
+                } else {
+                    const uint4 v = ring[(buf * NC + k) * stride];
+                    rnd[4 * k] = v.x; rnd[4 * k + 1] = v.y; rnd[4 * k + 2] = v.z; rnd[4 * k + 3] = v.w;
+                }
             }
         }
         if constexpr (X + 1 < BITS)
-            RowSites<L, MEAS, X + 1, FIRST, LASTW, DTA>::run(S, A, flips, chk, off, g1, gx1, c, FW, fw3t, patch, rnd, n, FWp, FWseq, ring,
-                                                            stride, buf, more);
+            RowSites<L, MEAS, X + 1, FIRST, LASTW, DTA, PIPE>::run(S, A, flips, chk, off, g1, gx1, c, FW, fw3t, patch, rnd, n, FWp, FWseq,
+                                                                  ring, stride, buf, more, pp);
     }
 };
 
@@ -213,12 +293,12 @@ struct RowSites {
 // the row is processed, the row below is prepared in `n` (old value, partial planes), its field words FWn are finished
 // (FWn[r] as soon as the sites 4q + r of this row are final) and its deviates replace this row's in rnd[] (call k after
 // site 4k + 3).  Out: `up` = this row's new value, A / off / g1 / gx1 for the row below.
-// Every site increments the bin of the state it STARTS from, i.e. of the state after the previous attempt.
+// Every site increments the bin of the state its attempt leads to (pipelined site macro).
 template <int L, bool MEAS>
 __device__ __forceinline__ void row_v6(uint32_t* __restrict__ lat, uint32_t& S, uint32_t& A, uint32_t& chk, uint32_t& off, uint32_t& g1,
                                        uint32_t& gx1, const int y, const bool more, uint32_t& up, const uint32_t c, uint32_t (&FW)[4],
                                        const uint32_t patch, uint32_t (&rnd)[Geo<L>::BITS], NextRow<L>& n, uint32_t (&FWn)[4],
-                                       const uint4* ring, int& buf, const int bar_id) {
+                                       const uint4* ring, int& buf, const int bar_id, SitePipe& pp) {
     using V = V6<L>;
     constexpr int SLOTS = V::SLOTS;
     // the deviates of row y + 1 are in ring[buf]; ring[buf ^ 1] (this row's, all fetched) may be refilled.  After the
@@ -228,8 +308,8 @@ __device__ __forceinline__ void row_v6(uint32_t* __restrict__ lat, uint32_t& S, 
     n.c = lat[y1 * SLOTS];
     n.dn = lat[y2 * SLOTS];   // row y + 2 is old (or row 0, final in this sweep, when y + 1 = L - 1)
     uint32_t flips = 0;
-    RowSites<L, MEAS, 0, true, true, V::SBASE + V::DT_OFF>::run(S, A, flips, chk, off, g1, gx1, c, FW, FW[3], patch, rnd, n, FWn, FWn, ring,
-                                                                SLOTS, buf, more);
+    RowSites<L, MEAS, 0, true, true, V::SBASE + V::DT_OFF, true>::run(S, A, flips, chk, off, g1, gx1, c, FW, FW[3], patch, rnd, n, FWn, FWn,
+                                                                      ring, SLOTS, buf, more, pp);
     buf ^= (int)more;
     up = c ^ flips;
     lat[y * SLOTS] = up;
@@ -238,7 +318,6 @@ __device__ __forceinline__ void row_v6(uint32_t* __restrict__ lat, uint32_t& S, 
 
 // Walker warp: sweeps s0 .. s1-1; `buf` is the ring buffer holding the deviates of the next row to fetch.  Rows are
 // processed in pairs so that the two register sets (this row / row below) swap roles without copies.
-// The caller compensates the first and the last attempt of the measured phase in the histogram (see row_v6).
 template <int L, bool MEAS>
 __device__ __forceinline__ void sweeps_v6(uint32_t* __restrict__ lat, uint32_t& S, uint32_t& chk, const uint32_t s0, const uint32_t s1,
                                           const uint4* ring, int& buf, const int bar_id) {
@@ -264,13 +343,17 @@ __device__ __forceinline__ void sweeps_v6(uint32_t* __restrict__ lat, uint32_t& 
     uint32_t off = (FWA[0] << 2) & 0x1Cu;      // site 0: its left neighbour (site L-1) has not been visited in this sweep
     uint32_t A = S + off;
     uint32_t g1 = (FWA[1] << 2) & 0x1Cu, gx1 = g1 ^ 4u;
+    SitePipe pp;
+    pp.dep = 0u;
+    asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(pp.t) : "r"(A) : "memory");                            // threshold and
+    asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(pp.d) : "r"(off + V::SBASE + V::DT_OFF) : "memory");   // delta of site 0
 #pragma unroll 1
     for (uint32_t s = s0; s < s1; ++s) {
 #pragma unroll 1
         for (int y = 0; y < L; y += 2) {
-            row_v6<L, MEAS>(lat, S, A, chk, off, g1, gx1, y, true, up, nA.c, FWA, nA.patch, rnd, nB, FWB, ring, buf, bar_id);
+            row_v6<L, MEAS>(lat, S, A, chk, off, g1, gx1, y, true, up, nA.c, FWA, nA.patch, rnd, nB, FWB, ring, buf, bar_id, pp);
             row_v6<L, MEAS>(lat, S, A, chk, off, g1, gx1, y + 1, s + 1 < s1 || y + 2 < L, up, nB.c, FWB, nB.patch, rnd, nA, FWA, ring, buf,
-                            bar_id);
+                            bar_id, pp);
         }
     }
 }
@@ -376,12 +459,9 @@ __global__ void __launch_bounds__(64 * V6<L>::MAX_WARPS, 1) sweep_kernel_v6(cons
     // ---- thermalisation sweeps: nothing is recorded
     if (is_walker) sweeps_v6<L, false>(lat, S, chk, prm.sweep_begin, s_th, ring + slot, buf, bar_id);
     else deviates_v6<L>(ring + slot, scratch, prm.sweep_begin, s_th, buf, bar_id, prm, walker, active, lane);
-    // ---- measured sweeps: every site counts the state it starts from, so the state before the first measured
-    //      attempt is taken out again here and the state after the last one is added below
+    // ---- measured sweeps: every attempt counts the state it leads to
     if (is_walker) {
-        if (s_th < prm.sweep_end) atomicSub(reinterpret_cast<uint32_t*>(sm + (S - sbase) + V::BIN_OFF), 1u);
         sweeps_v6<L, true>(lat, S, chk, s_th, prm.sweep_end, ring + slot, buf, bar_id);
-        if (s_th < prm.sweep_end) atomicAdd(reinterpret_cast<uint32_t*>(sm + (S - sbase) + V::BIN_OFF), 1u);
     } else {
         deviates_v6<L>(ring + slot, scratch, s_th, prm.sweep_end, buf, bar_id, prm, walker, active, lane);
     }

@@ -53,6 +53,7 @@ __device__ __forceinline__ void sweeps_s6(uint32_t* __restrict__ rows, const siz
     ld_row<WPR>(rows + (size_t)(2 % L) * row_stride, R2);
     uint32_t FWc[WPR][4], FWn[WPR][4], rnd[32], patch = 0, patch_n = 0;
     NextRow<L> n;
+    SitePipe pp{0u, 0u, 0u};                   // unused by the non-pipelined site macro
 #pragma unroll
     for (int k = 0; k < WPR; ++k) {            // field words of row 0 (the row above it, row L - 1, is final)
         n.c = R0[k]; n.left = R0[(k + WPR - 1) % WPR]; n.right = R0[(k + 1) % WPR]; n.dn = R1[k];
@@ -85,17 +86,17 @@ __device__ __forceinline__ void sweeps_s6(uint32_t* __restrict__ rows, const siz
                 n.c = R1[k]; n.left = R1[(k + WPR - 1) % WPR]; n.right = R1[(k + 1) % WPR]; n.dn = R2[k];
                 uint32_t flips = 0;
                 if (k == 0 && k == WPR - 1)
-                    RowSites<L, MEAS, 0, true, true, S6_DTA>::run(S, A, flips, chk, off, g1, gx1, R0[k], FWc[k], FWc[WPR - 1][3], patch, rnd, n,
-                                                                  FWn[k], FWn[0], ring, slots, buf, more);
+                    RowSites<L, MEAS, 0, true, true, S6_DTA, false>::run(S, A, flips, chk, off, g1, gx1, R0[k], FWc[k], FWc[WPR - 1][3], patch, rnd, n,
+                                                                  FWn[k], FWn[0], ring, slots, buf, more, pp);
                 else if (k == 0)
-                    RowSites<L, MEAS, 0, true, false, S6_DTA>::run(S, A, flips, chk, off, g1, gx1, R0[k], FWc[k], FWc[WPR - 1][3], patch, rnd, n,
-                                                                   FWn[k], FWc[(k + 1) % WPR], ring, slots, buf, more);
+                    RowSites<L, MEAS, 0, true, false, S6_DTA, false>::run(S, A, flips, chk, off, g1, gx1, R0[k], FWc[k], FWc[WPR - 1][3], patch, rnd, n,
+                                                                   FWn[k], FWc[(k + 1) % WPR], ring, slots, buf, more, pp);
                 else if (k == WPR - 1)
-                    RowSites<L, MEAS, 0, false, true, S6_DTA>::run(S, A, flips, chk, off, g1, gx1, R0[k], FWc[k], FWc[WPR - 1][3], patch, rnd, n,
-                                                                   FWn[k], FWn[0], ring, slots, buf, more);
+                    RowSites<L, MEAS, 0, false, true, S6_DTA, false>::run(S, A, flips, chk, off, g1, gx1, R0[k], FWc[k], FWc[WPR - 1][3], patch, rnd, n,
+                                                                   FWn[k], FWn[0], ring, slots, buf, more, pp);
                 else
-                    RowSites<L, MEAS, 0, false, false, S6_DTA>::run(S, A, flips, chk, off, g1, gx1, R0[k], FWc[k], FWc[WPR - 1][3], patch, rnd, n,
-                                                                    FWn[k], FWc[(k + 1) % WPR], ring, slots, buf, more);
+                    RowSites<L, MEAS, 0, false, false, S6_DTA, false>::run(S, A, flips, chk, off, g1, gx1, R0[k], FWc[k], FWc[WPR - 1][3], patch, rnd, n,
+                                                                    FWn[k], FWc[(k + 1) % WPR], ring, slots, buf, more, pp);
                 buf ^= (int)more;
                 R0[k] ^= flips;
                 FWn[k][3] = finish_word<L>(n, R0[k], 3);
