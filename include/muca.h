@@ -52,17 +52,17 @@ typedef enum muca_status {
     MUCA_ENOMEM = -4  /* workspace too small / allocation failed                                */
 } muca_status;
 
-/* Sweep-kernel variants (muca_set_option(ctx, MUCA_OPT_KERNEL, ...)).
- * AUTO picks RESIDENT for L <= 32 (lattices, threshold table and histogram in shared memory) and STREAMED_PAIRS for
- * L >= 64 (table and histogram in shared memory, lattice rows streamed from HBM/L2, Philox in paired deviate warps;
- * STREAMED_SMEM is the same with Philox in the walker thread).  At L = 128 the table no longer
- * fits: shared memory then holds a WINDOW of it around the walkers' energies; an iteration in which a walker leaves
- * the window is detected and repeated from a snapshot with STREAMED (thresholds through L1) -- same results. */
-enum { MUCA_KERNEL_AUTO = 0, MUCA_KERNEL_RESIDENT = 1, MUCA_KERNEL_STREAMED = 2,
-       MUCA_KERNEL_RESIDENT_V2 = 3, /* L <= 32 only: the earlier predicate-carried resident kernel, kept for A/B runs */
-       MUCA_KERNEL_RESIDENT_V3 = 4, /* L <= 32 only: the earlier paired walker/deviate-warp kernel, kept for A/B runs */
-       MUCA_KERNEL_STREAMED_SMEM = 5, /* L >= 32: lattice rows streamed, threshold table (or a window of it) + histogram in shared memory */
-       MUCA_KERNEL_STREAMED_PAIRS = 6 /* L >= 32: the same with Philox in paired deviate warps (as in RESIDENT) */ };
+/* Sweep-kernel variants (muca_set_option(ctx, MUCA_OPT_KERNEL, ...)); every variant gives the same Markov chains.
+ * AUTO picks RESIDENT for L <= 32 and STREAMED_PAIRS for L >= 64.
+ *   RESIDENT       (L <= 32) lattices, threshold table and histogram in shared memory, Philox in paired deviate warps;
+ *   STREAMED_PAIRS (L >= 32) table and histogram in shared memory, lattice rows streamed from HBM / L2, Philox in paired
+ *                  deviate warps.  At L = 128 the table no longer fits: shared memory then holds a WINDOW of it around
+ *                  the walkers' energies; an iteration in which a walker leaves the window is detected and repeated
+ *                  from a snapshot with STREAMED -- same results (muca_window_stats() counts both);
+ *   STREAMED       (L >= 32) thresholds read through L1, histogram in shared memory, lattice rows streamed, Philox in the
+ *                  walker thread: the plain kernel and the fallback of the window.
+ * A variant that does not exist for the context's L is replaced by the one AUTO would pick. */
+enum { MUCA_KERNEL_AUTO = 0, MUCA_KERNEL_RESIDENT = 1, MUCA_KERNEL_STREAMED = 2, MUCA_KERNEL_STREAMED_PAIRS = 3 };
 enum {
     MUCA_OPT_KERNEL = 1,          /* one of MUCA_KERNEL_*                                        */
     MUCA_OPT_THREADS_PER_BLOCK = 2, /* walkers per block (a multiple of 32); 0 = library default (walkers spread over all
@@ -78,10 +78,22 @@ enum {
                                      muca_production then runs therm_sweeps * N and sweeps * N updates per call) */
     MUCA_OPT_ROLE_MAP = 7,        /* resident kernel with 4 warp pairs per block: 0 = walker warps share schedulers with
                                      walker warps, 1 = every scheduler runs one walker and one deviate warp (A/B knob) */
-    MUCA_OPT_TABLE_WINDOW_ROWS = 6 /* STREAMED_SMEM kernel: rows of the threshold-table window held in shared memory;
-                                     0 = as many as fit.  A value below L*L+1 forces the windowed kernel (testing) */
+    MUCA_OPT_TABLE_WINDOW_ROWS = 6 /* STREAMED_PAIRS kernel: rows of the threshold-table window held in shared memory;
+                                     0 = as many as fit.  A value below L*L+1 forces a window (testing) */
 };
 enum { MUCA_SCHEME_TYPEWRITER = 0, MUCA_SCHEME_RANDOM_SITE = 1 };
+
+/* The walker count at which the current CUDA device is fully and evenly loaded by the default kernel for lattice size L --
+ * the analogue of the paper's N_opt, "the first and lowest minimum" of the time per spin flip over the number of walkers,
+ * which its code sets automatically when the user gives no W (W = 8 blocks x 256 threads x number of SMX;
+ * :201 "the first optimum as automatically chosen by our code").  Here one block runs per SM and a walker warp is paired
+ * with a deviate warp, so the optimum is
+ *     n_walkers = (number of SMs) x pairs_per_sm x 32,   pairs_per_sm = 4 (L <= 32), 8 (L = 64), 4 (L = 128)
+ * (the most warp pairs the default kernel runs per SM: the time per site of a walker grows more slowly than the number
+ * of pairs, profiles/README.md "flips/s over W"); any multiple of it loads the SMs evenly as well and runs in as many
+ * rounds.  Fewer walkers leave schedulers idle, a count in between loads the SMs unevenly.
+ * Host logic + one device-attribute query.  MUCA_EINVAL for an unsupported L or NULL outputs, MUCA_ECUDA without a device. */
+int muca_suggest_walkers(int L, int* n_walkers_out, int* pairs_per_sm_out);
 
 /* Device workspace needed by muca_create_in() for (L, n_walkers); 0 on bad arguments. */
 size_t muca_workspace_bytes(int L, int n_walkers);

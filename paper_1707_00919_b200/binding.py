@@ -12,9 +12,7 @@ import numpy as np
 from . import build as _build
 
 MUCA_OK = 0
-MUCA_KERNEL_AUTO, MUCA_KERNEL_RESIDENT, MUCA_KERNEL_STREAMED, MUCA_KERNEL_RESIDENT_V2, MUCA_KERNEL_RESIDENT_V3 = 0, 1, 2, 3, 4
-MUCA_KERNEL_STREAMED_SMEM = 5
-MUCA_KERNEL_STREAMED_PAIRS = 6
+MUCA_KERNEL_AUTO, MUCA_KERNEL_RESIDENT, MUCA_KERNEL_STREAMED, MUCA_KERNEL_STREAMED_PAIRS = 0, 1, 2, 3
 MUCA_OPT_KERNEL, MUCA_OPT_THREADS_PER_BLOCK, MUCA_OPT_MAX_SWEEPS_PER_LAUNCH, MUCA_OPT_WALKERS_PER_WARP = 1, 2, 3, 4
 MUCA_OPT_UPDATE_SCHEME = 5
 MUCA_OPT_TABLE_WINDOW_ROWS = 6
@@ -23,7 +21,7 @@ MUCA_SCHEME_TYPEWRITER, MUCA_SCHEME_RANDOM_SITE = 0, 1
 
 # every symbol include/muca.h declares (tests/test_abi.py checks the header against this list and the .so)
 EXPORTS = (
-    "muca_workspace_bytes", "muca_create", "muca_create_in", "muca_destroy", "muca_set_option",
+    "muca_workspace_bytes", "muca_suggest_walkers", "muca_create", "muca_create_in", "muca_destroy", "muca_set_option",
     "muca_set_log_weights", "muca_get_log_weights", "muca_run_iteration", "muca_get_histogram",
     "muca_update_weights", "muca_update_weights_with", "muca_get_energies", "muca_get_spins", "muca_set_spins",
     "muca_unpack_spins_device", "muca_get_thresholds", "muca_get_iteration", "muca_set_iteration",
@@ -69,6 +67,7 @@ def lib():
     L = C.CDLL(path)
     vp, u32p, u64p = C.c_void_p, C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)
     f64p, i8p, i32p = C.POINTER(C.c_double), C.POINTER(C.c_int8), C.POINTER(C.c_int32)
+    L.muca_suggest_walkers.argtypes = [C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int)]
     L.muca_workspace_bytes.argtypes = [C.c_int, C.c_int]
     L.muca_workspace_bytes.restype = C.c_size_t
     L.muca_create.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_uint64]
@@ -108,6 +107,15 @@ def lib():
 
 def _p(a, t):
     return a.ctypes.data_as(C.POINTER(t))
+
+
+def suggest_walkers(L: int):
+    """muca_suggest_walkers: (n_walkers, pairs_per_sm) that load the current device fully and evenly."""
+    w, p = C.c_int(), C.c_int()
+    rc = lib().muca_suggest_walkers(L, C.byref(w), C.byref(p))
+    if rc != MUCA_OK:
+        raise MucaError(f"muca_suggest_walkers failed rc={rc}")
+    return w.value, p.value
 
 
 def workspace_bytes(L: int, n_walkers: int) -> int:

@@ -17,7 +17,6 @@
 #include "muca_device.cuh"
 #include "muca_resident.cuh"
 #include "muca_random_site.cuh"
-#include "muca_window.cuh"
 #include "muca_streamed.cuh"
 
 using namespace muca;
@@ -55,6 +54,7 @@ struct muca_ctx {
     int* d_flag = nullptr;          // device int[4]: window-left flag, smallest / largest slot of the walkers
     int* h_flag = nullptr;          // pinned copy (tail of h_H's allocation)
     int stat_window_iterations = 0, stat_window_fallbacks = 0;
+    int win_margin = 8;             // rows asked for between the outermost walker and a sentinel; grows after a fallback
     int conv_w_prev = 0;            // width covered by the previous iteration of muca_converge (0: none yet)
     double conv_n_updates = 0.0;    // N_updates (flips per walker) of the previous iteration of muca_converge
     int opt_scheme = MUCA_SCHEME_TYPEWRITER;   // update scheme used by muca_converge / muca_production
@@ -172,15 +172,6 @@ void expand_table8(const std::vector<uint32_t>& t5, int bins, uint32_t* t8) {
 }
 
 template <int L>
-int launch_sweep_v3(muca_ctx* ctx, const SweepParams& prm, int tpb) {
-    SMEM(sweep_kernel_v3<L>, V3<L>::SMEM_BYTES);
-    const int grid = (prm.W + tpb - 1) / tpb;
-    sweep_kernel_v3<L><<<grid, 2 * tpb, V3<L>::SMEM_BYTES, ctx->stream>>>(prm);   // tpb walker + tpb deviate threads
-    CU(cudaGetLastError());
-    return MUCA_OK;
-}
-
-template <int L>
 int launch_sweep_v6(muca_ctx* ctx, const SweepParams& prm, int nw, int wpw) {
     SMEM(sweep_kernel_v6<L>, V6<L>::SMEM_BYTES);
     const int per_block = nw * wpw;
@@ -190,40 +181,38 @@ int launch_sweep_v6(muca_ctx* ctx, const SweepParams& prm, int nw, int wpw) {
     return MUCA_OK;
 }
 
-template <int L, int MODE>
-int launch_sweep_t(muca_ctx* ctx, const SweepParams& prm, int tpb) {
-    const size_t smem = sweep_smem_bytes<L, MODE>(tpb);
-    SMEM((sweep_kernel<L, MODE>), smem);
-    const int grid = (prm.W + tpb - 1) / tpb;
-    sweep_kernel<L, MODE><<<grid, tpb, smem, ctx->stream>>>(prm);
+template <int L>
+int launch_sweep_l1(muca_ctx* ctx, const SweepParams& prm, int tpb) {
+    SMEM(sweep_kernel_l1<L>, l1_smem_bytes<L>());
+    sweep_kernel_l1<L><<<(prm.W + tpb - 1) / tpb, tpb, l1_smem_bytes<L>(), ctx->stream>>>(prm);
     CU(cudaGetLastError());
     return MUCA_OK;
 }
 
-constexpr int MODE_WPAIR = 7;    // sweep_kernel_wpair: the same with Philox in paired deviate warps (round 1)
-constexpr int MODE_S6 = 8;       // sweep_kernel_s6 (muca_streamed.cuh): streamed lattices, v6 site chain, paired deviate warps
-constexpr int MODE_WINDOW = 6;   // sweep_kernel_window (muca_window.cuh): streamed lattices + a window of the table in shared memory
-struct Plan { int mode; int tpb; int nw; int wpw; };   // tpb = walkers per block; v5: nw warp pairs x wpw walkers per warp
+// kernels: MODE_V6 = sweep_kernel_v6 (muca_resident.cuh, L <= 32), MODE_S6 = sweep_kernel_s6 (muca_streamed.cuh, L >= 32),
+// MODE_L1 = sweep_kernel_l1 (muca_device.cuh, L >= 32)
+enum { MODE_V6 = 0, MODE_L1 = 1, MODE_S6 = 2 };
+struct Plan { int mode; int tpb; int nw; int wpw; };   // tpb = walkers per block; v6: nw warp pairs x wpw walkers per warp
+
+// walkers per block of the L1 kernel: with few walkers one warp per block (they spread over the SMs), otherwise two
+int l1_default_tpb(const muca_ctx* c) {
+    const int n_sm = c->n_sm > 0 ? c->n_sm : 148;
+    return c->W > 64 * n_sm ? 64 : 32;
+}
 
 Plan make_plan(const muca_ctx* c) {
     Plan p;
     const int L = c->L;
     int kern = c->opt_kernel;
     if (kern == MUCA_KERNEL_AUTO) kern = L <= 32 ? MUCA_KERNEL_RESIDENT : MUCA_KERNEL_STREAMED_PAIRS;
-    if (kern == MUCA_KERNEL_STREAMED && L < 32) kern = MUCA_KERNEL_RESIDENT;
-    if ((kern == MUCA_KERNEL_RESIDENT_V2 || kern == MUCA_KERNEL_RESIDENT_V3) && L > 32) kern = MUCA_KERNEL_RESIDENT;
+    if (L < 32) kern = MUCA_KERNEL_RESIDENT;                                        // the streamed kernels work on whole 32-site words
+    if (L > 32 && kern == MUCA_KERNEL_RESIDENT) kern = MUCA_KERNEL_STREAMED_PAIRS;   // lattices of L >= 64 do not fit beside the table
     p.nw = p.wpw = 0;
-    if (kern == MUCA_KERNEL_RESIDENT) p.mode = L <= 32 ? MODE_V5 : MODE_TBL_L1;
-    else if (kern == MUCA_KERNEL_RESIDENT_V3) p.mode = MODE_V3;
-    else if (kern == MUCA_KERNEL_RESIDENT_V2) p.mode = MODE_TBL_SMEM;
-    else if (kern == MUCA_KERNEL_STREAMED_PAIRS) p.mode = L < 32 ? MODE_V5 : MODE_S6;
-    else if (kern == MUCA_KERNEL_STREAMED_SMEM)
-        p.mode = L < 32 ? MODE_V5 : (L == 128 || c->opt_window_rows > 0) ? MODE_WINDOW : MODE_STREAMED_SMEM;
-    else p.mode = MODE_STREAMED;
-    if (p.mode == MODE_V5) {
+    const int n_sm = c->n_sm > 0 ? c->n_sm : 148;
+    if (kern == MUCA_KERNEL_RESIDENT) {
         // spread the walkers over all SMs: as few warps per SM as possible, then as few lanes per warp as possible
         // (one block per SM; a half-empty warp costs the same issue slots, but fewer lanes collide in the banks)
-        const int n_sm = c->n_sm > 0 ? c->n_sm : 148;
+        p.mode = MODE_V6;
         const int warps = (c->W + 31) / 32;
         int nw = c->opt_tpb > 0 ? c->opt_tpb / 32 : (warps <= n_sm ? 1 : warps <= 2 * n_sm ? 2 : 4);
         if (nw < 1) nw = 1;
@@ -235,66 +224,27 @@ Plan make_plan(const muca_ctx* c) {
         return p;
     }
     int tpb = c->opt_tpb;
-    if (tpb <= 0) {
-        if (p.mode == MODE_V3) tpb = L == 32 ? 128 : 32;
-        else if (p.mode == MODE_TBL_SMEM) tpb = 32;
-        else if (p.mode == MODE_TBL_L1) tpb = L == 64 ? 64 : 32;
-        else if (p.mode == MODE_STREAMED_SMEM || p.mode == MODE_WINDOW || p.mode == MODE_WPAIR || p.mode == MODE_S6) {
-            // one block per SM (164 KB of table at L = 64): spread the walkers over all SMs
-            const int n_sm = c->n_sm > 0 ? c->n_sm : 148;
+    if (kern == MUCA_KERNEL_STREAMED_PAIRS) {
+        p.mode = MODE_S6;
+        if (tpb <= 0) {   // one block per SM (147 KB of table at L = 64): spread the walkers over all SMs
             tpb = ((c->W + n_sm - 1) / n_sm + 31) / 32 * 32;
-            if (tpb > 512) tpb = 512;
-            if (p.mode == MODE_WPAIR && tpb > 32 * WPAIR_MAX_PAIRS) tpb = 32 * WPAIR_MAX_PAIRS;
-            if (p.mode == MODE_S6 && tpb > 32 * s6_max_pairs(L)) tpb = 32 * s6_max_pairs(L);
+            if (tpb > 32 * s6_max_pairs(L)) tpb = 32 * s6_max_pairs(L);
         }
-        else tpb = 32;
+    } else {
+        p.mode = MODE_L1;
+        if (tpb <= 0) tpb = l1_default_tpb(c);
     }
     p.tpb = tpb;
     return p;
 }
 
 size_t plan_smem(int L, const Plan& p) {
-    if (p.mode == MODE_WINDOW || p.mode == MODE_WPAIR || p.mode == MODE_S6) return 0;   // sized at run time from what the device allows
-    if (p.mode == MODE_V5) return L == 8 ? V6<8>::SMEM_BYTES : L == 16 ? V6<16>::SMEM_BYTES : V6<32>::SMEM_BYTES;
-    if (p.mode == MODE_V3) return L == 8 ? V3<8>::SMEM_BYTES : L == 16 ? V3<16>::SMEM_BYTES : V3<32>::SMEM_BYTES;
-    switch (L) {
-        case 8: return sweep_smem_bytes<8, MODE_TBL_SMEM>(p.tpb);
-        case 16: return sweep_smem_bytes<16, MODE_TBL_SMEM>(p.tpb);
-        case 32: return p.mode == MODE_STREAMED_SMEM ? sweep_smem_bytes<32, MODE_STREAMED_SMEM>(p.tpb)
-                        : p.mode == MODE_TBL_SMEM ? sweep_smem_bytes<32, MODE_TBL_SMEM>(p.tpb)
-                        : p.mode == MODE_TBL_L1 ? sweep_smem_bytes<32, MODE_TBL_L1>(p.tpb)
-                                                : sweep_smem_bytes<32, MODE_STREAMED>(p.tpb);
-        case 64: return p.mode == MODE_STREAMED ? sweep_smem_bytes<64, MODE_STREAMED>(p.tpb)
-                        : p.mode == MODE_STREAMED_SMEM ? sweep_smem_bytes<64, MODE_STREAMED_SMEM>(p.tpb)
-                                                : sweep_smem_bytes<64, MODE_TBL_L1>(p.tpb);
-        default: return p.mode == MODE_STREAMED_SMEM ? sweep_smem_bytes<128, MODE_STREAMED_SMEM>(p.tpb)
-                        : p.mode == MODE_STREAMED ? sweep_smem_bytes<128, MODE_STREAMED>(p.tpb)
-                                                : sweep_smem_bytes<128, MODE_TBL_L1>(p.tpb);
-    }
+    if (p.mode == MODE_S6) return 0;   // sized at run time from what the device allows
+    if (p.mode == MODE_V6) return L == 8 ? V6<8>::SMEM_BYTES : L == 16 ? V6<16>::SMEM_BYTES : V6<32>::SMEM_BYTES;
+    return L == 32 ? l1_smem_bytes<32>() : L == 64 ? l1_smem_bytes<64>() : l1_smem_bytes<128>();
 }
 
 struct Window { int j_lo = 0, n_rows = 0, sent_lo = 0, sent_hi = 0; };
-
-template <int L>
-int launch_window_t(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& win) {
-    const size_t smem = window_smem_bytes(win.n_rows);
-    SMEM((sweep_kernel_window<L>), smem);
-    sweep_kernel_window<L><<<(prm.W + tpb - 1) / tpb, tpb, smem, ctx->stream>>>(prm, win.j_lo, win.n_rows, win.sent_lo,
-                                                                               win.sent_hi, ctx->d_flag);
-    CU(cudaGetLastError());
-    return MUCA_OK;
-}
-
-template <int L>
-int launch_wpair_t(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& win) {
-    const int npairs = tpb / 32;
-    const size_t smem = wpair_smem_bytes(win.n_rows, npairs);
-    SMEM((sweep_kernel_wpair<L>), smem);
-    sweep_kernel_wpair<L><<<(prm.W + tpb - 1) / tpb, 2 * tpb, smem, ctx->stream>>>(prm, win.j_lo, win.n_rows, win.sent_lo,
-                                                                                  win.sent_hi, ctx->d_flag);
-    CU(cudaGetLastError());
-    return MUCA_OK;
-}
 
 template <int L>
 int launch_s6_t(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& win) {
@@ -317,55 +267,19 @@ int launch_s6(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& win)
     return fail(ctx, MUCA_EINVAL, "paired streamed kernel: L must be 32, 64 or 128");
 }
 
-int launch_wpair(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& win) {
-    switch (ctx->L) {
-        case 32: return launch_wpair_t<32>(ctx, prm, tpb, win);
-        case 64: return launch_wpair_t<64>(ctx, prm, tpb, win);
-        case 128: return launch_wpair_t<128>(ctx, prm, tpb, win);
-    }
-    return fail(ctx, MUCA_EINVAL, "paired streamed kernel: L must be 32, 64 or 128");
-}
-
-int launch_window(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& win) {
-    switch (ctx->L) {
-        case 32: return launch_window_t<32>(ctx, prm, tpb, win);
-        case 64: return launch_window_t<64>(ctx, prm, tpb, win);
-        case 128: return launch_window_t<128>(ctx, prm, tpb, win);
-    }
-    return fail(ctx, MUCA_EINVAL, "windowed kernel: L must be 32, 64 or 128");
-}
-
 int launch_sweep(muca_ctx* ctx, const SweepParams& prm, const Plan& p) {
-    if (p.mode == MODE_V5) {
+    if (p.mode == MODE_V6) {
         switch (ctx->L) {
             case 8: return launch_sweep_v6<8>(ctx, prm, p.nw, p.wpw);
             case 16: return launch_sweep_v6<16>(ctx, prm, p.nw, p.wpw);
             case 32: return launch_sweep_v6<32>(ctx, prm, p.nw, p.wpw);
         }
-    }
-    if (p.mode == MODE_V3) {
-        if (p.tpb > V3<32>::MAX_TPB) return fail(ctx, MUCA_EINVAL, "resident kernel: at most %d threads per block", V3<32>::MAX_TPB);
+    } else if (p.mode == MODE_L1) {
         switch (ctx->L) {
-            case 8: return launch_sweep_v3<8>(ctx, prm, p.tpb);
-            case 16: return launch_sweep_v3<16>(ctx, prm, p.tpb);
-            case 32: return launch_sweep_v3<32>(ctx, prm, p.tpb);
+            case 32: return launch_sweep_l1<32>(ctx, prm, p.tpb);
+            case 64: return launch_sweep_l1<64>(ctx, prm, p.tpb);
+            case 128: return launch_sweep_l1<128>(ctx, prm, p.tpb);
         }
-    }
-    switch (ctx->L) {
-        case 8: return launch_sweep_t<8, MODE_TBL_SMEM>(ctx, prm, p.tpb);
-        case 16: return launch_sweep_t<16, MODE_TBL_SMEM>(ctx, prm, p.tpb);
-        case 32:
-            if (p.mode == MODE_TBL_SMEM) return launch_sweep_t<32, MODE_TBL_SMEM>(ctx, prm, p.tpb);
-            if (p.mode == MODE_STREAMED_SMEM) return launch_sweep_t<32, MODE_STREAMED_SMEM>(ctx, prm, p.tpb);
-            if (p.mode == MODE_TBL_L1) return launch_sweep_t<32, MODE_TBL_L1>(ctx, prm, p.tpb);
-            return launch_sweep_t<32, MODE_STREAMED>(ctx, prm, p.tpb);
-        case 64:
-            if (p.mode == MODE_STREAMED) return launch_sweep_t<64, MODE_STREAMED>(ctx, prm, p.tpb);
-            if (p.mode == MODE_STREAMED_SMEM) return launch_sweep_t<64, MODE_STREAMED_SMEM>(ctx, prm, p.tpb);
-            return launch_sweep_t<64, MODE_TBL_L1>(ctx, prm, p.tpb);
-        case 128:
-            if (p.mode == MODE_STREAMED) return launch_sweep_t<128, MODE_STREAMED>(ctx, prm, p.tpb);
-            return launch_sweep_t<128, MODE_TBL_L1>(ctx, prm, p.tpb);
     }
     return fail(ctx, MUCA_EINVAL, "unsupported L=%d", ctx->L);
 }
@@ -464,6 +378,17 @@ int launch_random_site(muca_ctx* ctx, const RandomSiteParams& prm, int tpb) {
 extern "C" {
 
 const char* muca_version(void) { return "muca_b200 0.1 (sm_100a)"; }
+
+int muca_suggest_walkers(int L, int* n_walkers_out, int* pairs_per_sm_out) {
+    if (!valid_L(L) || !n_walkers_out || !pairs_per_sm_out) return MUCA_EINVAL;
+    int dev = 0, n_sm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n_sm < 1)
+        return MUCA_ECUDA;
+    const int pairs = L <= 32 ? V6<32>::MAX_WARPS : s6_max_pairs(L);   // the most warp pairs make_plan() gives one block (= one SM)
+    *pairs_per_sm_out = pairs;
+    *n_walkers_out = n_sm * pairs * 32;
+    return MUCA_OK;
+}
 
 size_t muca_workspace_bytes(int L, int n_walkers) {
     if (!valid_L(L) || n_walkers < 1) return 0;
@@ -575,10 +500,10 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
 
     // windowed table (muca_window.cuh): pick the window around the walkers' slots, keep a snapshot for the fallback
     Plan fallback;
-    fallback.mode = MODE_STREAMED; fallback.tpb = 32; fallback.nw = fallback.wpw = 0;
+    fallback.mode = MODE_L1; fallback.tpb = l1_default_tpb(ctx); fallback.nw = fallback.wpw = 0;
     Window win;
     bool guarded = false;   // the window has sentinel rows: the result counts only if no walker entered one
-    const bool windowed_plan = plan.mode == MODE_WINDOW || plan.mode == MODE_WPAIR || plan.mode == MODE_S6;
+    const bool windowed_plan = plan.mode == MODE_S6;
     if (windowed_plan) {
         const size_t spin_bytes = (size_t)ctx->W * (ctx->N / 8);
         ctx->h_flag[0] = 0; ctx->h_flag[1] = 0x7FFFFFFF; ctx->h_flag[2] = -1;
@@ -588,11 +513,13 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
         CU(cudaMemcpyAsync(ctx->h_flag, ctx->d_flag, 3 * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
         CU(cudaStreamSynchronize(ctx->stream));
         const int lo = ctx->h_flag[1], hi = ctx->h_flag[2];
-        const size_t ring = plan.mode == MODE_WPAIR ? wpair_ring_bytes(plan.tpb / 32) : plan.mode == MODE_S6 ? s6_ring_bytes(plan.tpb / 32) + S6_RING_OFF : 0;
-        int cap = plan.mode == MODE_S6 ? (int)(((size_t)max_smem - ring) / S6_RS) - 2 * S6_PAD_ROWS
-                                       : (int)(((size_t)max_smem - 1024 - ring) / (ROW_SMEM_WORDS * 4)) - 2 * WINDOW_PAD_ROWS;
+        const size_t ring = s6_ring_bytes(plan.tpb / 32) + S6_RING_OFF;
+        int cap = (int)(((size_t)max_smem - ring) / S6_RS) - 2 * S6_PAD_ROWS;
         if (ctx->opt_window_rows > 0 && ctx->opt_window_rows < cap) cap = ctx->opt_window_rows;
-        const int margin = 8;   // rows between the outermost walker and a sentinel at the start of the iteration
+        // rows between the outermost walker and a sentinel at the start of the iteration.  An iteration that a walker left
+        // through a sentinel ran twice, so the margin asked for is quadrupled after such an iteration (the plain kernel is
+        // then taken at once where the walkers' span comes close to the window) and halved again after a clean one.
+        const int margin = ctx->win_margin;
         if (cap >= ctx->n_bins) {
             win.j_lo = 0; win.n_rows = ctx->n_bins;                          // the whole table fits: nothing to guard
         } else if (hi - lo + 1 + 2 * (2 + margin) > cap) {
@@ -608,7 +535,7 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
             CU(cudaMemcpyAsync(ctx->d_snap, ctx->d_spins, spin_bytes, cudaMemcpyDeviceToDevice, ctx->stream));
             CU(cudaMemcpyAsync((char*)ctx->d_snap + align_up(spin_bytes), ctx->d_E, (size_t)ctx->W * 4, cudaMemcpyDeviceToDevice, ctx->stream));
         }
-        if (plan.mode != MODE_STREAMED) ctx->stat_window_iterations += 1;
+        if (plan.mode != MODE_L1) ctx->stat_window_iterations += 1;
     }
 
     // a2-a4: sweeps.  A block's uint32 bins must not overflow: tpb * measured sweeps * N < 2^32 per launch.
@@ -620,10 +547,8 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
     int launches = windowed_plan ? 1 : 0;   // the slot-range kernel
     auto run_sweeps = [&](const Plan& pl) -> int {
         uint64_t max_meas = 0xFFFFFFFFull / ((uint64_t)pl.tpb * (uint64_t)ctx->N);
-        if (pl.mode == MODE_WINDOW || pl.mode == MODE_WPAIR) max_meas = 0xFFFFFFFFull / ((uint64_t)pl.tpb * (uint64_t)ctx->N) / 2;   // thermalisation counts too
         if (max_meas < 1) max_meas = 1;
-        const uint64_t max_any = ctx->opt_max_sweeps > 0 ? (uint64_t)ctx->opt_max_sweeps
-                                 : (pl.mode == MODE_WINDOW || pl.mode == MODE_WPAIR ? max_meas : total + 1);
+        const uint64_t max_any = ctx->opt_max_sweeps > 0 ? (uint64_t)ctx->opt_max_sweeps : total + 1;
         uint64_t s = 0;
         while (s < total) {
             uint64_t e = total;
@@ -631,9 +556,7 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
             if (e > meas_begin + max_meas) e = meas_begin + max_meas;
             if (e > s + max_any) e = s + max_any;
             prm.sweep_begin = (uint32_t)s; prm.sweep_end = (uint32_t)e;
-            const int rc = pl.mode == MODE_WINDOW ? launch_window(ctx, prm, pl.tpb, win)
-                           : pl.mode == MODE_WPAIR ? launch_wpair(ctx, prm, pl.tpb, win)
-                           : pl.mode == MODE_S6 ? launch_s6(ctx, prm, pl.tpb, win) : launch_sweep(ctx, prm, pl);
+            const int rc = pl.mode == MODE_S6 ? launch_s6(ctx, prm, pl.tpb, win) : launch_sweep(ctx, prm, pl);
             if (rc != MUCA_OK) return rc;
             ++launches;
             s = e;
@@ -645,7 +568,7 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
         const int rc = run_sweeps(plan);
         if (rc != MUCA_OK) return rc;
     }
-    if ((plan.mode == MODE_WINDOW || plan.mode == MODE_WPAIR || plan.mode == MODE_S6) && guarded) {
+    if (plan.mode == MODE_S6 && guarded) {
         CU(cudaMemcpyAsync(ctx->h_flag, ctx->d_flag, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
         CU(cudaStreamSynchronize(ctx->stream));
         if (ctx->h_flag[0]) {   // a walker left the window: repeat the iteration from the snapshot with the L1 kernel
@@ -654,8 +577,11 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
             CU(cudaMemcpyAsync(ctx->d_E, (char*)ctx->d_snap + align_up(spin_bytes), (size_t)ctx->W * 4, cudaMemcpyDeviceToDevice, ctx->stream));
             CU(cudaMemsetAsync(ctx->d_H, 0, (size_t)ctx->n_bins * 8, ctx->stream));
             ctx->stat_window_fallbacks += 1;
+            ctx->win_margin = ctx->win_margin * 4 > 4096 ? 4096 : ctx->win_margin * 4;
             const int rc = run_sweeps(fallback);
             if (rc != MUCA_OK) return rc;
+        } else if (ctx->win_margin > 8) {
+            ctx->win_margin /= 2;
         }
     }
     CU(cudaEventRecord(ctx->ev1, ctx->stream));

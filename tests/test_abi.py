@@ -35,6 +35,9 @@ def test_host_only_entry_points():
         n = mb.workspace_bytes(L, W)
         assert n >= W * L * L // 8 + 4 * W + (L * L + 1) * 40 and n % 256 == 0
     assert mb.workspace_bytes(12, 32) == 0 and mb.workspace_bytes(32, 0) == 0
+    w, p = ctypes.c_int(), ctypes.c_int()
+    assert lib.muca_suggest_walkers(12, ctypes.byref(w), ctypes.byref(p)) == -1
+    assert lib.muca_suggest_walkers(32, None, ctypes.byref(p)) == -1
     # bad arguments are rejected before any CUDA call
     h = ctypes.c_void_p()
     assert lib.muca_create(ctypes.byref(h), 7, 32, 1) == -1 and not h
