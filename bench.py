@@ -34,9 +34,19 @@ UNIT = "flips/s"
 # site update = 20 thread-instructions, of which 11.7 can only run on the 16-lane ALU pipe (LOP3/IADD3/SHF/SEL/ISETP).
 ALU_OPS_PER_FLIP = 11.7             # binding pipe: ALU, 16 lanes per scheduler per clock (profiles/r01_ubench_pipes.txt)
 OPS_PER_FLIP = 20.0                 # all thread-instructions (issue slots: 32 lanes per scheduler per clock)
-SM_COUNT, SCHED_PER_SM, ALU_LANES, ISSUE_LANES = 148, 4, 16, 32
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE sweep-kernel launch from the ncu --set full capture under profiles/
-NCU_DRAM_BYTES_PER_LAUNCH = {"L32_w16384": 2.24e6}
+SCHED_PER_SM, ALU_LANES, ISSUE_LANES = 4, 16, 32
+# Counters of ONE sweep-kernel launch per workload, copied from the ncu --set full captures under profiles/ by hand into
+# this file (dram__bytes_read.sum + dram__bytes_write.sum, pipe and issue utilisation; profiles/README.md names the
+# captures): read at run time, nothing is measured under the profiler here.
+NCU_SUMMARY = os.path.join(ROOT, "profiles", "r02_ncu_summary.json")
+
+
+def ncu_summary(workload):
+    try:
+        with open(NCU_SUMMARY) as f:
+            return json.load(f).get(workload)
+    except Exception:
+        return None
 
 
 def parse():
@@ -245,6 +255,8 @@ def run_ours(args, cfg):
 
     pk, pk_kind = peaks()
     f_max_hz = float(pk.get("sm_max_mhz", 1965.0)) * 1e6
+    SM_COUNT = torch.cuda.get_device_properties(dev).multi_processor_count
+    ncu = ncu_summary(cfg.name) if world == 1 else None
     value = world * flips_per_step * args.steps / (ms_dev * 1e-3)
     e2e_v = world * flips_per_step * args.steps / (ms_e2e * 1e-3)
     # dominant kernel: the sweep kernel (one launch per iteration)
@@ -254,11 +266,16 @@ def run_ours(args, cfg):
     achieved = kern_flips_s * ALU_OPS_PER_FLIP / 1e12
     peak = SM_COUNT * SCHED_PER_SM * ALU_LANES * f_max_hz / 1e12
     issue_peak = SM_COUNT * SCHED_PER_SM * ISSUE_LANES * f_max_hz / 1e12
-    kernel = "muca::sweep_kernel_v5<%d>" % cfg.L if cfg.L <= 32 else \
-        "muca::sweep_kernel_wpair<%d>" % cfg.L
+    kernel = "muca::sweep_kernel_v6<%d>" % cfg.L if cfg.L <= 32 else "muca::sweep_kernel_s6<%d>" % cfg.L
+    clk = sampler.result()
+    f_run_hz = (clk["sm_mhz"] or 0.0) * 1e6
     roofline = {
         "bound": "alu", "achieved": achieved, "peak": peak, "unit": "T lane-ops/s on the ALU pipe", "frac": achieved / peak,
-        "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(cfg.name) if world == 1 else None,
+        "frac_kind": "ALGORITHMIC: flips/s x 11.7 ALU-only instructions per attempted flip (DESIGN.md 6.2) over the ALU-pipe "
+                     "peak at sm_max_mhz; the instructions actually executed and the pipe utilisation ncu measured are under 'ncu'",
+        "frac_at_sampled_clock": achieved / (SM_COUNT * SCHED_PER_SM * ALU_LANES * f_run_hz / 1e12) if f_run_hz else None,
+        "traffic": ncu.get("dram_bytes_per_launch") if ncu else None,
+        "ncu": ncu,
         "kernel": kernel, "kernel_flips_per_s": kern_flips_s,
         "ops_per_flip": ALU_OPS_PER_FLIP, "avg_launch_ms": avg_launch_s * 1e3, "kernel_share_of_step": stats["sweep_ms"] / ms_dev,
         "c_flip_cycles": W * f_max_hz / kern_flips_s,
@@ -267,9 +284,12 @@ def run_ours(args, cfg):
         "issue": {"achieved": kern_flips_s * OPS_PER_FLIP / 1e12, "peak": issue_peak, "unit": "T thread-instructions/s",
                   "frac": kern_flips_s * OPS_PER_FLIP / 1e12 / issue_peak, "ops_per_flip": OPS_PER_FLIP},
         "hbm": {"algorithmic_bytes_per_flip": 0.0 if cfg.L <= 32 else 0.25, "peak_gbs": pk.get("hbm_gbs"),
-                "achieved_gbs": (0.0 if cfg.L <= 32 else 0.25) * kern_flips_s / 1e9,
-                "note": "lattices are shared-memory resident for L <= 32 (MiB of HBM traffic per launch); streamed at "
-                        "L >= 64: every packed word read and written once per sweep (16 MiB per config: served by L2)"},
+                "algorithmic_lattice_gbs": (0.0 if cfg.L <= 32 else 0.25) * kern_flips_s / 1e9,
+                "ncu_dram_gbs": ncu["dram_bytes_per_launch"] / avg_launch_s / 1e9 if ncu and ncu.get("dram_bytes_per_launch") else None,
+                "note": "algorithmic_lattice_gbs = 0.25 B per flip (every packed word of a streamed lattice read and written "
+                        "once per sweep) x flips/s: traffic between the SMs and L2, which holds the 16 MiB of lattices of "
+                        "configs 4 and 5; ncu_dram_gbs = what ncu saw at the DRAM interface for one launch over the launch "
+                        "time measured here.  Lattices are shared-memory resident for L <= 32."},
     }
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -279,7 +299,7 @@ def run_ours(args, cfg):
                    "therm_sweeps": cfg.therm_sweeps, "sweeps": cfg.sweeps, "seed": cfg.seed,
                    "flips_per_step_per_gpu": flips_per_step, "l2": "flushed between timed steps (256 MiB write)",
                    "parallelism": f"walkers x{world}, one all-reduce(H) per iteration" if world > 1 else "1 GPU"},
-        "clocks": sampler.result(),
+        "clocks": clk,
         "e2e": {"value": e2e_v, "unit": UNIT,
                 "h2d_bytes_per_step": cfg.iterations * table_bytes,
                 "d2h_bytes_per_step": cfg.iterations * hist_bytes + h_E.nbytes + h_spins.nbytes,

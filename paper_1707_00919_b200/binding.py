@@ -49,8 +49,13 @@ class MucaError(RuntimeError):
 _lib = None
 
 
+def checked() -> bool:
+    """MUCA_CHECKED=1 in the environment selects the self-checking build of the library (build.py LIB_CHECKED)."""
+    return os.environ.get("MUCA_CHECKED", "0") not in ("", "0")
+
+
 def lib_path() -> str:
-    return _build.LIB
+    return _build.LIB_CHECKED if checked() else _build.LIB
 
 
 def lib():
@@ -59,11 +64,11 @@ def lib():
     if _lib is not None:
         return _lib
     try:
-        path = _build.build()
+        path = _build.build(checked=checked())
     except _build.NvccMissing as e:   # no compiler here: a library built elsewhere is used as it is; a compile ERROR propagates
-        if not os.path.exists(_build.LIB):
-            raise MucaError(f"libmuca_b200.so is not built and cannot be built here: {e}") from e
-        path = _build.LIB
+        if not os.path.exists(lib_path()):
+            raise MucaError(f"{os.path.basename(lib_path())} is not built and cannot be built here: {e}") from e
+        path = lib_path()
     L = C.CDLL(path)
     vp, u32p, u64p = C.c_void_p, C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)
     f64p, i8p, i32p = C.POINTER(C.c_double), C.POINTER(C.c_int8), C.POINTER(C.c_int32)

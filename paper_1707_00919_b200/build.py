@@ -14,6 +14,9 @@ SOURCES = [os.path.join(CSRC, "muca.cu")]
 DEPS = SOURCES + sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith(".cuh")) + \
     [os.path.join(os.path.dirname(HERE), "include", "muca.h")]
 LIB = os.path.join(HERE, "libmuca_b200.so")
+# the same sources with -DMUCA_CHECKED: the kernels check their ring hand-overs and state addresses themselves
+# (csrc/muca_device.cuh "Self-checks"); loaded instead of LIB when the environment has MUCA_CHECKED=1
+LIB_CHECKED = os.path.join(HERE, "libmuca_b200_checked.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
@@ -25,10 +28,10 @@ def nvcc() -> str:
     return cand if os.path.exists(cand) else "nvcc"
 
 
-def stale() -> bool:
-    if not os.path.exists(LIB):
+def stale(lib: str = LIB) -> bool:
+    if not os.path.exists(lib):
         return True
-    t = os.path.getmtime(LIB)
+    t = os.path.getmtime(lib)
     return any(os.path.getmtime(d) > t for d in DEPS)
 
 
@@ -36,10 +39,11 @@ class NvccMissing(RuntimeError):
     """No nvcc on this machine (the only case in which an existing library may be used as it is)."""
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not stale():
-        return LIB
-    cmd = [nvcc()] + NVCC_FLAGS + ["-o", LIB + ".tmp"] + SOURCES
+def build(force: bool = False, verbose: bool = False, checked: bool = False) -> str:
+    lib = LIB_CHECKED if checked else LIB
+    if not force and not stale(lib):
+        return lib
+    cmd = [nvcc()] + NVCC_FLAGS + (["-DMUCA_CHECKED"] if checked else []) + ["-o", lib + ".tmp"] + SOURCES
     try:
         res = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     except FileNotFoundError as e:
@@ -47,10 +51,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if verbose or res.returncode != 0:
         sys.stderr.write(res.stdout)
     if res.returncode != 0:
-        raise RuntimeError("nvcc failed building libmuca_b200.so")
-    os.replace(LIB + ".tmp", LIB)
-    return LIB
+        raise RuntimeError("nvcc failed building " + os.path.basename(lib))
+    os.replace(lib + ".tmp", lib)
+    return lib
 
 
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose=True))
+    print(build(force="--force" in sys.argv, verbose=True, checked=True))

@@ -6,6 +6,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <limits>
 #include <map>
@@ -377,7 +378,11 @@ int launch_random_site(muca_ctx* ctx, const RandomSiteParams& prm, int tpb) {
 
 extern "C" {
 
-const char* muca_version(void) { return "muca_b200 0.1 (sm_100a)"; }
+#ifdef MUCA_CHECKED
+const char* muca_version(void) { return "muca_b200 0.2 (sm_100a) +checked"; }
+#else
+const char* muca_version(void) { return "muca_b200 0.2 (sm_100a)"; }
+#endif
 
 int muca_suggest_walkers(int L, int* n_walkers_out, int* pairs_per_sm_out) {
     if (!valid_L(L) || !n_walkers_out || !pairs_per_sm_out) return MUCA_EINVAL;
@@ -544,6 +549,11 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
     prm.W = ctx->W; prm.walker_offset = ctx->walker_offset;
     prm.key0 = (uint32_t)(ctx->seed & 0xFFFFFFFFull); prm.key1 = (uint32_t)(ctx->seed >> 32);
     prm.iteration = ctx->iteration; prm.therm = (uint32_t)therm_sweeps;
+    prm.check = ctx->d_flag + 3; prm.fault = 0u;
+#ifdef MUCA_CHECKED
+    if (const char* f = getenv("MUCA_CHECKED_FAULT")) prm.fault = (uint32_t)atoi(f);   // tests: make the self-check fire
+    CU(cudaMemsetAsync(ctx->d_flag + 3, 0, sizeof(int), ctx->stream));
+#endif
     int launches = windowed_plan ? 1 : 0;   // the slot-range kernel
     auto run_sweeps = [&](const Plan& pl) -> int {
         uint64_t max_meas = 0xFFFFFFFFull / ((uint64_t)pl.tpb * (uint64_t)ctx->N);
@@ -586,7 +596,15 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
     }
     CU(cudaEventRecord(ctx->ev1, ctx->stream));
     CU(cudaMemcpyAsync(ctx->h_H, ctx->d_H, (size_t)ctx->n_bins * 8, cudaMemcpyDeviceToHost, ctx->stream));
+#ifdef MUCA_CHECKED
+    CU(cudaMemcpyAsync(ctx->h_flag + 3, ctx->d_flag + 3, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+#endif
     CU(cudaStreamSynchronize(ctx->stream));
+#ifdef MUCA_CHECKED
+    if (ctx->h_flag[3])
+        return fail(ctx, MUCA_ECUDA, "checked build: self-check failed, mask 0x%x (1 = state is not a table row, 2 = deviates read before "
+                    "written, 4 = deviates overwritten while read)", ctx->h_flag[3]);
+#endif
     float ms = 0.f;
     CU(cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
     ctx->last_sweep_ms = ms;

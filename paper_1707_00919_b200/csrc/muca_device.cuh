@@ -181,7 +181,55 @@ struct SweepParams {
     uint32_t sweep_begin;       // first sweep index of this launch (ctr.y)
     uint32_t sweep_end;         // one past the last
     uint32_t therm;             // sweeps with index < therm are not recorded
+    int* check;                 // MUCA_CHECKED build: device word the violations are OR-ed into
+    uint32_t fault;             // MUCA_CHECKED build, tests: 1 + the hand-over that pair 0 of block 0 tags wrongly; 0 = none
 };
+
+// ------------------------------------------------------------------------------------------------
+// Self-checks of the MUCA_CHECKED build (libmuca_b200_checked.so; paper_1707_00919_b200/build.py).  compute-sanitizer
+// is not available on the GPU pool this library is developed on (profiles/r02_sanitizer.txt), so the two things its
+// racecheck / memcheck tools would watch in these kernels are checked by the kernels themselves:
+//  * the hand-over of deviates from a deviate warp to its walker warp through the double-buffered shared ring (named
+//    barriers): the deviate warp tags every buffer it fills with a running number, the walker warp compares the tag with
+//    its own count when it starts to fetch from a buffer (CHK_RING_EARLY: read before written) and when it has fetched
+//    the last call (CHK_RING_LATE: overwritten while being read);
+//  * the shared-memory address that IS the walker's state (every table load and histogram increment is relative to
+//    it): after every row it must be the address of a table row (CHK_STATE).
+// A violation sets a bit in a device word; muca_run_iteration then fails with MUCA_ECUDA.  In the normal build all of
+// this compiles to nothing.
+// ------------------------------------------------------------------------------------------------
+enum { CHK_STATE = 1, CHK_RING_EARLY = 2, CHK_RING_LATE = 4 };
+struct RingCheck {
+#ifdef MUCA_CHECKED
+    uint32_t ctr = 0;                     // hand-overs so far (deviate warp: published, walker warp: fetched)
+    volatile uint32_t* tags = nullptr;    // tags[buf * stride]: number of the hand-over whose deviates are in ring[buf]
+    int stride = 1;
+    int* flag = nullptr;
+    uint32_t fault = 0;
+#endif
+};
+__device__ __forceinline__ void ring_publish(RingCheck& rc, const int buf, const int lane) {   // deviate warp, in front of the barrier
+#ifdef MUCA_CHECKED
+    if (lane == 0) rc.tags[buf * rc.stride] = rc.ctr + (rc.fault == rc.ctr + 1u ? 1u : 0u);
+    rc.ctr += 1u;
+#endif
+}
+__device__ __forceinline__ void ring_expect(RingCheck& rc, const int buf, const int code) {    // walker warp, behind the barrier
+#ifdef MUCA_CHECKED
+    if (rc.tags[buf * rc.stride] != rc.ctr) atomicOr(rc.flag, code);
+#endif
+}
+__device__ __forceinline__ void ring_fetched(RingCheck& rc, const int buf) {                   // walker warp: last call of a buffer fetched
+#ifdef MUCA_CHECKED
+    ring_expect(rc, buf, CHK_RING_LATE);
+    rc.ctr += 1u;
+#endif
+}
+__device__ __forceinline__ void state_check(RingCheck& rc, const bool ok) {
+#ifdef MUCA_CHECKED
+    if (!ok) atomicOr(rc.flag, CHK_STATE);
+#endif
+}
 
 template <int L>
 struct Geo {

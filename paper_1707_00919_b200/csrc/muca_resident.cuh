@@ -43,7 +43,8 @@ struct V6 {
     static constexpr uint32_t RING_OFF = LAT_OFF + (uint32_t)L * 4u * SLOTS;
     static constexpr uint32_t RING_BYTES = 2u * NC * 16u * SLOTS;
     static constexpr uint32_t SCRATCH_OFF = RING_OFF + RING_BYTES;          // 16 bytes per call and deviate warp (philox_unit)
-    static constexpr size_t SMEM_BYTES = (size_t)SCRATCH_OFF + 16u * NC * MAX_WARPS;
+    static constexpr uint32_t TAG_OFF = SCRATCH_OFF + 16u * NC * MAX_WARPS;   // MUCA_CHECKED build: 2 x MAX_WARPS hand-over tags
+    static constexpr size_t SMEM_BYTES = (size_t)TAG_OFF + 8u * MAX_WARPS;
 };
 
 // Field words of a row: nibble q of FW[r] holds the column f = hl + 2*n3 of site 4q + r (hl: bond to the left
@@ -298,18 +299,23 @@ template <int L, bool MEAS>
 __device__ __forceinline__ void row_v6(uint32_t* __restrict__ lat, uint32_t& S, uint32_t& A, uint32_t& chk, uint32_t& off, uint32_t& g1,
                                        uint32_t& gx1, const int y, const bool more, uint32_t& up, const uint32_t c, uint32_t (&FW)[4],
                                        const uint32_t patch, uint32_t (&rnd)[Geo<L>::BITS], NextRow<L>& n, uint32_t (&FWn)[4],
-                                       const uint4* ring, int& buf, const int bar_id, SitePipe& pp) {
+                                       const uint4* ring, int& buf, const int bar_id, SitePipe& pp, RingCheck& rc) {
     using V = V6<L>;
     constexpr int SLOTS = V::SLOTS;
     // the deviates of row y + 1 are in ring[buf]; ring[buf ^ 1] (this row's, all fetched) may be refilled.  After the
     // last row of a phase there is no such barrier (the deviate warp has left its loop) and nothing is fetched.
-    if (more) pair_barrier(bar_id);
+    if (more) {
+        pair_barrier(bar_id);
+        ring_expect(rc, buf, CHK_RING_EARLY);
+    }
     const int y1 = (y + 1) & (L - 1), y2 = (y + 2) & (L - 1);
     n.c = lat[y1 * SLOTS];
     n.dn = lat[y2 * SLOTS];   // row y + 2 is old (or row 0, final in this sweep, when y + 1 = L - 1)
     uint32_t flips = 0;
     RowSites<L, MEAS, 0, true, true, V::SBASE + V::DT_OFF, true>::run(S, A, flips, chk, off, g1, gx1, c, FW, FW[3], patch, rnd, n, FWn, FWn,
                                                                       ring, SLOTS, buf, more, pp);
+    if (more) ring_fetched(rc, buf);
+    state_check(rc, S >= V::SBASE && S <= V::SBASE + V::BINS * V::RS && (S - V::SBASE) % V::RS == 0u);
     buf ^= (int)more;
     up = c ^ flips;
     lat[y * SLOTS] = up;
@@ -320,7 +326,7 @@ __device__ __forceinline__ void row_v6(uint32_t* __restrict__ lat, uint32_t& S, 
 // processed in pairs so that the two register sets (this row / row below) swap roles without copies.
 template <int L, bool MEAS>
 __device__ __forceinline__ void sweeps_v6(uint32_t* __restrict__ lat, uint32_t& S, uint32_t& chk, const uint32_t s0, const uint32_t s1,
-                                          const uint4* ring, int& buf, const int bar_id) {
+                                          const uint4* ring, int& buf, const int bar_id, RingCheck& rc) {
     using G = Geo<L>;
     using V = V6<L>;
     constexpr int BITS = G::BITS, NC = V::NC, SLOTS = V::SLOTS;
@@ -334,11 +340,13 @@ __device__ __forceinline__ void sweeps_v6(uint32_t* __restrict__ lat, uint32_t& 
 #pragma unroll
     for (int r = 0; r < 4; ++r) FWA[r] = finish_word<L>(nA, up, r);
     pair_barrier(bar_id);                      // the deviates of the first row are in ring[buf]
+    ring_expect(rc, buf, CHK_RING_EARLY);
 #pragma unroll
     for (int k = 0; k < NC; ++k) {
         const uint4 v = ring[(buf * NC + k) * SLOTS];
         rnd[4 * k] = v.x; rnd[4 * k + 1] = v.y; rnd[4 * k + 2] = v.z; rnd[4 * k + 3] = v.w;
     }
+    ring_fetched(rc, buf);
     buf ^= 1;
     uint32_t off = (FWA[0] << 2) & 0x1Cu;      // site 0: its left neighbour (site L-1) has not been visited in this sweep
     uint32_t A = S + off;
@@ -351,9 +359,9 @@ __device__ __forceinline__ void sweeps_v6(uint32_t* __restrict__ lat, uint32_t& 
     for (uint32_t s = s0; s < s1; ++s) {
 #pragma unroll 1
         for (int y = 0; y < L; y += 2) {
-            row_v6<L, MEAS>(lat, S, A, chk, off, g1, gx1, y, true, up, nA.c, FWA, nA.patch, rnd, nB, FWB, ring, buf, bar_id, pp);
+            row_v6<L, MEAS>(lat, S, A, chk, off, g1, gx1, y, true, up, nA.c, FWA, nA.patch, rnd, nB, FWB, ring, buf, bar_id, pp, rc);
             row_v6<L, MEAS>(lat, S, A, chk, off, g1, gx1, y + 1, s + 1 < s1 || y + 2 < L, up, nB.c, FWB, nB.patch, rnd, nA, FWA, ring, buf,
-                            bar_id, pp);
+                            bar_id, pp, rc);
         }
     }
 }
@@ -364,7 +372,8 @@ __device__ __forceinline__ void sweeps_v6(uint32_t* __restrict__ lat, uint32_t& 
 // R4: ctr = (i >> 2, sweep, iteration, walker).
 template <int L>
 __device__ __forceinline__ void deviates_v6(uint4* ring, uint4* scratch, const uint32_t s0, const uint32_t s1, int& buf,
-                                            const int bar_id, const SweepParams& prm, const uint32_t walker, const bool active, const int lane) {
+                                            const int bar_id, const SweepParams& prm, const uint32_t walker, const bool active, const int lane,
+                                            RingCheck& rc) {
     constexpr int NC = V6<L>::NC, SLOTS = V6<L>::SLOTS;
 #pragma unroll 1
     for (uint32_t s = s0; s < s1; ++s) {
@@ -376,6 +385,7 @@ __device__ __forceinline__ void deviates_v6(uint4* ring, uint4* scratch, const u
 #pragma unroll
             for (int k = 0; k < NC; ++k)
                 if (active) ring[(buf * NC + k) * SLOTS] = make_uint4(st[k][0], st[k][1], st[k][2], st[k][3]);
+            ring_publish(rc, buf, lane);
             pair_barrier(bar_id);
             buf ^= 1;
         }
@@ -456,14 +466,21 @@ __global__ void __launch_bounds__(64 * V6<L>::MAX_WARPS, 1) sweep_kernel_v6(cons
     uint32_t S = sbase + (is_walker && active ? (uint32_t)((prm.E[w] + 2 * N) >> 2) : (uint32_t)BINS) * V::RS;
     int buf = 0;
     uint32_t chk = 0;
+    RingCheck rc;
+#ifdef MUCA_CHECKED
+    rc.tags = reinterpret_cast<volatile uint32_t*>(sm + V::TAG_OFF) + pair;
+    rc.stride = V::MAX_WARPS;
+    rc.flag = prm.check;
+    rc.fault = blockIdx.x == 0 && pair == 0 ? prm.fault : 0u;
+#endif
     // ---- thermalisation sweeps: nothing is recorded
-    if (is_walker) sweeps_v6<L, false>(lat, S, chk, prm.sweep_begin, s_th, ring + slot, buf, bar_id);
-    else deviates_v6<L>(ring + slot, scratch, prm.sweep_begin, s_th, buf, bar_id, prm, walker, active, lane);
+    if (is_walker) sweeps_v6<L, false>(lat, S, chk, prm.sweep_begin, s_th, ring + slot, buf, bar_id, rc);
+    else deviates_v6<L>(ring + slot, scratch, prm.sweep_begin, s_th, buf, bar_id, prm, walker, active, lane, rc);
     // ---- measured sweeps: every attempt counts the state it leads to
     if (is_walker) {
-        sweeps_v6<L, true>(lat, S, chk, s_th, prm.sweep_end, ring + slot, buf, bar_id);
+        sweeps_v6<L, true>(lat, S, chk, s_th, prm.sweep_end, ring + slot, buf, bar_id, rc);
     } else {
-        deviates_v6<L>(ring + slot, scratch, s_th, prm.sweep_end, buf, bar_id, prm, walker, active, lane);
+        deviates_v6<L>(ring + slot, scratch, s_th, prm.sweep_end, buf, bar_id, prm, walker, active, lane, rc);
     }
     if (is_walker) {
         if (chk == 0x9E3779B9u && !active) lat[0] = chk;   // keeps the checksum of the site macro alive (never true for a parked lane: its addresses are constant)

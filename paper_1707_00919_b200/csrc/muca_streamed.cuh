@@ -28,7 +28,8 @@ constexpr uint32_t S6_DTA = S6_SBASE; // the delta table sits first: the site ma
 
 __host__ __device__ constexpr size_t s6_ring_bytes(int npairs) { return (size_t)npairs * 2 * 8 * 32 * 16; }
 constexpr uint32_t S6_SCRATCH_OFF = 32, S6_SCRATCH_BYTES = 8 * 8 * 16;   // behind DT: 16 bytes per call and deviate warp (philox_unit)
-constexpr uint32_t S6_RING_OFF = S6_SCRATCH_OFF + S6_SCRATCH_BYTES;
+constexpr uint32_t S6_TAG_OFF = S6_SCRATCH_OFF + S6_SCRATCH_BYTES, S6_TAG_BYTES = 2 * 8 * 4;   // MUCA_CHECKED build: hand-over tags
+constexpr uint32_t S6_RING_OFF = S6_TAG_OFF + S6_TAG_BYTES;
 __host__ __device__ constexpr size_t s6_smem_bytes(int n_rows, int npairs) {
     return S6_RING_OFF + s6_ring_bytes(npairs) + (size_t)(n_rows + 2 * S6_PAD_ROWS) * S6_RS;
 }
@@ -40,7 +41,7 @@ template <int L, bool MEAS>
 __device__ __forceinline__ void sweeps_s6(uint32_t* __restrict__ rows, const size_t row_stride, const bool store, uint32_t& S,
                                           uint32_t& chk, bool& left, const uint32_t win_lo, const uint32_t win_span, const uint32_t s0,
                                           const uint32_t s1, const uint4* ring, const int slots, int& buf,
-                                          const int bar_id) {
+                                          const int bar_id, RingCheck& rc, const uint32_t all_lo, const uint32_t all_span) {
     using G = Geo<L>;
     constexpr int WPR = G::WPR;
     static_assert(G::BITS == 32, "streamed kernel: rows of whole 32-site words");
@@ -63,11 +64,13 @@ __device__ __forceinline__ void sweeps_s6(uint32_t* __restrict__ rows, const siz
         if (k == WPR - 1) patch = n.patch;
     }
     pair_barrier(bar_id);                      // the deviates of the first word are in ring[buf]
+    ring_expect(rc, buf, CHK_RING_EARLY);
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
         const uint4 v = ring[(buf * 8 + q) * slots];
         rnd[4 * q] = v.x; rnd[4 * q + 1] = v.y; rnd[4 * q + 2] = v.z; rnd[4 * q + 3] = v.w;
     }
+    ring_fetched(rc, buf);
     buf ^= 1;
     uint32_t off = (FWc[0][0] << 2) & 0x1Cu;   // site 0: its left neighbour (site L-1) has not been visited in this sweep
     uint32_t A = S + off;
@@ -82,7 +85,10 @@ __device__ __forceinline__ void sweeps_s6(uint32_t* __restrict__ rows, const siz
             for (int k = 0; k < WPR; ++k) {
                 const bool more = more_rows || k + 1 < WPR;
                 // the deviates of the next word are in ring[buf]; ring[buf ^ 1] (this word's, all fetched) may be refilled
-                if (more) pair_barrier(bar_id);
+                if (more) {
+                    pair_barrier(bar_id);
+                    ring_expect(rc, buf, CHK_RING_EARLY);
+                }
                 n.c = R1[k]; n.left = R1[(k + WPR - 1) % WPR]; n.right = R1[(k + 1) % WPR]; n.dn = R2[k];
                 uint32_t flips = 0;
                 if (k == 0 && k == WPR - 1)
@@ -97,6 +103,8 @@ __device__ __forceinline__ void sweeps_s6(uint32_t* __restrict__ rows, const siz
                 else
                     RowSites<L, MEAS, 0, false, false, S6_DTA, false>::run(S, A, flips, chk, off, g1, gx1, R0[k], FWc[k], FWc[WPR - 1][3], patch, rnd, n,
                                                                     FWn[k], FWc[(k + 1) % WPR], ring, slots, buf, more, pp);
+                if (more) ring_fetched(rc, buf);
+                state_check(rc, S - all_lo < all_span && (S - all_lo) % S6_RS == 0u);   // a row of the window, its sentinels or its pads
                 buf ^= (int)more;
                 R0[k] ^= flips;
                 FWn[k][3] = finish_word<L>(n, R0[k], 3);
@@ -120,7 +128,8 @@ __device__ __forceinline__ void sweeps_s6(uint32_t* __restrict__ rows, const siz
 // 0xFFFFFFFF for good).  One barrier per word hands the buffer over.  R4: ctr = (i >> 2, sweep, iteration, walker).
 template <int L>
 __device__ __forceinline__ void deviates_s6(uint4* ring, uint4* scratch, const int slots, int& buf, const int bar_id, const uint32_t s0,
-                                            const uint32_t s1, const SweepParams& prm, const uint32_t walker, const bool active, const int lane) {
+                                            const uint32_t s1, const SweepParams& prm, const uint32_t walker, const bool active, const int lane,
+                                            RingCheck& rc) {
     constexpr int WPR = Geo<L>::WPR;
 #pragma unroll 1
     for (uint32_t s = s0; s < s1; ++s) {
@@ -132,6 +141,7 @@ __device__ __forceinline__ void deviates_s6(uint4* ring, uint4* scratch, const i
 #pragma unroll
             for (int q = 0; q < 8; ++q)
                 if (active) ring[(buf * 8 + q) * slots] = make_uint4(st[q][0], st[q][1], st[q][2], st[q][3]);
+            ring_publish(rc, buf, lane);
             pair_barrier(bar_id);
             buf ^= 1;
         }
@@ -197,12 +207,20 @@ sweep_kernel_s6(const SweepParams prm, const int j_lo, const int n_rows, const i
     uint32_t chk = 0;
     bool left = false;
     const int bar_id = 1 + pair;
+    RingCheck rc;
+#ifdef MUCA_CHECKED
+    rc.tags = reinterpret_cast<volatile uint32_t*>(sm + S6_TAG_OFF) + pair;
+    rc.stride = 8;
+    rc.flag = prm.check;
+    rc.fault = blockIdx.x == 0 && pair == 0 ? prm.fault : 0u;
+#endif
+    const uint32_t all_lo = o_base - S6_PAD_ROWS * S6_RS, all_span = (uint32_t)(n_rows + 2 * S6_PAD_ROWS) * S6_RS;
     if (is_walker) {
-        sweeps_s6<L, false>(rows, row_stride, active, S, chk, left, win_lo, win_span, prm.sweep_begin, s_th, ring, slots, buf, bar_id);
+        sweeps_s6<L, false>(rows, row_stride, active, S, chk, left, win_lo, win_span, prm.sweep_begin, s_th, ring, slots, buf, bar_id, rc, all_lo, all_span);
         // measured sweeps: every site counts the state it starts from, so the state before the first measured attempt
         // is taken out again here and the state after the last one is added below
         if (s_th < prm.sweep_end) atomicSub(reinterpret_cast<uint32_t*>(sm + (S - S6_SBASE) + S6_BIN_OFF), 1u);
-        sweeps_s6<L, true>(rows, row_stride, active, S, chk, left, win_lo, win_span, s_th, prm.sweep_end, ring, slots, buf, bar_id);
+        sweeps_s6<L, true>(rows, row_stride, active, S, chk, left, win_lo, win_span, s_th, prm.sweep_end, ring, slots, buf, bar_id, rc, all_lo, all_span);
         if (s_th < prm.sweep_end) atomicAdd(reinterpret_cast<uint32_t*>(sm + (S - S6_SBASE) + S6_BIN_OFF), 1u);
         if (chk == 0x9E3779B9u && !active) ring[0] = make_uint4(chk, chk, chk, chk);   // keeps the checksum of the site macro alive (never true for a parked lane: its addresses are constant)
         if (active) {
@@ -210,8 +228,8 @@ sweep_kernel_s6(const SweepParams prm, const int j_lo, const int n_rows, const i
             if (left) atomicOr(overflow, 1);
         }
     } else {
-        deviates_s6<L>(ring, scratch, slots, buf, bar_id, prm.sweep_begin, s_th, prm, walker, active, lane);
-        deviates_s6<L>(ring, scratch, slots, buf, bar_id, s_th, prm.sweep_end, prm, walker, active, lane);
+        deviates_s6<L>(ring, scratch, slots, buf, bar_id, prm.sweep_begin, s_th, prm, walker, active, lane, rc);
+        deviates_s6<L>(ring, scratch, slots, buf, bar_id, s_th, prm.sweep_end, prm, walker, active, lane, rc);
     }
     __syncthreads();
     // ---- a4: merge the bins of the real rows into the global uint64 histogram
