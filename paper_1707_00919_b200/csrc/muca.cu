@@ -627,7 +627,10 @@ int muca_run_iteration_random_site(muca_ctx* ctx, uint64_t therm_updates, uint64
     expand_table8(t5, ctx->n_bins, ctx->h_table);
     CU(cudaMemcpyAsync(ctx->d_table, ctx->h_table, (size_t)ctx->n_bins * 8 * 4, cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaMemsetAsync(ctx->d_H, 0, (size_t)ctx->n_bins * 8, ctx->stream));
-    const int tpb = ctx->L == 128 ? 32 : 128;                                     // 64 KiB of lattice words per block at L >= 64
+    // one block per SM where the walkers allow it; the lattice words of a block's walkers must fit beside table and bins
+    const int tpb_max = ctx->L <= 32 ? 512 : ctx->L == 64 ? 256 : 64;
+    int tpb = ((ctx->W + ctx->n_sm - 1) / ctx->n_sm + 31) / 32 * 32;
+    if (tpb > tpb_max) tpb = tpb_max;
     RandomSiteParams prm;
     prm.spins = ctx->d_spins; prm.E = ctx->d_E; prm.table = ctx->d_table; prm.H = ctx->d_H;
     prm.W = ctx->W; prm.walker_offset = ctx->walker_offset;

@@ -4,9 +4,17 @@
 // DESIGN.md R22: update u of iteration n proposes site i_u = word (u & 3) of Philox(ctr = (u >> 2 mod 2^32, u >> 34,
 // n, 0xFFFFFFFF), key) mod N; global walker g accepts iff word (u & 3) of Philox(ctr = (u >> 2 mod 2^32, u >> 34, n, g),
 // key) <= thresh[j][a].  Work is counted in updates (attempted flips per walker), the paper's own unit.
-// Straightforward kernel (not the tuned path): one thread per walker, lattice words and bins in shared memory
-// (lat[word * tpb + tid]: the site is warp-uniform, so every access is conflict-free -- the paper's coalescing
-// argument), thresholds through L1, Philox in the thread.
+// One thread per walker.  Shared memory (L <= 64): the threshold table as rows of 5 words thresh[j][a] (odd stride:
+// consecutive rows rotate through all banks), the bins, the lattice words (lat[word * tpb + tid]: the site is
+// warp-uniform, so every lattice access is conflict-free -- the paper's coalescing argument) and, for the
+// next RS_CHUNK updates, a DESCRIPTOR of the update that the block computes once for all its walkers: the shared site
+// stream (one Philox call gives four sites) turned into the five (word offset, bit) pairs of the site and its
+// neighbours, plus a flag saying whether the update touches the word the update before may have changed.  So a thread
+// does no index arithmetic at all, and -- the sites of successive updates being the same for all walkers and rarely
+// adjacent -- it fetches the neighbourhood of update u + 1 BEFORE it decides update u unless that flag is set (a
+// warp-uniform branch): the per-update chain is   j -> LDS thresh[j][a] -> compare -> j'   as in the typewriter kernels.
+// The acceptance deviates come from one Philox call per four updates in the walker's thread.  At L = 128 the table
+// (320 KB) does not fit: thresholds are read through L1 there.
 #pragma once
 #include "muca_device.cuh"
 
@@ -22,57 +30,170 @@ struct RandomSiteParams {
     unsigned long long u_begin, u_end, therm;   // updates [u_begin, u_end); updates with index < therm are not recorded
 };
 
+constexpr int RS_CHUNK = 256;     // updates described ahead, per block
+
+template <int L>
+struct RandomSite {
+    static constexpr int N = L * L, BINS = N + 1, NW = N / 32;
+    static constexpr bool TBL_SMEM = L <= 64;
+    static constexpr int TBL_WORDS = TBL_SMEM ? ((BINS * 5 + 3) & ~3) : 0;
+    static constexpr int BIN_WORDS = (BINS + 3) & ~3;
+    static constexpr int DESC_WORDS = 8 * (RS_CHUNK + 2);      // two uint4 per update + two entries behind the chunk
+    static constexpr int SITE_WORDS = RS_CHUNK + 4;            // the sites of the chunk, [0] = last site of the chunk before
+    __host__ __device__ static constexpr size_t smem_bytes(int tpb) {
+        return ((size_t)TBL_WORDS + BIN_WORDS + DESC_WORDS + SITE_WORDS + (size_t)NW * tpb) * 4;
+    }
+};
+
+// The five lattice words of an update as loaded (RsWords) and what the decision needs from them (RsHood).  Loading and
+// evaluating are two steps so that the threshold load of the update before can be issued between them: a warp issues
+// in order, and the evaluation would otherwise wait for the words in front of that load.
+struct RsWords { uint32_t wc, wr, wl, wd, wu; };
+struct RsHood { uint32_t a, wc, addr_c, mask; };
+
+// descriptor word p = (byte offset of the lattice word in this thread's column << 5) | bit
+__device__ __forceinline__ RsWords rs_load(const char* lat, const uint4 d0, const uint4 d1) {
+    RsWords r;
+    r.wc = *reinterpret_cast<const volatile uint32_t*>(lat + (d0.x >> 5));
+    r.wr = *reinterpret_cast<const volatile uint32_t*>(lat + (d0.y >> 5));
+    r.wl = *reinterpret_cast<const volatile uint32_t*>(lat + (d0.z >> 5));
+    r.wd = *reinterpret_cast<const volatile uint32_t*>(lat + (d0.w >> 5));
+    r.wu = *reinterpret_cast<const volatile uint32_t*>(lat + (d1.x >> 5));
+    return r;
+}
+__device__ __forceinline__ RsHood rs_eval(const RsWords& r, const uint4 d0, const uint4 d1) {
+    const uint32_t s = __funnelshift_r(r.wc, r.wc, d0.x);       // rotate by the low 5 bits: bit 0 = the spin
+    RsHood h;
+    h.a = ((__funnelshift_r(r.wr, r.wr, d0.y) ^ s) & 1u) + ((__funnelshift_r(r.wl, r.wl, d0.z) ^ s) & 1u) +
+          ((__funnelshift_r(r.wd, r.wd, d0.w) ^ s) & 1u) + ((__funnelshift_r(r.wu, r.wu, d1.x) ^ s) & 1u);   // antiparallel neighbours
+    h.wc = r.wc;
+    h.addr_c = d0.x >> 5;
+    h.mask = 1u << (d0.x & 31u);
+    return h;
+}
+
+// Updates k .. k + 3 of the chunk (one acceptance call).  MEAS: 0 = none of the four is recorded, 1 = all are,
+// 2 = the group straddles the begin / end of the launch or the end of the thermalisation (k0, k1, kth decide per update).
+// In: cur = neighbourhood of update k, (d0, d1) = descriptor of update k + 1.  Per update: the words of the NEXT update
+// are loaded at once, then the threshold of this one, then the descriptor of the update after the next; only then is
+// anything evaluated -- three independent loads in flight, one round trip per update.  If the next update touches the
+// word this one may change (flag in its descriptor, warp-uniform, ~5 / number of words of the time) its words are
+// loaded again behind the store.
+template <int L, int MEAS>
+__device__ __forceinline__ void rs_group(char* lat, const uint4* desc, const uint32_t* tbl, uint32_t* bins, const RandomSiteParams& prm,
+                                         const int k, const int k0, const int k1, const int kth, const uint32_t (&ra)[4], int& j, RsHood& cur,
+                                         uint4& d0, uint4& d1) {
+    constexpr bool TBL_SMEM = RandomSite<L>::TBL_SMEM;
+#pragma unroll
+    for (int m = 0; m < 4; ++m) {
+        RsWords nw = rs_load(lat, d0, d1);
+        const bool live = MEAS != 2 || (k + m >= k0 && k + m < k1);
+        uint32_t t = 0u;
+        if (live) t = TBL_SMEM ? *reinterpret_cast<const volatile uint32_t*>(tbl + 5 * j + (int)cur.a)
+                               : __ldg(prm.table + (size_t)j * 8 + (cur.a ? 2u * cur.a - 1u : 0u));
+        const uint4 e0 = desc[2 * (k + m) + 4], e1 = desc[2 * (k + m) + 5];   // descriptor of update k + m + 2 (two dummies behind the chunk)
+        RsHood nxt = rs_eval(nw, d0, d1);
+        if (live) {
+            if (ra[m] <= t) {                                                // R6/R7
+                *reinterpret_cast<volatile uint32_t*>(lat + cur.addr_c) = cur.wc ^ cur.mask;
+                j += 2 - (int)cur.a;                                         // dE = 8 - 4a
+            }
+            if (MEAS == 1 || (MEAS == 2 && k + m >= kth)) atomicAdd(bins + j, 1u);   // H[j]++ after EVERY measured attempt
+        }
+        if (d1.y != 0u) {                                                    // warp-uniform
+            nw = rs_load(lat, d0, d1);
+            nxt = rs_eval(nw, d0, d1);
+        }
+        cur = nxt; d0 = e0; d1 = e1;
+    }
+}
+
 template <int L>
 __global__ void random_site_kernel(const RandomSiteParams prm) {
-    constexpr int N = L * L, BINS = N + 1, NW = N / 32;
+    using R = RandomSite<L>;
+    constexpr int N = R::N, BINS = R::BINS, NW = R::NW;
+    constexpr int LOG_L = L == 8 ? 3 : L == 16 ? 4 : L == 32 ? 5 : L == 64 ? 6 : 7;
     extern __shared__ __align__(16) uint32_t smem[];
     const int tid = threadIdx.x, tpb = blockDim.x;
     const int w = blockIdx.x * tpb + tid;
     const bool active = w < prm.W;
-    uint32_t* const bins = smem;
-    uint32_t* const lat = smem + ((BINS + 3) & ~3) + tid;      // typewriter word t of this walker at lat[t * tpb]
+    uint32_t* const tbl = smem;                                 // thresh[j][a] at tbl[5 j + a]
+    uint32_t* const bins = smem + R::TBL_WORDS;
+    uint4* const desc = reinterpret_cast<uint4*>(bins + R::BIN_WORDS);
+    uint32_t* const sites = bins + R::BIN_WORDS + R::DESC_WORDS;
+    uint32_t* const latw = sites + R::SITE_WORDS + tid;         // typewriter word t of this walker at latw[t * tpb]
+    char* const lat = reinterpret_cast<char*>(latw);
+    if (R::TBL_SMEM)
+        for (int idx = tid; idx < BINS * 5; idx += tpb) {
+            const int j = idx / 5, a = idx - 5 * j;
+            tbl[idx] = prm.table[j * 8 + (a ? 2 * a - 1 : 0)];   // a column of T8 with a(f) = a
+        }
     for (int j = tid; j < BINS; j += tpb) bins[j] = 0u;
+    if (tid == 0) {
+        sites[0] = 0xFFFFFFFFu;                                 // no update before the first one of this launch
+        for (int e = 0; e < 2; ++e) {                           // the entries behind the chunk: word 0, "load again"
+            desc[2 * (RS_CHUNK + e)] = make_uint4(0u, 0u, 0u, 0u);
+            desc[2 * (RS_CHUNK + e) + 1] = make_uint4(0u, 1u, 0u, 0u);
+        }
+    }
     if (active)
-        for (int t = 0; t < NW; ++t) lat[t * tpb] = prm.spins[word_index(L, prm.W, w, t)];
-    __syncthreads();
-    if (active) {
-        int j = (prm.E[w] + 2 * N) >> 2;                       // slot
-        const uint32_t g = prm.walker_offset + (uint32_t)w;
-        uint32_t rs[4] = {0, 0, 0, 0}, ra[4] = {0, 0, 0, 0};
-        for (unsigned long long u = prm.u_begin; u < prm.u_end; ++u) {
-            if ((u & 3ull) == 0ull || u == prm.u_begin) {
-                const uint32_t c0 = (uint32_t)((u >> 2) & 0xFFFFFFFFull), c1 = (uint32_t)(u >> 34);
-                philox4x32_10(c0, c1, prm.iteration, 0xFFFFFFFFu, prm.key0, prm.key1, rs);   // site stream, shared by all walkers
-                philox4x32_10(c0, c1, prm.iteration, g, prm.key0, prm.key1, ra);             // acceptance stream of this walker
-            }
-            const int i = (int)(rs[u & 3ull] & (uint32_t)(N - 1));   // mod N, N a power of two
-            const int x = i & (L - 1), y = i / L;
+        for (int t = 0; t < NW; ++t) latw[t * tpb] = prm.spins[word_index(L, prm.W, w, t)];
+    int j = active ? (prm.E[w] + 2 * N) >> 2 : 0;              // slot
+    const uint32_t g = prm.walker_offset + (uint32_t)w;
+    for (unsigned long long u0 = prm.u_begin & ~3ull; u0 < prm.u_end; u0 += RS_CHUNK) {   // chunks start at a multiple of 4
+        __syncthreads();                                        // the descriptors of the chunk before have been used
+        for (int c = tid; c < RS_CHUNK / 4; c += tpb) {         // site stream, shared by all walkers (R22): one call gives 4 sites
+            const unsigned long long uc = u0 + 4ull * c;
+            uint32_t rs[4];
+            philox4x32_10((uint32_t)((uc >> 2) & 0xFFFFFFFFull), (uint32_t)(uc >> 34), prm.iteration, 0xFFFFFFFFu, prm.key0, prm.key1, rs);
+#pragma unroll
+            for (int m = 0; m < 4; ++m) sites[1 + 4 * c + m] = rs[m] & (uint32_t)(N - 1);   // mod N, N a power of two
+        }
+        __syncthreads();
+        for (int k = tid; k < RS_CHUNK; k += tpb) {             // descriptors
+            const int i = (int)sites[1 + k];
+            const int x = i & (L - 1), y = i >> LOG_L;
             const int ir = y * L + ((x + 1) & (L - 1)), il = y * L + ((x + L - 1) & (L - 1));
             const int id = ((y + 1) & (L - 1)) * L + x, iu = ((y + L - 1) & (L - 1)) * L + x;
-            const uint32_t wc = lat[(i >> 5) * tpb];
-            const uint32_t s = (wc >> (i & 31)) & 1u;
-            const uint32_t a = (((lat[(ir >> 5) * tpb] >> (ir & 31)) & 1u) ^ s) + (((lat[(il >> 5) * tpb] >> (il & 31)) & 1u) ^ s) +
-                               (((lat[(id >> 5) * tpb] >> (id & 31)) & 1u) ^ s) + (((lat[(iu >> 5) * tpb] >> (iu & 31)) & 1u) ^ s);
-            const uint32_t f = a ? 2u * a - 1u : 0u;             // a column of T8 with a(f) = a
-            const uint32_t t = __ldg(prm.table + (size_t)j * 8 + f);
-            if (ra[u & 3ull] <= t) {                             // R6/R7
-                lat[(i >> 5) * tpb] = wc ^ (1u << (i & 31));
-                j += 2 - (int)a;                                 // dE = 8 - 4a
-            }
-            if (u >= prm.therm) atomicAdd(bins + j, 1u);        // H[j]++ after EVERY measured attempt
+            auto pk = [&](int s) { return (uint32_t)(((s >> 5) * tpb * 4) << 5) | (uint32_t)(s & 31); };
+            const uint32_t prev = sites[k];                     // the site of the update before (0xFFFFFFFF: none)
+            const uint32_t pw = prev >> 5;                      // the word it may have changed
+            const bool hazard = prev == 0xFFFFFFFFu || pw == (uint32_t)(i >> 5) || pw == (uint32_t)(ir >> 5) || pw == (uint32_t)(il >> 5) ||
+                                pw == (uint32_t)(id >> 5) || pw == (uint32_t)(iu >> 5);
+            desc[2 * k] = make_uint4(pk(i), pk(ir), pk(il), pk(id));
+            desc[2 * k + 1] = make_uint4(pk(iu), hazard ? 1u : 0u, 0u, 0u);
         }
+        __syncthreads();
+        if (tid == 0) sites[0] = sites[RS_CHUNK];               // read again only behind the next barrier
+        if (!active) continue;
+        // the chunk in 32-bit numbers: updates k0 .. k1-1 of it belong to this launch, those from kth on are recorded
+        const int k0 = prm.u_begin > u0 ? (int)(prm.u_begin - u0) : 0;
+        const int k1 = prm.u_end - u0 < (unsigned long long)RS_CHUNK ? (int)(prm.u_end - u0) : RS_CHUNK;
+        const int kth = prm.therm <= u0 ? 0 : (prm.therm - u0 < (unsigned long long)RS_CHUNK ? (int)(prm.therm - u0) : RS_CHUNK);
+        RsHood cur = rs_eval(rs_load(lat, desc[0], desc[1]), desc[0], desc[1]);   // the first update of a chunk: fetched behind the store before it
+        uint4 d0 = desc[2], d1 = desc[3];
+        for (int k = 0; k < k1; k += 4) {
+            uint32_t ra[4];   // acceptance stream of this walker: one call per four updates
+            const unsigned long long u = u0 + (unsigned long long)k;
+            philox4x32_10((uint32_t)((u >> 2) & 0xFFFFFFFFull), (uint32_t)(u >> 34), prm.iteration, g, prm.key0, prm.key1, ra);
+            if (k >= k0 && k + 4 <= k1 && k >= kth) rs_group<L, 1>(lat, desc, tbl, bins, prm, k, k0, k1, kth, ra, j, cur, d0, d1);
+            else if (k >= k0 && k + 4 <= k1 && k + 4 <= kth) rs_group<L, 0>(lat, desc, tbl, bins, prm, k, k0, k1, kth, ra, j, cur, d0, d1);
+            else rs_group<L, 2>(lat, desc, tbl, bins, prm, k, k0, k1, kth, ra, j, cur, d0, d1);
+        }
+    }
+    if (active) {
         prm.E[w] = 4 * j - 2 * N;
-        for (int t = 0; t < NW; ++t) prm.spins[word_index(L, prm.W, w, t)] = lat[t * tpb];
+        for (int t = 0; t < NW; ++t) prm.spins[word_index(L, prm.W, w, t)] = latw[t * tpb];
     }
     __syncthreads();
     if (prm.u_end > prm.therm)
-        for (int j = tid; j < BINS; j += tpb)
-            if (bins[j]) atomicAdd(prm.H + j, (unsigned long long)bins[j]);
+        for (int jj = tid; jj < BINS; jj += tpb)
+            if (bins[jj]) atomicAdd(prm.H + jj, (unsigned long long)bins[jj]);
 }
 
 template <int L>
 __host__ __device__ constexpr size_t random_site_smem_bytes(int tpb) {
-    return ((size_t)((L * L + 1 + 3) & ~3) + (size_t)(L * L / 32) * tpb) * 4;
+    return RandomSite<L>::smem_bytes(tpb);
 }
 
 }  // namespace muca
