@@ -82,11 +82,16 @@ __device__ __forceinline__ RsHood rs_eval(const RsWords& r, const uint4 d0, cons
 template <int L, int MEAS>
 __device__ __forceinline__ void rs_group(char* lat, const uint4* desc, const uint32_t* tbl, uint32_t* bins, const RandomSiteParams& prm,
                                          const int k, const int k0, const int k1, const int kth, const uint32_t (&ra)[4], int& j, RsHood& cur,
-                                         uint4& d0, uint4& d1) {
+                                         uint4& d0, uint4& d1, uint32_t (&st)[4]) {
     constexpr bool TBL_SMEM = RandomSite<L>::TBL_SMEM;
 #pragma unroll
     for (int m = 0; m < 4; ++m) {
         RsWords nw = rs_load(lat, d0, d1);
+        // the acceptance call of the NEXT four updates, 3 + 2 + 3 + 2 of its ten rounds per update, behind the loads: a call
+        // is one dependent chain of wide multiplies, which a warp that issues in order cannot hide when it comes as a block
+#pragma unroll
+        for (int r = (m >> 1) * 5 + (m & 1) * 3; r < (m >> 1) * 5 + (m & 1) * 3 + ((m & 1) ? 2 : 3); ++r)
+            philox_round(st, prm.key0 + (uint32_t)r * 0x9E3779B9u, prm.key1 + (uint32_t)r * 0xBB67AE85u);
         const bool live = MEAS != 2 || (k + m >= k0 && k + m < k1);
         uint32_t t = 0u;
         if (live) t = TBL_SMEM ? *reinterpret_cast<const volatile uint32_t*>(tbl + 5 * j + (int)cur.a)
@@ -172,13 +177,17 @@ __global__ void random_site_kernel(const RandomSiteParams prm) {
         const int kth = prm.therm <= u0 ? 0 : (prm.therm - u0 < (unsigned long long)RS_CHUNK ? (int)(prm.therm - u0) : RS_CHUNK);
         RsHood cur = rs_eval(rs_load(lat, desc[0], desc[1]), desc[0], desc[1]);   // the first update of a chunk: fetched behind the store before it
         uint4 d0 = desc[2], d1 = desc[3];
+        // acceptance stream of this walker (R22): one call per four updates; the call of the first group of the chunk here,
+        // the call of every further group inside the group before it (rs_group)
+        uint32_t st[4];
+        philox4x32_10((uint32_t)((u0 >> 2) & 0xFFFFFFFFull), (uint32_t)(u0 >> 34), prm.iteration, g, prm.key0, prm.key1, st);
         for (int k = 0; k < k1; k += 4) {
-            uint32_t ra[4];   // acceptance stream of this walker: one call per four updates
-            const unsigned long long u = u0 + (unsigned long long)k;
-            philox4x32_10((uint32_t)((u >> 2) & 0xFFFFFFFFull), (uint32_t)(u >> 34), prm.iteration, g, prm.key0, prm.key1, ra);
-            if (k >= k0 && k + 4 <= k1 && k >= kth) rs_group<L, 1>(lat, desc, tbl, bins, prm, k, k0, k1, kth, ra, j, cur, d0, d1);
-            else if (k >= k0 && k + 4 <= k1 && k + 4 <= kth) rs_group<L, 0>(lat, desc, tbl, bins, prm, k, k0, k1, kth, ra, j, cur, d0, d1);
-            else rs_group<L, 2>(lat, desc, tbl, bins, prm, k, k0, k1, kth, ra, j, cur, d0, d1);
+            const uint32_t ra[4] = {st[0], st[1], st[2], st[3]};
+            const unsigned long long un = u0 + (unsigned long long)k + 4ull;   // counter of the next group
+            st[0] = (uint32_t)((un >> 2) & 0xFFFFFFFFull); st[1] = (uint32_t)(un >> 34); st[2] = prm.iteration; st[3] = g;
+            if (k >= k0 && k + 4 <= k1 && k >= kth) rs_group<L, 1>(lat, desc, tbl, bins, prm, k, k0, k1, kth, ra, j, cur, d0, d1, st);
+            else if (k >= k0 && k + 4 <= k1 && k + 4 <= kth) rs_group<L, 0>(lat, desc, tbl, bins, prm, k, k0, k1, kth, ra, j, cur, d0, d1, st);
+            else rs_group<L, 2>(lat, desc, tbl, bins, prm, k, k0, k1, kth, ra, j, cur, d0, d1, st);
         }
     }
     if (active) {
