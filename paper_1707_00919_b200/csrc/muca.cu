@@ -3,6 +3,7 @@
 // There is NO CPU fallback: every compute entry point needs a CUDA device and fails with MUCA_ECUDA otherwise.
 #include "../../include/muca.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -56,6 +57,11 @@ struct muca_ctx {
     int* h_flag = nullptr;          // pinned copy (tail of h_H's allocation)
     int stat_window_iterations = 0, stat_window_fallbacks = 0;
     int win_margin = 8;             // rows asked for between the outermost walker and a sentinel; grows after a fallback
+    int* d_perm = nullptr;          // sorted-window launches: walker served by position i of the launch (in the workspace, L >= 32)
+    int* d_blk_jlo = nullptr;       // ... and the first table row of every block's window
+    unsigned long long* d_Hsnap = nullptr;   // ... and the histogram as it was before the launch
+    int32_t* h_E = nullptr;         // pinned: energies, then the permutation and the window starts (3 W ints)
+    int stat_sorted_launches = 0;
     int conv_w_prev = 0;            // width covered by the previous iteration of muca_converge (0: none yet)
     double conv_n_updates = 0.0;    // N_updates (flips per walker) of the previous iteration of muca_converge
     int opt_scheme = MUCA_SCHEME_TYPEWRITER;   // update scheme used by muca_converge / muca_production
@@ -73,7 +79,7 @@ inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 bool valid_L(int L) { return L == 8 || L == 16 || L == 32 || L == 64 || L == 128; }
 
-struct Carve { size_t spins, E, table, H, flag, snap, stage, total; };
+struct Carve { size_t spins, E, table, H, flag, snap, perm, blkwin, hsnap, stage, total; };
 Carve carve(int L, int W) {
     const size_t N = (size_t)L * L, bins = N + 1;
     Carve c;
@@ -84,6 +90,9 @@ Carve carve(int L, int W) {
     c.H = off;     off += align_up(bins * 8);
     c.flag = off;  off += align_up(4 * sizeof(int));                       // windowed kernels: left-the-window flag, slot range
     c.snap = off;  off += L >= 32 ? align_up((size_t)W * (N / 8)) + align_up((size_t)W * 4) : 0;   // and their snapshot of spins + E
+    c.perm = off;  off += L >= 32 ? align_up((size_t)W * 4) : 0;           // sorted-window launches (L >= 32): permutation,
+    c.blkwin = off; off += L >= 32 ? align_up((size_t)((W + 31) / 32) * 4) : 0;   // window start per block,
+    c.hsnap = off; off += L >= 32 ? align_up(bins * 8) : 0;                 // histogram before the launch
     c.stage = off; off += align_up((size_t)W * N);                        // int8 spins of muca_get_spins / muca_set_spins
     c.total = off;
     return c;
@@ -248,22 +257,23 @@ size_t plan_smem(int L, const Plan& p) {
 struct Window { int j_lo = 0, n_rows = 0, sent_lo = 0, sent_hi = 0; };
 
 template <int L>
-int launch_s6_t(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& win) {
+int launch_s6_t(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& win, bool sorted) {
     const int npairs = tpb / 32;
     if (npairs < 1 || npairs > s6_max_pairs(L)) return fail(ctx, MUCA_EINVAL, "paired streamed kernel: 1 to %d warp pairs per block at L = %d", s6_max_pairs(L), L);
     const size_t smem = s6_smem_bytes(win.n_rows, npairs);
     SMEM((sweep_kernel_s6<L>), smem);
     sweep_kernel_s6<L><<<(prm.W + tpb - 1) / tpb, 2 * tpb, smem, ctx->stream>>>(prm, win.j_lo, win.n_rows, win.sent_lo, win.sent_hi,
-                                                                               ctx->opt_role_map, ctx->d_flag);
+                                                                               ctx->opt_role_map, ctx->d_flag, sorted ? ctx->d_perm : nullptr,
+                                                                               sorted ? ctx->d_blk_jlo : nullptr);
     CU(cudaGetLastError());
     return MUCA_OK;
 }
 
-int launch_s6(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& win) {
+int launch_s6(muca_ctx* ctx, const SweepParams& prm, int tpb, const Window& win, bool sorted = false) {
     switch (ctx->L) {
-        case 32: return launch_s6_t<32>(ctx, prm, tpb, win);
-        case 64: return launch_s6_t<64>(ctx, prm, tpb, win);
-        case 128: return launch_s6_t<128>(ctx, prm, tpb, win);
+        case 32: return launch_s6_t<32>(ctx, prm, tpb, win, sorted);
+        case 64: return launch_s6_t<64>(ctx, prm, tpb, win, sorted);
+        case 128: return launch_s6_t<128>(ctx, prm, tpb, win, sorted);
     }
     return fail(ctx, MUCA_EINVAL, "paired streamed kernel: L must be 32, 64 or 128");
 }
@@ -341,6 +351,9 @@ int create_common(muca_ctx** out, int L, int W, uint64_t seed, uint32_t walker_o
     ctx->d_flag = (int*)(base + c.flag);
     ctx->d_stage = (void*)(base + c.stage);
     ctx->d_snap = L >= 32 ? (void*)(base + c.snap) : nullptr;
+    ctx->d_perm = L >= 32 ? (int*)(base + c.perm) : nullptr;
+    ctx->d_blk_jlo = L >= 32 ? (int*)(base + c.blkwin) : nullptr;
+    ctx->d_Hsnap = L >= 32 ? (unsigned long long*)(base + c.hsnap) : nullptr;
     ctx->logw.assign(ctx->n_bins, 0.0);   // R2: omega == 0
     ctx->H.assign(ctx->n_bins, 0);
     ctx->h_table = (uint32_t*)pinned_pool().get(pinned_table_bytes(ctx->n_bins));
@@ -421,6 +434,7 @@ void muca_destroy(muca_ctx* ctx) {
     if (ctx->stream || ctx->d_workspace) cudaStreamSynchronize(ctx->stream);
     pinned_pool().put(pinned_table_bytes(ctx->n_bins), ctx->h_table);
     pinned_pool().put(pinned_hist_bytes(ctx->n_bins), ctx->h_H);
+    pinned_pool().put((size_t)ctx->W * 12, ctx->h_E);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
 
@@ -508,6 +522,7 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
     fallback.mode = MODE_L1; fallback.tpb = l1_default_tpb(ctx); fallback.nw = fallback.wpw = 0;
     Window win;
     bool guarded = false;   // the window has sentinel rows: the result counts only if no walker entered one
+    bool sorted = false;    // one window per block over walkers sorted by energy, a few sweeps per launch (run_sorted below)
     const bool windowed_plan = plan.mode == MODE_S6;
     if (windowed_plan) {
         const size_t spin_bytes = (size_t)ctx->W * (ctx->N / 8);
@@ -528,7 +543,8 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
         if (cap >= ctx->n_bins) {
             win.j_lo = 0; win.n_rows = ctx->n_bins;                          // the whole table fits: nothing to guard
         } else if (hi - lo + 1 + 2 * (2 + margin) > cap) {
-            plan = fallback;                                                  // the walkers are spread too widely
+            sorted = true;                                                    // the walkers are spread too widely for ONE window
+            win.n_rows = cap;
         } else {
             int j_lo = lo - (cap - (hi - lo + 1)) / 2;
             if (j_lo < 0) j_lo = 0;
@@ -540,7 +556,7 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
             CU(cudaMemcpyAsync(ctx->d_snap, ctx->d_spins, spin_bytes, cudaMemcpyDeviceToDevice, ctx->stream));
             CU(cudaMemcpyAsync((char*)ctx->d_snap + align_up(spin_bytes), ctx->d_E, (size_t)ctx->W * 4, cudaMemcpyDeviceToDevice, ctx->stream));
         }
-        if (plan.mode != MODE_L1) ctx->stat_window_iterations += 1;
+        if (plan.mode != MODE_L1 && !sorted) ctx->stat_window_iterations += 1;
     }
 
     // a2-a4: sweeps.  A block's uint32 bins must not overflow: tpb * measured sweeps * N < 2^32 per launch.
@@ -573,9 +589,85 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
         }
         return MUCA_OK;
     };
+    // Walkers spread over more table rows than shared memory holds (L = 128 once the weights have spread them: the regime of
+    // every production run): the iteration is cut into launches of a few sweeps.  Before each one the walkers are sorted by
+    // energy on the host (8192 energies: a D2H copy and a sort, ~0.3 ms against milliseconds of sweeps), every block is
+    // handed neighbours in energy and a window of its own around them, and spins, energies and histogram are copied aside;
+    // a launch that a walker left through a sentinel is undone and repeated with the plain kernel.  The number of sweeps per
+    // launch follows from the rows left between a block's walkers and its sentinels: a sweep moves a walker by about
+    // sqrt(3 N / 4) slots (N attempts, every second one accepted, mean squared step 1.5), and 6 sigma must fit.
+    auto run_sorted = [&]() -> int {
+        const int W = ctx->W, tpb = plan.tpb, n_blocks = (W + tpb - 1) / tpb, cap = win.n_rows;
+        const size_t spin_bytes = (size_t)W * (ctx->N / 8);
+        if (!ctx->h_E) ctx->h_E = (int32_t*)pinned_pool().get((size_t)W * 12);
+        if (!ctx->h_E) return fail(ctx, MUCA_ECUDA, "pinned allocation failed");
+        int32_t* const h_perm = ctx->h_E + W;
+        int32_t* const h_jlo = ctx->h_E + 2 * W;
+        std::vector<int> order(W);
+        const uint64_t max_meas = std::max<uint64_t>(1, 0xFFFFFFFFull / ((uint64_t)tpb * (uint64_t)ctx->N));
+        const double sigma1 = std::sqrt(0.75 * (double)ctx->N);
+        bool any_window = false;
+        uint64_t s = 0;
+        while (s < total) {
+            CU(cudaMemcpyAsync(ctx->h_E, ctx->d_E, (size_t)W * 4, cudaMemcpyDeviceToHost, ctx->stream));
+            CU(cudaStreamSynchronize(ctx->stream));
+            for (int i = 0; i < W; ++i) order[i] = i;
+            std::sort(order.begin(), order.end(), [&](int a, int b) { return ctx->h_E[a] != ctx->h_E[b] ? ctx->h_E[a] < ctx->h_E[b] : a < b; });
+            int room = cap;   // rows between a block's walkers and its sentinels, smallest over the blocks
+            for (int b = 0; b < n_blocks; ++b) {
+                const int i0 = b * tpb, i1 = std::min(W, i0 + tpb) - 1;
+                const int lo_b = (ctx->h_E[order[i0]] + 2 * ctx->N) >> 2, hi_b = (ctx->h_E[order[i1]] + 2 * ctx->N) >> 2;
+                int j_lo = lo_b - (cap - (hi_b - lo_b + 1)) / 2;
+                if (j_lo < 0) j_lo = 0;
+                if (j_lo + cap > ctx->n_bins) j_lo = ctx->n_bins - cap;
+                h_jlo[b] = j_lo;
+                const int below = j_lo > 0 ? lo_b - j_lo - 2 : cap, above = j_lo + cap < ctx->n_bins ? j_lo + cap - 1 - hi_b - 2 : cap;
+                room = std::min(room, std::min(below, above));
+            }
+            for (int i = 0; i < W; ++i) h_perm[i] = order[i];
+            uint64_t e = total;
+            const uint64_t meas_begin = s > (uint64_t)therm_sweeps ? s : (uint64_t)therm_sweeps;
+            if (e > meas_begin + max_meas) e = meas_begin + max_meas;
+            if (ctx->opt_max_sweeps > 0 && e > s + (uint64_t)ctx->opt_max_sweeps) e = s + (uint64_t)ctx->opt_max_sweeps;
+            const double k = room > ctx->win_margin ? (double)room / (6.0 * sigma1) : 0.0;
+            uint64_t chunk = (uint64_t)(k * k);
+            if (chunk > 64) chunk = 64;
+            prm.sweep_begin = (uint32_t)s;
+            if (chunk >= 1) {
+                if (e > s + chunk) e = s + chunk;
+                prm.sweep_end = (uint32_t)e;
+                CU(cudaMemcpyAsync(ctx->d_perm, h_perm, (size_t)W * 4, cudaMemcpyHostToDevice, ctx->stream));
+                CU(cudaMemcpyAsync(ctx->d_blk_jlo, h_jlo, (size_t)n_blocks * 4, cudaMemcpyHostToDevice, ctx->stream));
+                CU(cudaMemcpyAsync(ctx->d_snap, ctx->d_spins, spin_bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+                CU(cudaMemcpyAsync((char*)ctx->d_snap + align_up(spin_bytes), ctx->d_E, (size_t)W * 4, cudaMemcpyDeviceToDevice, ctx->stream));
+                CU(cudaMemcpyAsync(ctx->d_Hsnap, ctx->d_H, (size_t)ctx->n_bins * 8, cudaMemcpyDeviceToDevice, ctx->stream));
+                CU(cudaMemsetAsync(ctx->d_flag, 0, sizeof(int), ctx->stream));
+                const int rc = launch_s6(ctx, prm, tpb, win, true);
+                if (rc != MUCA_OK) return rc;
+                ++launches; ctx->stat_sorted_launches += 1; any_window = true;
+                CU(cudaMemcpyAsync(ctx->h_flag, ctx->d_flag, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+                CU(cudaStreamSynchronize(ctx->stream));
+                if (!ctx->h_flag[0]) { s = e; continue; }
+                // a walker left its block's window: undo the launch
+                CU(cudaMemcpyAsync(ctx->d_spins, ctx->d_snap, spin_bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+                CU(cudaMemcpyAsync(ctx->d_E, (char*)ctx->d_snap + align_up(spin_bytes), (size_t)W * 4, cudaMemcpyDeviceToDevice, ctx->stream));
+                CU(cudaMemcpyAsync(ctx->d_H, ctx->d_Hsnap, (size_t)ctx->n_bins * 8, cudaMemcpyDeviceToDevice, ctx->stream));
+                ctx->stat_window_fallbacks += 1;
+            } else {
+                if (e > s + 4) e = s + 4;   // no room for a window now: a few sweeps with the plain kernel, then look again
+            }
+            prm.sweep_end = (uint32_t)e;
+            const int rc = launch_sweep(ctx, prm, fallback);
+            if (rc != MUCA_OK) return rc;
+            ++launches;
+            s = e;
+        }
+        if (any_window) ctx->stat_window_iterations += 1;
+        return MUCA_OK;
+    };
     CU(cudaEventRecord(ctx->ev0, ctx->stream));
     {
-        const int rc = run_sweeps(plan);
+        const int rc = sorted ? run_sorted() : run_sweeps(plan);
         if (rc != MUCA_OK) return rc;
     }
     if (plan.mode == MODE_S6 && guarded) {

@@ -153,8 +153,8 @@ __device__ __forceinline__ void deviates_s6(uint4* ring, uint4* scratch, const i
 // walker warps share schedulers with walker warps; role_map 1: walker and deviate warps alternate on every scheduler.
 template <int L>
 __global__ void __launch_bounds__(64 * s6_max_pairs(L), 1)
-sweep_kernel_s6(const SweepParams prm, const int j_lo, const int n_rows, const int sent_lo, const int sent_hi, const int role_map,
-                int* __restrict__ overflow) {
+sweep_kernel_s6(const SweepParams prm, const int j_lo_all, const int n_rows, const int sent_lo_all, const int sent_hi_all, const int role_map,
+                int* __restrict__ overflow, const int* __restrict__ perm, const int* __restrict__ blk_j_lo) {
     using G = Geo<L>;
     constexpr int WPR = G::WPR, N = G::N;
     extern __shared__ __align__(16) uint32_t smem[];
@@ -166,8 +166,15 @@ sweep_kernel_s6(const SweepParams prm, const int j_lo, const int n_rows, const i
     // the warp among the warps of its role
     const int pair = role_map == 0 ? warp_id >> 1 : ((warp_id >> 2) << 1) | ((warp_id & 3) >> 1);
     const int slot = 32 * pair + lane, slots = 32 * npairs;
-    const int w = blockIdx.x * slots + slot;
-    const bool active = w < prm.W;
+    // Walkers are independent and identified by their GLOBAL id (R16), so which block serves which walker is free: with
+    // `perm` the host hands every block walkers of neighbouring energies (sorted) and a table window of its own
+    // (blk_j_lo[block]) -- the way the window keeps up with walkers that are spread over the whole energy range.
+    const int idx = blockIdx.x * slots + slot;
+    const bool active = idx < prm.W;
+    const int w = perm ? perm[active ? idx : prm.W - 1] : idx;
+    const int j_lo = blk_j_lo ? blk_j_lo[blockIdx.x] : j_lo_all;
+    const int sent_lo = blk_j_lo ? (j_lo > 0 ? 2 : 0) : sent_lo_all;
+    const int sent_hi = blk_j_lo ? (j_lo + n_rows < N + 1 ? 2 : 0) : sent_hi_all;
     if ((uint32_t)__cvta_generic_to_shared(smem) != S6_SBASE) __trap();   // the site macro addresses the delta table by an immediate
     uint4* const ring = reinterpret_cast<uint4*>(sm + S6_RING_OFF) + slot;
     uint4* const scratch = reinterpret_cast<uint4*>(sm + S6_SCRATCH_OFF) + pair * 8;
@@ -197,7 +204,7 @@ sweep_kernel_s6(const SweepParams prm, const int j_lo, const int n_rows, const i
                           : (prm.therm > prm.sweep_end ? prm.sweep_end : prm.therm);
     // Lanes without a walker take part in the pair barriers of their warp, so they run the same code: they read the
     // rows of the last walker and store nothing.
-    const int wl = active ? w : prm.W - 1;
+    const int wl = active ? w : (perm ? w : prm.W - 1);
     uint32_t* rows = prm.spins + (size_t)wl * WPR;
     const size_t row_stride = (size_t)prm.W * WPR;
     const uint32_t walker = prm.walker_offset + (uint32_t)w;

@@ -253,6 +253,44 @@ def test_windowed_table_and_fallback(L, W, rows, iters, therm, sweeps, expect_fa
         g.close(); o.close()
 
 
+# Walkers spread over more table rows than the window holds (L = 128 in every production run): the library sorts the
+# walkers by energy, gives every block a window of its own and cuts the iteration into launches of a few sweeps
+# (muca.cu run_sorted).  Here: L = 32 with a forced 600-row window and exact flat-histogram weights, L = 64 with 1500 rows
+# and omega = 0 (walkers leave their windows: launches are undone and repeated), walkers started all over the energy range.
+@pytest.mark.parametrize("L,W,rows,sweeps", [(32, 200, 600, 8), (64, 150, 1500, 6)])
+def test_sorted_windows_for_widely_spread_walkers(L, W, rows, sweeps):
+    import os
+    N = L * L
+    rng = np.random.default_rng(5)
+    p = np.linspace(0.0, 0.5, W)[:, None]                       # walker k: a fraction p_k of its spins down -> E from -2N up to ~0
+    spins = np.where(rng.random((W, N)) < p, -1, 1).astype(np.int8)
+    if L == 32:                                                 # every second walker times a checkerboard: E -> -E, up to +2N
+        yy, xx = np.divmod(np.arange(N), L)
+        spins[1::2] *= np.where((xx + yy) % 2 == 0, 1, -1).astype(np.int8)[None, :]
+    g, o = mb.Muca(L, W, PRIMARY_SEED, walker_offset=9), mo.Oracle(L, W, PRIMARY_SEED, walker_offset=9)
+    try:
+        g.set_spins(spins); o.set_spins(spins)
+        if L == 32:                                             # omega = -ln g: every walker diffuses slowly from where it starts
+            with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "ising_dos_L32.txt")) as f:
+                gE = [int(x) for x in f if not x.startswith("#")]
+            import mpmath as mp
+            w = np.array([-float(mp.log(v)) if v > 0 else 0.0 for v in gE])
+            g.set_log_weights(w); o.set_log_weights(w)
+        g.set_option(B.MUCA_OPT_KERNEL, B.MUCA_KERNEL_STREAMED_PAIRS)
+        g.set_option(B.MUCA_OPT_TABLE_WINDOW_ROWS, rows)
+        E0 = g.get_energies()
+        assert (E0.max() - E0.min()) // 4 > rows                # one window cannot hold them
+        for it in range(3):
+            Hg, Ho = g.run_iteration(2, sweeps), o.run_iteration(2, sweeps, n_threads=mo.max_threads())
+            assert np.array_equal(Hg, Ho), f"it{it}: H differs in slots {np.nonzero(Hg != Ho)[0][:8]}"
+            compare_state(g, o, f"it{it}")
+            g.update_weights(); o.update_weights()
+        windowed, undone = g.window_stats()
+        assert windowed > 0, (windowed, undone)                 # launches with per-block windows did run
+    finally:
+        g.close(); o.close()
+
+
 def test_split_launches_give_the_same_iteration():
     # an iteration split into several launches (the uint32-bin overflow guard) is the same Markov chain
     run_pair(32, 70, PRIMARY_SEED, 3, 3, 9, options=((B.MUCA_OPT_MAX_SWEEPS_PER_LAUNCH, 2),))
