@@ -57,8 +57,10 @@ typedef enum muca_status {
  *   RESIDENT       (L <= 32) lattices, threshold table and histogram in shared memory, Philox in paired deviate warps;
  *   STREAMED_PAIRS (L >= 32) table and histogram in shared memory, lattice rows streamed from HBM / L2, Philox in paired
  *                  deviate warps.  At L = 128 the table no longer fits: shared memory then holds a WINDOW of it around
- *                  the walkers' energies; an iteration in which a walker leaves the window is detected and repeated
- *                  from a snapshot with STREAMED -- same results (muca_window_stats() counts both);
+ *                  the walkers' energies (one window for all walkers while they fit into it, otherwise one per block
+ *                  over walkers sorted by energy, a few sweeps per launch); a launch in which a walker leaves its window
+ *                  is detected, undone from a snapshot and repeated with STREAMED -- same results
+ *                  (muca_window_stats() counts both);
  *   STREAMED       (L >= 32) thresholds read through L1, histogram in shared memory, lattice rows streamed, Philox in the
  *                  walker thread: the plain kernel and the fallback of the window.
  * A variant that does not exist for the context's L is replaced by the one AUTO would pick. */
@@ -243,8 +245,10 @@ int muca_get_thresholds(muca_ctx* ctx, uint32_t* out, size_t n);
 int muca_get_iteration(muca_ctx* ctx, uint32_t* n_out);
 int muca_set_iteration(muca_ctx* ctx, uint32_t n);
 int muca_last_sweep_ms(muca_ctx* ctx, double* ms_out, int* launches_out);
-/* windowed STREAMED_SMEM kernel: iterations run with a table window so far, and how many of them were repeated
- * with STREAMED because a walker left the window. */
+/* STREAMED_PAIRS kernel with a table window (L = 128, or MUCA_OPT_TABLE_WINDOW_ROWS): iterations in which at least one
+ * launch ran with a window so far, and launches that a walker left through a sentinel row and that were therefore undone
+ * and repeated with the plain STREAMED kernel (same results either way).  Walkers spread over more rows than one window
+ * holds are sorted by energy and served with one window per block, a few sweeps per launch. */
 int muca_window_stats(muca_ctx* ctx, int* windowed_iterations_out, int* fallbacks_out);
 const char* muca_last_error(const muca_ctx* ctx);
 

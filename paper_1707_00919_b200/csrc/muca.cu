@@ -517,7 +517,7 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
     const uint64_t total = (uint64_t)therm_sweeps + (uint64_t)sweeps;
     if (total > 0xFFFFFFFFull) return fail(ctx, MUCA_EINVAL, "too many sweeps");
 
-    // windowed table (muca_window.cuh): pick the window around the walkers' slots, keep a snapshot for the fallback
+    // windowed table (muca_streamed.cuh): pick the window around the walkers' slots, keep a snapshot for the fallback
     Plan fallback;
     fallback.mode = MODE_L1; fallback.tpb = l1_default_tpb(ctx); fallback.nw = fallback.wpw = 0;
     Window win;
