@@ -720,9 +720,18 @@ int muca_run_iteration_random_site(muca_ctx* ctx, uint64_t therm_updates, uint64
     CU(cudaMemcpyAsync(ctx->d_table, ctx->h_table, (size_t)ctx->n_bins * 8 * 4, cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaMemsetAsync(ctx->d_H, 0, (size_t)ctx->n_bins * 8, ctx->stream));
     // one block per SM where the walkers allow it; the lattice words of a block's walkers must fit beside table and bins
-    const int tpb_max = ctx->L <= 32 ? 512 : ctx->L == 64 ? 256 : 64;
+    auto rs_smem = [&](int t) -> size_t {
+        switch (ctx->L) {
+            case 8: return random_site_smem_bytes<8>(t);
+            case 16: return random_site_smem_bytes<16>(t);
+            case 32: return random_site_smem_bytes<32>(t);
+            case 64: return random_site_smem_bytes<64>(t);
+            default: return random_site_smem_bytes<128>(t);
+        }
+    };
     int tpb = ((ctx->W + ctx->n_sm - 1) / ctx->n_sm + 31) / 32 * 32;
-    if (tpb > tpb_max) tpb = tpb_max;
+    if (tpb > 512) tpb = 512;
+    while (tpb > 32 && rs_smem(tpb) > (size_t)ctx->max_smem_optin) tpb -= 32;
     RandomSiteParams prm;
     prm.spins = ctx->d_spins; prm.E = ctx->d_E; prm.table = ctx->d_table; prm.H = ctx->d_H;
     prm.W = ctx->W; prm.walker_offset = ctx->walker_offset;

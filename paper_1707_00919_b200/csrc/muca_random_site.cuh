@@ -36,8 +36,13 @@ template <int L>
 struct RandomSite {
     static constexpr int N = L * L, BINS = N + 1, NW = N / 32;
     static constexpr bool TBL_SMEM = L <= 64;
-    static constexpr int TBL_WORDS = TBL_SMEM ? ((BINS * 5 + 3) & ~3) : 0;
-    static constexpr int BIN_WORDS = (BINS + 3) & ~3;
+    // L <= 32: rows of thresh[j][0..4] | bin of slot j | pad (7 words, odd stride: all banks): threshold and bin are one
+    // add away from the row address.  L = 64: rows of 5 thresholds and the bins apart (beside 208 walkers' lattices a
+    // 7-word table would not fit).  L = 128: bins only.
+    static constexpr bool BIN_IN_ROW = L <= 32;
+    static constexpr int ROW_WORDS = BIN_IN_ROW ? 7 : 5;
+    static constexpr int TBL_WORDS = TBL_SMEM ? ((BINS * ROW_WORDS + 3) & ~3) : 0;
+    static constexpr int BIN_WORDS = BIN_IN_ROW ? 0 : ((BINS + 3) & ~3);
     static constexpr int DESC_WORDS = 8 * (RS_CHUNK + 2);      // two uint4 per update + two entries behind the chunk
     static constexpr int SITE_WORDS = RS_CHUNK + 4;            // the sites of the chunk, [0] = last site of the chunk before
     __host__ __device__ static constexpr size_t smem_bytes(int tpb) {
@@ -49,14 +54,19 @@ struct RandomSite {
 // evaluating are two steps so that the threshold load of the update before can be issued between them: a warp issues
 // in order, and the evaluation would otherwise wait for the words in front of that load.
 struct RsWords { uint32_t wc, wr, wl, wd, wu; };
-struct RsHood { uint32_t a, wc, addr_c, mask; };
+struct RsHood { uint32_t a, wc, addr_c, mask; };   // mask: bit of the site in its word (from the descriptor)
 
 // descriptor word p = (byte offset of the lattice word in this thread's column << 5) | bit
+template <int L>
 __device__ __forceinline__ RsWords rs_load(const char* lat, const uint4 d0, const uint4 d1) {
     RsWords r;
     r.wc = *reinterpret_cast<const volatile uint32_t*>(lat + (d0.x >> 5));
-    r.wr = *reinterpret_cast<const volatile uint32_t*>(lat + (d0.y >> 5));
-    r.wl = *reinterpret_cast<const volatile uint32_t*>(lat + (d0.z >> 5));
+    if constexpr (L <= 32) {   // a row lies within one word: left and right neighbour are bits of the site's own word
+        r.wr = r.wc; r.wl = r.wc;
+    } else {
+        r.wr = *reinterpret_cast<const volatile uint32_t*>(lat + (d0.y >> 5));
+        r.wl = *reinterpret_cast<const volatile uint32_t*>(lat + (d0.z >> 5));
+    }
     r.wd = *reinterpret_cast<const volatile uint32_t*>(lat + (d0.w >> 5));
     r.wu = *reinterpret_cast<const volatile uint32_t*>(lat + (d1.x >> 5));
     return r;
@@ -68,7 +78,7 @@ __device__ __forceinline__ RsHood rs_eval(const RsWords& r, const uint4 d0, cons
           ((__funnelshift_r(r.wd, r.wd, d0.w) ^ s) & 1u) + ((__funnelshift_r(r.wu, r.wu, d1.x) ^ s) & 1u);   // antiparallel neighbours
     h.wc = r.wc;
     h.addr_c = d0.x >> 5;
-    h.mask = 1u << (d0.x & 31u);
+    h.mask = d1.z;
     return h;
 }
 
@@ -83,30 +93,32 @@ template <int L, int MEAS>
 __device__ __forceinline__ void rs_group(char* lat, const uint4* desc, const uint32_t* tbl, uint32_t* bins, const RandomSiteParams& prm,
                                          const int k, const int k0, const int k1, const int kth, const uint32_t (&ra)[4], int& j, RsHood& cur,
                                          uint4& d0, uint4& d1, uint32_t (&st)[4]) {
-    constexpr bool TBL_SMEM = RandomSite<L>::TBL_SMEM;
+    constexpr bool TBL_SMEM = RandomSite<L>::TBL_SMEM, BIN_IN_ROW = RandomSite<L>::BIN_IN_ROW;
 #pragma unroll
     for (int m = 0; m < 4; ++m) {
-        RsWords nw = rs_load(lat, d0, d1);
+        RsWords nw = rs_load<L>(lat, d0, d1);
         // the acceptance call of the NEXT four updates, 3 + 2 + 3 + 2 of its ten rounds per update, behind the loads: a call
         // is one dependent chain of wide multiplies, which a warp that issues in order cannot hide when it comes as a block
 #pragma unroll
         for (int r = (m >> 1) * 5 + (m & 1) * 3; r < (m >> 1) * 5 + (m & 1) * 3 + ((m & 1) ? 2 : 3); ++r)
             philox_round(st, prm.key0 + (uint32_t)r * 0x9E3779B9u, prm.key1 + (uint32_t)r * 0xBB67AE85u);
         const bool live = MEAS != 2 || (k + m >= k0 && k + m < k1);
-        uint32_t t = 0u;
-        if (live) t = TBL_SMEM ? *reinterpret_cast<const volatile uint32_t*>(tbl + 5 * j + (int)cur.a)
+        uint32_t t = 0u;   // BIN_IN_ROW: j is the BYTE offset of the walker's table row (28 j), so that threshold and bin need one add
+        if (live) t = BIN_IN_ROW ? *reinterpret_cast<const volatile uint32_t*>(reinterpret_cast<const char*>(tbl) + j + 4 * (int)cur.a)
+                    : TBL_SMEM ? *reinterpret_cast<const volatile uint32_t*>(tbl + 5 * j + (int)cur.a)
                                : __ldg(prm.table + (size_t)j * 8 + (cur.a ? 2u * cur.a - 1u : 0u));
         const uint4 e0 = desc[2 * (k + m) + 4], e1 = desc[2 * (k + m) + 5];   // descriptor of update k + m + 2 (two dummies behind the chunk)
         RsHood nxt = rs_eval(nw, d0, d1);
         if (live) {
             if (ra[m] <= t) {                                                // R6/R7
                 *reinterpret_cast<volatile uint32_t*>(lat + cur.addr_c) = cur.wc ^ cur.mask;
-                j += 2 - (int)cur.a;                                         // dE = 8 - 4a
+                j += (BIN_IN_ROW ? 4 * RandomSite<L>::ROW_WORDS : 1) * (2 - (int)cur.a);   // dE = 8 - 4a
             }
-            if (MEAS == 1 || (MEAS == 2 && k + m >= kth)) atomicAdd(bins + j, 1u);   // H[j]++ after EVERY measured attempt
+            if (MEAS == 1 || (MEAS == 2 && k + m >= kth))                    // H[j]++ after EVERY measured attempt
+                atomicAdd(BIN_IN_ROW ? reinterpret_cast<uint32_t*>(reinterpret_cast<char*>(bins) + j + 20) : bins + j, 1u);
         }
         if (d1.y != 0u) {                                                    // warp-uniform
-            nw = rs_load(lat, d0, d1);
+            nw = rs_load<L>(lat, d0, d1);
             nxt = rs_eval(nw, d0, d1);
         }
         cur = nxt; d0 = e0; d1 = e1;
@@ -122,18 +134,20 @@ __global__ void random_site_kernel(const RandomSiteParams prm) {
     const int tid = threadIdx.x, tpb = blockDim.x;
     const int w = blockIdx.x * tpb + tid;
     const bool active = w < prm.W;
-    uint32_t* const tbl = smem;                                 // thresh[j][a] at tbl[5 j + a]
-    uint32_t* const bins = smem + R::TBL_WORDS;
-    uint4* const desc = reinterpret_cast<uint4*>(bins + R::BIN_WORDS);
-    uint32_t* const sites = bins + R::BIN_WORDS + R::DESC_WORDS;
+    uint32_t* const tbl = smem;                                 // row j: thresh[j][0..4] | bin | pad
+    uint32_t* const bins = R::BIN_IN_ROW ? smem : smem + R::TBL_WORDS;   // BIN_IN_ROW: bin of slot j at tbl[7 j + 5]
+    uint4* const desc = reinterpret_cast<uint4*>(smem + R::TBL_WORDS + R::BIN_WORDS);
+    uint32_t* const sites = smem + R::TBL_WORDS + R::BIN_WORDS + R::DESC_WORDS;
     uint32_t* const latw = sites + R::SITE_WORDS + tid;         // typewriter word t of this walker at latw[t * tpb]
     char* const lat = reinterpret_cast<char*>(latw);
-    if (R::TBL_SMEM)
-        for (int idx = tid; idx < BINS * 5; idx += tpb) {
-            const int j = idx / 5, a = idx - 5 * j;
-            tbl[idx] = prm.table[j * 8 + (a ? 2 * a - 1 : 0)];   // a column of T8 with a(f) = a
+    if (R::TBL_SMEM) {
+        for (int idx = tid; idx < BINS * R::ROW_WORDS; idx += tpb) {
+            const int j = idx / R::ROW_WORDS, a = idx - R::ROW_WORDS * j;
+            tbl[idx] = a < 5 ? prm.table[j * 8 + (a ? 2 * a - 1 : 0)] : 0u;   // a column of T8 with a(f) = a; bin and pad: 0
         }
-    for (int j = tid; j < BINS; j += tpb) bins[j] = 0u;
+    }
+    if (!R::BIN_IN_ROW)
+        for (int j = tid; j < BINS; j += tpb) bins[j] = 0u;
     if (tid == 0) {
         sites[0] = 0xFFFFFFFFu;                                 // no update before the first one of this launch
         for (int e = 0; e < 2; ++e) {                           // the entries behind the chunk: word 0, "load again"
@@ -143,7 +157,8 @@ __global__ void random_site_kernel(const RandomSiteParams prm) {
     }
     if (active)
         for (int t = 0; t < NW; ++t) latw[t * tpb] = prm.spins[word_index(L, prm.W, w, t)];
-    int j = active ? (prm.E[w] + 2 * N) >> 2 : 0;              // slot
+    constexpr int JS = R::BIN_IN_ROW ? 4 * R::ROW_WORDS : 1;   // j is kept times JS (rs_group)
+    int j = active ? ((prm.E[w] + 2 * N) >> 2) * JS : 0;       // slot
     const uint32_t g = prm.walker_offset + (uint32_t)w;
     for (unsigned long long u0 = prm.u_begin & ~3ull; u0 < prm.u_end; u0 += RS_CHUNK) {   // chunks start at a multiple of 4
         __syncthreads();                                        // the descriptors of the chunk before have been used
@@ -166,7 +181,7 @@ __global__ void random_site_kernel(const RandomSiteParams prm) {
             const bool hazard = prev == 0xFFFFFFFFu || pw == (uint32_t)(i >> 5) || pw == (uint32_t)(ir >> 5) || pw == (uint32_t)(il >> 5) ||
                                 pw == (uint32_t)(id >> 5) || pw == (uint32_t)(iu >> 5);
             desc[2 * k] = make_uint4(pk(i), pk(ir), pk(il), pk(id));
-            desc[2 * k + 1] = make_uint4(pk(iu), hazard ? 1u : 0u, 0u, 0u);
+            desc[2 * k + 1] = make_uint4(pk(iu), hazard ? 1u : 0u, 1u << (i & 31), 0u);
         }
         __syncthreads();
         if (tid == 0) sites[0] = sites[RS_CHUNK];               // read again only behind the next barrier
@@ -175,7 +190,7 @@ __global__ void random_site_kernel(const RandomSiteParams prm) {
         const int k0 = prm.u_begin > u0 ? (int)(prm.u_begin - u0) : 0;
         const int k1 = prm.u_end - u0 < (unsigned long long)RS_CHUNK ? (int)(prm.u_end - u0) : RS_CHUNK;
         const int kth = prm.therm <= u0 ? 0 : (prm.therm - u0 < (unsigned long long)RS_CHUNK ? (int)(prm.therm - u0) : RS_CHUNK);
-        RsHood cur = rs_eval(rs_load(lat, desc[0], desc[1]), desc[0], desc[1]);   // the first update of a chunk: fetched behind the store before it
+        RsHood cur = rs_eval(rs_load<L>(lat, desc[0], desc[1]), desc[0], desc[1]);   // the first update of a chunk: fetched behind the store before it
         uint4 d0 = desc[2], d1 = desc[3];
         // acceptance stream of this walker (R22): one call per four updates; the call of the first group of the chunk here,
         // the call of every further group inside the group before it (rs_group)
@@ -191,13 +206,15 @@ __global__ void random_site_kernel(const RandomSiteParams prm) {
         }
     }
     if (active) {
-        prm.E[w] = 4 * j - 2 * N;
+        prm.E[w] = 4 * (j / JS) - 2 * N;
         for (int t = 0; t < NW; ++t) prm.spins[word_index(L, prm.W, w, t)] = latw[t * tpb];
     }
     __syncthreads();
     if (prm.u_end > prm.therm)
-        for (int jj = tid; jj < BINS; jj += tpb)
-            if (bins[jj]) atomicAdd(prm.H + jj, (unsigned long long)bins[jj]);
+        for (int jj = tid; jj < BINS; jj += tpb) {
+            const uint32_t v = R::BIN_IN_ROW ? tbl[jj * R::ROW_WORDS + 5] : bins[jj];
+            if (v) atomicAdd(prm.H + jj, (unsigned long long)v);
+        }
 }
 
 template <int L>
