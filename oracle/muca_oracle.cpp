@@ -23,6 +23,9 @@
 //   invariants         -> tracked E == recomputed E, sum H = W*sweeps*N, forbidden slots empty
 //   random-site scheme -> omega == 0 closed form (site stream recomputed from the pinned Philox, H replayed in
 //                         numpy), canonical weights against exact g(E) at L = 4   (tests/test_random_site.py)
+//   fp32 acceptance    -> exp32 against mpmath (2 ulp), uniform32 against cuRAND's host generator (its uniform floats
+//                         from the same raw words), canonical weights against exact g(E) at L = 4, threshold and fp32
+//                         chains identical where every weight difference is 0 or -infinity-like   (tests/test_random_site.py)
 // No function here is "parity unpinned".
 
 #include <cmath>
@@ -247,6 +250,79 @@ void run_walker_random_site(const Oracle& o, int w, uint64_t therm, uint64_t upd
     E_io = E;
 }
 
+// ---------------------------------------------------------------------------
+// Single-precision acceptance of the paper's own scheme (SURVEY 8(f)3 "optionally"; "We store the
+// weights in single precision and hence also use a single precision version of the exponential function ... To ensure
+// identical results between the CPU and GPU versions of the code, the example code provided does not use the hardware
+// version __expf()").  Reading R23: omega_f[j] = (float) omega[j]; a proposal j -> j' = j + 2 - a with a != 2 is
+// accepted iff D = omega_f[j'] - omega_f[j] (one fp32 subtraction) >= 0 or U < exp32(D), where
+//   U        = fma32(fl32(x), 2^-32, 2^-33) in (0, 1]: the Philox word x mapped as cuRAND's curand_uniform does;
+//   exp32(D) = the fixed sequence of IEEE fp32 operations below (so that CPU and GPU agree bit for bit, the paper's own
+//              requirement; libm's expf differs between host and device): 0 for D < -24 (exp(-24) < 2^-33 <= U: such
+//              a move is never accepted), else n = rint(D * log2 e), r = D - n ln 2 in two fma steps, a degree-6
+//              Taylor polynomial of exp(r) in Horner form with fma, times 2^n.
+// a == 2 (dE = 0) is always accepted (R9); j' outside [0, N] cannot occur and is rejected.
+// ---------------------------------------------------------------------------
+float uniform32(uint32_t x) { return fmaf((float)x, 2.3283064365386963e-10f, 1.1641532182693481e-10f); }
+
+float exp32(float d) {
+    if (d < -24.0f) return 0.0f;
+    const float t = d * 1.4426950408889634f;          // log2(e), one fp32 product
+    const long n = lrintf(t);                          // round to nearest even (default rounding mode)
+    const float fn = (float)n;
+    float r = fmaf(fn, -0.693145751953125f, d);        // ln 2 split: high part has 13 significant bits, n * hi is exact
+    r = fmaf(fn, -1.428606765330187e-06f, r);
+    float p = 1.0f / 720.0f;
+    p = fmaf(p, r, 1.0f / 120.0f);
+    p = fmaf(p, r, 1.0f / 24.0f);
+    p = fmaf(p, r, 1.0f / 6.0f);
+    p = fmaf(p, r, 0.5f);
+    p = fmaf(p, r, 1.0f);
+    p = fmaf(p, r, 1.0f);
+    uint32_t bits = (uint32_t)(n + 127) << 23;         // 2^n, n in [-35, 0]
+    float s;
+    std::memcpy(&s, &bits, 4);
+    return p * s;
+}
+
+void run_walker_random_site_expf(const Oracle& o, int w, uint64_t therm, uint64_t updates, const float* wf,
+                                 int8_t* s, int32_t& E_io, uint64_t* H) {
+    const int L = o.L, N = o.N;
+    const uint32_t key[2] = {(uint32_t)(o.seed & 0xFFFFFFFFu), (uint32_t)(o.seed >> 32)};
+    const uint32_t g = o.walker_offset + (uint32_t)w;
+    int E = E_io;
+    uint32_t rs[4] = {0, 0, 0, 0}, ra[4] = {0, 0, 0, 0};
+    for (uint64_t u = 0; u < therm + updates; ++u) {
+        if ((u & 3) == 0) {                            // the two streams of R22
+            const uint32_t cs[4] = {(uint32_t)((u >> 2) & 0xFFFFFFFFu), (uint32_t)(u >> 34), o.iteration, 0xFFFFFFFFu};
+            const uint32_t ca[4] = {(uint32_t)((u >> 2) & 0xFFFFFFFFu), (uint32_t)(u >> 34), o.iteration, g};
+            philox4x32_10(cs, key, rs);
+            philox4x32_10(ca, key, ra);
+        }
+        const int i = (int)(rs[u & 3] % (uint32_t)N);
+        const int x = i % L, y = i / L;
+        const int here = s[i];
+        const int nb[4] = {s[y * L + (x + 1) % L], s[y * L + (x + L - 1) % L], s[((y + 1) % L) * L + x],
+                           s[((y + L - 1) % L) * L + x]};
+        int a = 0;
+        for (int k = 0; k < 4; ++k) a += (nb[k] != here);
+        const int j = slot_of(E, N), jn = j + 2 - a;
+        bool accept;
+        if (a == 2) accept = true;
+        else if (jn < 0 || jn > N) accept = false;
+        else {
+            const float D = wf[jn] - wf[j];
+            accept = D >= 0.0f || uniform32(ra[u & 3]) < exp32(D);
+        }
+        if (accept) {
+            s[i] = (int8_t)(-here);
+            E += 8 - 4 * a;
+        }
+        if (u >= therm) H[slot_of(E, N)] += 1;
+    }
+    E_io = E;
+}
+
 }  // namespace
 
 // ---------------------------------------------------------------------------
@@ -355,6 +431,39 @@ int oracle_run_iteration_random_site(void* h, uint64_t therm_updates, uint64_t u
 #endif
         run_walker_random_site(*o, w, therm_updates, updates, thresh.data(), &o->spin[(size_t)w * o->N], o->E[w],
                                Hpriv[t].data());
+    }
+    for (int j = 0; j < n_bins; ++j) {
+        uint64_t sum = 0;
+        for (int t = 0; t < n_threads; ++t) sum += Hpriv[t][j];
+        o->H[j] = sum;
+        H_out[j] = sum;
+    }
+    o->iteration += 1;
+    return 0;
+}
+
+float oracle_exp32(float d) { return exp32(d); }
+float oracle_uniform32(uint32_t x) { return uniform32(x); }
+
+int oracle_run_iteration_random_site_expf(void* h, uint64_t therm_updates, uint64_t updates, uint64_t* H_out, int n_bins,
+                                          int n_threads) {
+    Oracle* o = (Oracle*)h;
+    if (n_bins != o->N + 1) return -1;
+    if (o->iteration == 0xFFFFFFFFu) return -2;
+    std::vector<float> wf(n_bins);
+    for (int j = 0; j < n_bins; ++j) wf[j] = (float)o->logw[j];   // R23: weights stored in single precision
+    if (n_threads < 1) n_threads = 1;
+    std::vector<std::vector<uint64_t>> Hpriv(n_threads, std::vector<uint64_t>(n_bins, 0));
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) num_threads(n_threads)
+#endif
+    for (int w = 0; w < o->W; ++w) {
+        int t = 0;
+#ifdef _OPENMP
+        t = omp_get_thread_num();
+#endif
+        run_walker_random_site_expf(*o, w, therm_updates, updates, wf.data(), &o->spin[(size_t)w * o->N], o->E[w],
+                                    Hpriv[t].data());
     }
     for (int j = 0; j < n_bins; ++j) {
         uint64_t sum = 0;

@@ -44,6 +44,11 @@ def lib():
         L.oracle_get_log_weights.argtypes = [C.c_void_p, f64p, C.c_int]
         L.oracle_run_iteration.argtypes = [C.c_void_p, C.c_int, C.c_int, u64p, C.c_int, C.c_int]
         L.oracle_run_iteration_random_site.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, u64p, C.c_int, C.c_int]
+        L.oracle_run_iteration_random_site_expf.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, u64p, C.c_int, C.c_int]
+        L.oracle_exp32.argtypes = [C.c_float]
+        L.oracle_exp32.restype = C.c_float
+        L.oracle_uniform32.argtypes = [C.c_uint32]
+        L.oracle_uniform32.restype = C.c_float
         L.oracle_update_weights.argtypes = [C.c_void_p]
         L.oracle_update_weights_with.argtypes = [C.c_void_p, u64p, C.c_int]
         L.oracle_get_energies.argtypes = [C.c_void_p, i32p, C.c_int]
@@ -143,6 +148,15 @@ class Oracle:
                                                     _p(H, C.c_uint64), H.size, n_threads)
         if rc != 0:
             raise ValueError(f"oracle_run_iteration_random_site failed rc={rc}")
+        return H
+
+    def run_iteration_random_site_expf(self, therm_updates: int, updates: int, n_threads: int = 1) -> np.ndarray:
+        """The same with the paper's single-precision acceptance U < exp32(omega_f[j'] - omega_f[j]) (R23)."""
+        H = np.zeros(self.n_bins, dtype=np.uint64)
+        rc = lib().oracle_run_iteration_random_site_expf(self._h, C.c_uint64(therm_updates), C.c_uint64(updates),
+                                                         _p(H, C.c_uint64), H.size, n_threads)
+        if rc != 0:
+            raise ValueError(f"oracle_run_iteration_random_site_expf failed rc={rc}")
         return H
 
     def update_weights(self):

@@ -46,4 +46,5 @@ def curand_pin(tmp_path_factory):
     lib.pin_curand_philox4x32_10.argtypes = [u32p, u32p, u32p]
     lib.pin_curand_philox4x32_10.restype = None
     lib.pin_curand_host_generate.argtypes = [ctypes.c_ulonglong, ctypes.c_ulonglong, u32p, ctypes.c_size_t]
+    lib.pin_curand_host_generate_uniform.argtypes = [ctypes.c_ulonglong, ctypes.c_ulonglong, ctypes.POINTER(ctypes.c_float), ctypes.c_size_t]
     return lib

@@ -36,4 +36,17 @@ int pin_curand_host_generate(unsigned long long seed, unsigned long long offset,
     return rc;
 }
 
+// n uniform floats of the host generator with the given seed and offset: the library's own mapping of the raw 32-bit
+// words (pin_curand_host_generate with the same seed and offset) to (0, 1] -- pins the oracle's uniform32 (R23).
+int pin_curand_host_generate_uniform(unsigned long long seed, unsigned long long offset, float* out, size_t n) {
+    curandGenerator_t g;
+    if (curandCreateGeneratorHost(&g, CURAND_RNG_PSEUDO_PHILOX4_32_10) != CURAND_STATUS_SUCCESS) return -1;
+    int rc = 0;
+    if (curandSetPseudoRandomGeneratorSeed(g, seed) != CURAND_STATUS_SUCCESS) rc = -2;
+    if (!rc && curandSetGeneratorOffset(g, offset) != CURAND_STATUS_SUCCESS) rc = -3;
+    if (!rc && curandGenerateUniform(g, out, n) != CURAND_STATUS_SUCCESS) rc = -4;
+    curandDestroyGenerator(g);
+    return rc;
+}
+
 }  // extern "C"

@@ -1,7 +1,7 @@
 """The paper's own update scheme (R22): the same random site in all
 walkers, per-walker acceptance stream, work counted in updates.
 
-not gpu: pins of the oracle's variant -- omega == 0 closed form (every update accepted: the final configuration is
+not gpu: pins of the oracle's variants -- omega == 0 closed form (every update accepted: the final configuration is
          the initial one with every site flipped as often as the shared site stream drew it, the stream recomputed
          from the pinned Philox), canonical weights against the exact g(E) at L = 4, invariants.
 gpu    : muca_run_iteration_random_site against the oracle, bit for bit.
@@ -85,6 +85,66 @@ def test_walkers_share_sites_but_not_decisions():
     assert all(set(np.nonzero(changed[w])[0].tolist()) <= sites for w in range(W))
     assert len({tuple(c) for c in changed}) > 1
     o.close()
+
+
+# ------------------------------------------------------------------------------------------------ fp32 acceptance (R23)
+def test_exp32_against_arbitrary_precision():
+    # PAPER.md:109 "a single precision version of the exponential function"; R23: a fixed sequence of fp32 operations
+    L = mo.lib()
+    xs = np.concatenate([np.linspace(-24.0, 0.0, 20001), -np.logspace(-12, 1.3, 500), [-24.0, -1e-30, -0.0, -0.6931472, -23.99999]])
+    worst = 0.0
+    for d in xs.astype(np.float32):
+        v, ref = L.oracle_exp32(float(d)), mp.exp(mp.mpf(float(d)))
+        worst = max(worst, abs(float((mp.mpf(v) - ref) / ref)))
+    assert worst < 2.0 * 2.0 ** -23, worst                     # 2 ulp
+    assert L.oracle_exp32(-24.5) == 0.0 and L.oracle_exp32(-1e30) == 0.0 and L.oracle_exp32(-0.0) == 1.0
+    ys = np.array([L.oracle_exp32(float(d)) for d in np.linspace(-24, 0, 3001).astype(np.float32)])
+    assert np.all(np.diff(ys) >= -2.0 ** -23 * ys[1:])          # monotone up to its own rounding
+
+
+def test_uniform32_is_curands_mapping(curand_pin):
+    # the Philox word -> (0, 1] as curand_uniform does it: compared with what libcurand's host generator returns for
+    # the same raw words
+    n = 1 << 16
+    raw = np.zeros(n, dtype=np.uint32)
+    uni = np.zeros(n, dtype=np.float32)
+    import ctypes
+    assert curand_pin.pin_curand_host_generate(77, 0, raw.ctypes.data_as(ctypes.POINTER(ctypes.c_uint32)), n) == 0
+    assert curand_pin.pin_curand_host_generate_uniform(77, 0, uni.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), n) == 0
+    L = mo.lib()
+    mine = np.array([L.oracle_uniform32(int(x)) for x in raw], dtype=np.float32)
+    assert np.array_equal(mine, uni)
+    assert L.oracle_uniform32(0) == 2.0 ** -33 and L.oracle_uniform32(2 ** 32 - 1) == 1.0
+
+
+@pytest.mark.parametrize("beta", [0.25, -0.1])
+def test_fp32_acceptance_reproduces_boltzmann_distribution(beta):
+    # the same canonical check as above with U < exp32(omega_f[j'] - omega_f[j])
+    L, N, W = 4, 16, 512
+    with open(os.path.join(GOLDEN, "ising_dos_L4.txt")) as f:
+        g = np.array([float(x) for x in f if not x.startswith("#")])
+    E = -2 * N + 4 * np.arange(N + 1)
+    o = mo.Oracle(L, W, 5)
+    o.set_log_weights(-beta * E)
+    H = o.run_iteration_random_site_expf(50 * N, 2000 * N, n_threads=THREADS)
+    P, Pe = H / H.sum(), g * np.exp(-beta * E)
+    Pe /= Pe.sum()
+    assert np.abs(P - Pe).max() < 2e-3 and abs((P * E).sum() - (Pe * E).sum()) < 0.05
+    assert H[1] == 0 and H[N - 1] == 0 and int(H.sum()) == W * 2000 * N
+    assert np.array_equal(energy_numpy(o.get_spins()), o.get_energies())
+    o.close()
+
+
+def test_fp32_and_threshold_acceptance_agree_where_no_rounding_is_involved():
+    # omega == 0: every weight difference is 0 -> accepted in both forms; omega with steps of -100 per slot: a move
+    # up in omega is always accepted, a move down never (exp(-100) < 2^-33 in fp32, T = floor(exp(-100) 2^32) -> 1, i.e.
+    # accepted only for the deviate 0): the two chains coincide (no deviate is 0 in these short runs)
+    for logw in (np.zeros(65), -100.0 * np.arange(65)):
+        a, b = mo.Oracle(8, 40, 11), mo.Oracle(8, 40, 11)
+        a.set_log_weights(logw); b.set_log_weights(logw)
+        Ha, Hb = a.run_iteration_random_site(10, 4000), b.run_iteration_random_site_expf(10, 4000)
+        assert np.array_equal(Ha, Hb) and np.array_equal(a.get_spins(), b.get_spins())
+        a.close(); b.close()
 
 
 # ------------------------------------------------------------------------------------------------ GPU parity
