@@ -78,12 +78,19 @@ enum {
                                      schedule rounded up to whole sweeps, R18) or MUCA_SCHEME_RANDOM_SITE (the paper's
                                      own scheme and units: N_therm = 30 w and N_updates attempted flips per walker;
                                      muca_production then runs therm_sweeps * N and sweeps * N updates per call) */
+    MUCA_OPT_ACCEPTANCE = 8,      /* muca_run_iteration_random_site only: MUCA_ACCEPT_THRESHOLD (default: integer thresholds from
+                                     double omega, R6/R7) or MUCA_ACCEPT_EXPF32, the paper's single-precision form (
+                                     DESIGN.md R23): omega rounded to fp32, a proposal j -> j' is accepted iff the difference
+                                     D = omega_f[j'] - omega_f[j] >= 0 or U < exp32(D), U the Philox word mapped to (0, 1] as
+                                     cuRAND's curand_uniform maps it, exp32 a fixed sequence of fp32 operations (identical on
+                                     CPU and GPU, which is what the paper asks of its own code) */
     MUCA_OPT_ROLE_MAP = 7,        /* resident kernel with 4 warp pairs per block: 0 = walker warps share schedulers with
                                      walker warps, 1 = every scheduler runs one walker and one deviate warp (A/B knob) */
     MUCA_OPT_TABLE_WINDOW_ROWS = 6 /* STREAMED_PAIRS kernel: rows of the threshold-table window held in shared memory;
                                      0 = as many as fit.  A value below L*L+1 forces a window (testing) */
 };
 enum { MUCA_SCHEME_TYPEWRITER = 0, MUCA_SCHEME_RANDOM_SITE = 1 };
+enum { MUCA_ACCEPT_THRESHOLD = 0, MUCA_ACCEPT_EXPF32 = 1 };
 
 /* The walker count at which the current CUDA device is fully and evenly loaded by the default kernel for lattice size L --
  * the analogue of the paper's N_opt, "the first and lowest minimum" of the time per spin flip over the number of walkers,

@@ -16,6 +16,8 @@ MUCA_KERNEL_AUTO, MUCA_KERNEL_RESIDENT, MUCA_KERNEL_STREAMED, MUCA_KERNEL_STREAM
 MUCA_OPT_KERNEL, MUCA_OPT_THREADS_PER_BLOCK, MUCA_OPT_MAX_SWEEPS_PER_LAUNCH, MUCA_OPT_WALKERS_PER_WARP = 1, 2, 3, 4
 MUCA_OPT_UPDATE_SCHEME = 5
 MUCA_OPT_TABLE_WINDOW_ROWS = 6
+MUCA_OPT_ACCEPTANCE = 8
+MUCA_ACCEPT_THRESHOLD, MUCA_ACCEPT_EXPF32 = 0, 1
 MUCA_OPT_ROLE_MAP = 7
 MUCA_SCHEME_TYPEWRITER, MUCA_SCHEME_RANDOM_SITE = 0, 1
 

@@ -65,6 +65,7 @@ struct muca_ctx {
     int conv_w_prev = 0;            // width covered by the previous iteration of muca_converge (0: none yet)
     double conv_n_updates = 0.0;    // N_updates (flips per walker) of the previous iteration of muca_converge
     int opt_scheme = MUCA_SCHEME_TYPEWRITER;   // update scheme used by muca_converge / muca_production
+    int opt_acceptance = MUCA_ACCEPT_THRESHOLD;   // MUCA_OPT_ACCEPTANCE (random-site scheme only)
     int conv_full = 0;              // the previous iteration already worked on the whole energy range
     int device = 0;                 // CUDA device the context lives on: every entry point selects it (DeviceGuard)
     int n_sm = 0;
@@ -379,11 +380,11 @@ int create_common(muca_ctx** out, int L, int W, uint64_t seed, uint32_t walker_o
 }  // namespace
 
 namespace {
-template <int L>
+template <int L, int ACC>
 int launch_random_site(muca_ctx* ctx, const RandomSiteParams& prm, int tpb) {
-    const size_t smem = random_site_smem_bytes<L>(tpb);
-    SMEM((random_site_kernel<L>), smem);
-    random_site_kernel<L><<<(prm.W + tpb - 1) / tpb, tpb, smem, ctx->stream>>>(prm);
+    const size_t smem = random_site_smem_bytes<L, ACC>(tpb);
+    SMEM((random_site_kernel<L, ACC>), smem);
+    random_site_kernel<L, ACC><<<(prm.W + tpb - 1) / tpb, tpb, smem, ctx->stream>>>(prm);
     CU(cudaGetLastError());
     return MUCA_OK;
 }
@@ -467,6 +468,11 @@ int muca_set_option(muca_ctx* ctx, int option, int value) {
     if (option == MUCA_OPT_UPDATE_SCHEME) {
         if (value != MUCA_SCHEME_TYPEWRITER && value != MUCA_SCHEME_RANDOM_SITE) return fail(ctx, MUCA_EINVAL, "bad update scheme %d", value);
         ctx->opt_scheme = value;
+        return MUCA_OK;
+    }
+    if (option == MUCA_OPT_ACCEPTANCE) {
+        if (value != MUCA_ACCEPT_THRESHOLD && value != MUCA_ACCEPT_EXPF32) return fail(ctx, MUCA_EINVAL, "bad acceptance form %d", value);
+        ctx->opt_acceptance = value;
         return MUCA_OK;
     }
     if (option == MUCA_OPT_ROLE_MAP) {
@@ -714,19 +720,25 @@ int muca_run_iteration_random_site(muca_ctx* ctx, uint64_t therm_updates, uint64
     if (ctx->iteration == 0xFFFFFFFFu) return fail(ctx, MUCA_ERANGE, "iteration counter exhausted");
     if (therm_updates > (1ull << 60) || updates > (1ull << 60)) return fail(ctx, MUCA_EINVAL, "too many updates");
     const DeviceGuard guard(ctx);
-    std::vector<uint32_t> t5;
-    build_thresholds5(ctx->logw, t5);                                           // a1, as in muca_run_iteration
-    expand_table8(t5, ctx->n_bins, ctx->h_table);
+    const bool expf32 = ctx->opt_acceptance == MUCA_ACCEPT_EXPF32;
+    if (expf32) {   // R23: the weights in single precision; the kernel evaluates U < exp32(omega_f[j'] - omega_f[j])
+        float* wf = reinterpret_cast<float*>(ctx->h_table);
+        for (int j = 0; j < ctx->n_bins; ++j) wf[j] = (float)ctx->logw[j];
+    } else {
+        std::vector<uint32_t> t5;
+        build_thresholds5(ctx->logw, t5);                                       // a1, as in muca_run_iteration
+        expand_table8(t5, ctx->n_bins, ctx->h_table);
+    }
     CU(cudaMemcpyAsync(ctx->d_table, ctx->h_table, (size_t)ctx->n_bins * 8 * 4, cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaMemsetAsync(ctx->d_H, 0, (size_t)ctx->n_bins * 8, ctx->stream));
     // one block per SM where the walkers allow it; the lattice words of a block's walkers must fit beside table and bins
     auto rs_smem = [&](int t) -> size_t {
         switch (ctx->L) {
-            case 8: return random_site_smem_bytes<8>(t);
-            case 16: return random_site_smem_bytes<16>(t);
-            case 32: return random_site_smem_bytes<32>(t);
-            case 64: return random_site_smem_bytes<64>(t);
-            default: return random_site_smem_bytes<128>(t);
+            case 8: return expf32 ? random_site_smem_bytes<8, 1>(t) : random_site_smem_bytes<8, 0>(t);
+            case 16: return expf32 ? random_site_smem_bytes<16, 1>(t) : random_site_smem_bytes<16, 0>(t);
+            case 32: return expf32 ? random_site_smem_bytes<32, 1>(t) : random_site_smem_bytes<32, 0>(t);
+            case 64: return expf32 ? random_site_smem_bytes<64, 1>(t) : random_site_smem_bytes<64, 0>(t);
+            default: return expf32 ? random_site_smem_bytes<128, 1>(t) : random_site_smem_bytes<128, 0>(t);
         }
     };
     int tpb = ((ctx->W + ctx->n_sm - 1) / ctx->n_sm + 31) / 32 * 32;
@@ -749,11 +761,11 @@ int muca_run_iteration_random_site(muca_ctx* ctx, uint64_t therm_updates, uint64
         prm.u_begin = u; prm.u_end = e;
         int rc = MUCA_EINVAL;
         switch (ctx->L) {
-            case 8: rc = launch_random_site<8>(ctx, prm, tpb); break;
-            case 16: rc = launch_random_site<16>(ctx, prm, tpb); break;
-            case 32: rc = launch_random_site<32>(ctx, prm, tpb); break;
-            case 64: rc = launch_random_site<64>(ctx, prm, tpb); break;
-            case 128: rc = launch_random_site<128>(ctx, prm, tpb); break;
+            case 8: rc = expf32 ? launch_random_site<8, 1>(ctx, prm, tpb) : launch_random_site<8, 0>(ctx, prm, tpb); break;
+            case 16: rc = expf32 ? launch_random_site<16, 1>(ctx, prm, tpb) : launch_random_site<16, 0>(ctx, prm, tpb); break;
+            case 32: rc = expf32 ? launch_random_site<32, 1>(ctx, prm, tpb) : launch_random_site<32, 0>(ctx, prm, tpb); break;
+            case 64: rc = expf32 ? launch_random_site<64, 1>(ctx, prm, tpb) : launch_random_site<64, 0>(ctx, prm, tpb); break;
+            case 128: rc = expf32 ? launch_random_site<128, 1>(ctx, prm, tpb) : launch_random_site<128, 0>(ctx, prm, tpb); break;
         }
         if (rc != MUCA_OK) return rc;
         ++launches;

@@ -32,15 +32,42 @@ struct RandomSiteParams {
 
 constexpr int RS_CHUNK = 256;     // updates described ahead, per block
 
-template <int L>
+// ACC: how a proposal is decided.  0 = integer thresholds thresh[j][a] (R6/R7, the library's own form); 1 = the paper's
+// single-precision form U < exp32(omega_f[j'] - omega_f[j]) (R23), with omega_f as BINS floats in
+// shared memory for every L.
+enum { RS_ACC_THRESHOLD = 0, RS_ACC_EXPF32 = 1 };
+
+// R23: the Philox word mapped to (0, 1] as cuRAND's curand_uniform does, and exp for arguments <= 0 as a fixed sequence
+// of IEEE fp32 operations (the paper's requirement of identical results on CPU and GPU; restated, not
+// shared, by the CPU implementation the tests compare with)
+__device__ __forceinline__ float rs_uniform32(const uint32_t x) {
+    return __fmaf_rn(__uint2float_rn(x), 2.3283064365386963e-10f, 1.1641532182693481e-10f);
+}
+__device__ __forceinline__ float rs_exp32(const float d) {
+    if (d < -24.0f) return 0.0f;                                 // exp(-24) < 2^-33 <= U: never accepted
+    const int n = __float2int_rn(__fmul_rn(d, 1.4426950408889634f));
+    const float fn = __int2float_rn(n);
+    float r = __fmaf_rn(fn, -0.693145751953125f, d);
+    r = __fmaf_rn(fn, -1.428606765330187e-06f, r);
+    float p = 1.0f / 720.0f;
+    p = __fmaf_rn(p, r, 1.0f / 120.0f);
+    p = __fmaf_rn(p, r, 1.0f / 24.0f);
+    p = __fmaf_rn(p, r, 1.0f / 6.0f);
+    p = __fmaf_rn(p, r, 0.5f);
+    p = __fmaf_rn(p, r, 1.0f);
+    p = __fmaf_rn(p, r, 1.0f);
+    return __fmul_rn(p, __int_as_float((n + 127) << 23));
+}
+
+template <int L, int ACC = RS_ACC_THRESHOLD>
 struct RandomSite {
     static constexpr int N = L * L, BINS = N + 1, NW = N / 32;
-    static constexpr bool TBL_SMEM = L <= 64;
+    static constexpr bool TBL_SMEM = L <= 64 || ACC == RS_ACC_EXPF32;
     // L <= 32: rows of thresh[j][0..4] | bin of slot j | pad (7 words, odd stride: all banks): threshold and bin are one
     // add away from the row address.  L = 64: rows of 5 thresholds and the bins apart (beside 208 walkers' lattices a
     // 7-word table would not fit).  L = 128: bins only.
-    static constexpr bool BIN_IN_ROW = L <= 32;
-    static constexpr int ROW_WORDS = BIN_IN_ROW ? 7 : 5;
+    static constexpr bool BIN_IN_ROW = L <= 32 && ACC == RS_ACC_THRESHOLD;
+    static constexpr int ROW_WORDS = ACC == RS_ACC_EXPF32 ? 1 : (BIN_IN_ROW ? 7 : 5);
     static constexpr int TBL_WORDS = TBL_SMEM ? ((BINS * ROW_WORDS + 3) & ~3) : 0;
     static constexpr int BIN_WORDS = BIN_IN_ROW ? 0 : ((BINS + 3) & ~3);
     static constexpr int DESC_WORDS = 8 * (RS_CHUNK + 2);      // two uint4 per update + two entries behind the chunk
@@ -89,11 +116,12 @@ __device__ __forceinline__ RsHood rs_eval(const RsWords& r, const uint4 d0, cons
 // anything evaluated -- three independent loads in flight, one round trip per update.  If the next update touches the
 // word this one may change (flag in its descriptor, warp-uniform, ~5 / number of words of the time) its words are
 // loaded again behind the store.
-template <int L, int MEAS>
+template <int L, int MEAS, int ACC>
 __device__ __forceinline__ void rs_group(char* lat, const uint4* desc, const uint32_t* tbl, uint32_t* bins, const RandomSiteParams& prm,
                                          const int k, const int k0, const int k1, const int kth, const uint32_t (&ra)[4], int& j, RsHood& cur,
                                          uint4& d0, uint4& d1, uint32_t (&st)[4]) {
-    constexpr bool TBL_SMEM = RandomSite<L>::TBL_SMEM, BIN_IN_ROW = RandomSite<L>::BIN_IN_ROW;
+    constexpr bool TBL_SMEM = RandomSite<L, ACC>::TBL_SMEM, BIN_IN_ROW = RandomSite<L, ACC>::BIN_IN_ROW;
+    constexpr int N = L * L;
 #pragma unroll
     for (int m = 0; m < 4; ++m) {
         RsWords nw = rs_load<L>(lat, d0, d1);
@@ -104,15 +132,31 @@ __device__ __forceinline__ void rs_group(char* lat, const uint4* desc, const uin
             philox_round(st, prm.key0 + (uint32_t)r * 0x9E3779B9u, prm.key1 + (uint32_t)r * 0xBB67AE85u);
         const bool live = MEAS != 2 || (k + m >= k0 && k + m < k1);
         uint32_t t = 0u;   // BIN_IN_ROW: j is the BYTE offset of the walker's table row (28 j), so that threshold and bin need one add
-        if (live) t = BIN_IN_ROW ? *reinterpret_cast<const volatile uint32_t*>(reinterpret_cast<const char*>(tbl) + j + 4 * (int)cur.a)
-                    : TBL_SMEM ? *reinterpret_cast<const volatile uint32_t*>(tbl + 5 * j + (int)cur.a)
-                               : __ldg(prm.table + (size_t)j * 8 + (cur.a ? 2u * cur.a - 1u : 0u));
+        float w_here = 0.0f, w_there = 0.0f;
+        const int jn = j + 2 - (int)cur.a;                      // ACC = 1: j is the slot itself
+        if constexpr (ACC == RS_ACC_EXPF32) {
+            if (live) {
+                w_here = __uint_as_float(*reinterpret_cast<const volatile uint32_t*>(tbl + j));
+                w_there = __uint_as_float(*reinterpret_cast<const volatile uint32_t*>(tbl + (jn < 0 ? 0 : jn > N ? N : jn)));
+            }
+        } else {
+            if (live) t = BIN_IN_ROW ? *reinterpret_cast<const volatile uint32_t*>(reinterpret_cast<const char*>(tbl) + j + 4 * (int)cur.a)
+                        : TBL_SMEM ? *reinterpret_cast<const volatile uint32_t*>(tbl + 5 * j + (int)cur.a)
+                                   : __ldg(prm.table + (size_t)j * 8 + (cur.a ? 2u * cur.a - 1u : 0u));
+        }
         const uint4 e0 = desc[2 * (k + m) + 4], e1 = desc[2 * (k + m) + 5];   // descriptor of update k + m + 2 (two dummies behind the chunk)
         RsHood nxt = rs_eval(nw, d0, d1);
         if (live) {
-            if (ra[m] <= t) {                                                // R6/R7
+            bool accept;
+            if constexpr (ACC == RS_ACC_EXPF32) {                            // R23
+                const float D = __fsub_rn(w_there, w_here);
+                accept = cur.a == 2u || (jn >= 0 && jn <= N && (D >= 0.0f || rs_uniform32(ra[m]) < rs_exp32(D)));
+            } else {
+                accept = ra[m] <= t;                                         // R6/R7
+            }
+            if (accept) {
                 *reinterpret_cast<volatile uint32_t*>(lat + cur.addr_c) = cur.wc ^ cur.mask;
-                j += (BIN_IN_ROW ? 4 * RandomSite<L>::ROW_WORDS : 1) * (2 - (int)cur.a);   // dE = 8 - 4a
+                j += (BIN_IN_ROW ? 4 * RandomSite<L, ACC>::ROW_WORDS : 1) * (2 - (int)cur.a);   // dE = 8 - 4a
             }
             if (MEAS == 1 || (MEAS == 2 && k + m >= kth))                    // H[j]++ after EVERY measured attempt
                 atomicAdd(BIN_IN_ROW ? reinterpret_cast<uint32_t*>(reinterpret_cast<char*>(bins) + j + 20) : bins + j, 1u);
@@ -125,9 +169,9 @@ __device__ __forceinline__ void rs_group(char* lat, const uint4* desc, const uin
     }
 }
 
-template <int L>
+template <int L, int ACC>
 __global__ void random_site_kernel(const RandomSiteParams prm) {
-    using R = RandomSite<L>;
+    using R = RandomSite<L, ACC>;
     constexpr int N = R::N, BINS = R::BINS, NW = R::NW;
     constexpr int LOG_L = L == 8 ? 3 : L == 16 ? 4 : L == 32 ? 5 : L == 64 ? 6 : 7;
     extern __shared__ __align__(16) uint32_t smem[];
@@ -140,7 +184,9 @@ __global__ void random_site_kernel(const RandomSiteParams prm) {
     uint32_t* const sites = smem + R::TBL_WORDS + R::BIN_WORDS + R::DESC_WORDS;
     uint32_t* const latw = sites + R::SITE_WORDS + tid;         // typewriter word t of this walker at latw[t * tpb]
     char* const lat = reinterpret_cast<char*>(latw);
-    if (R::TBL_SMEM) {
+    if (ACC == RS_ACC_EXPF32) {
+        for (int j = tid; j < BINS; j += tpb) tbl[j] = prm.table[j];       // omega_f[j] (float bits; the host rounded omega)
+    } else if (R::TBL_SMEM) {
         for (int idx = tid; idx < BINS * R::ROW_WORDS; idx += tpb) {
             const int j = idx / R::ROW_WORDS, a = idx - R::ROW_WORDS * j;
             tbl[idx] = a < 5 ? prm.table[j * 8 + (a ? 2 * a - 1 : 0)] : 0u;   // a column of T8 with a(f) = a; bin and pad: 0
@@ -200,9 +246,9 @@ __global__ void random_site_kernel(const RandomSiteParams prm) {
             const uint32_t ra[4] = {st[0], st[1], st[2], st[3]};
             const unsigned long long un = u0 + (unsigned long long)k + 4ull;   // counter of the next group
             st[0] = (uint32_t)((un >> 2) & 0xFFFFFFFFull); st[1] = (uint32_t)(un >> 34); st[2] = prm.iteration; st[3] = g;
-            if (k >= k0 && k + 4 <= k1 && k >= kth) rs_group<L, 1>(lat, desc, tbl, bins, prm, k, k0, k1, kth, ra, j, cur, d0, d1, st);
-            else if (k >= k0 && k + 4 <= k1 && k + 4 <= kth) rs_group<L, 0>(lat, desc, tbl, bins, prm, k, k0, k1, kth, ra, j, cur, d0, d1, st);
-            else rs_group<L, 2>(lat, desc, tbl, bins, prm, k, k0, k1, kth, ra, j, cur, d0, d1, st);
+            if (k >= k0 && k + 4 <= k1 && k >= kth) rs_group<L, 1, ACC>(lat, desc, tbl, bins, prm, k, k0, k1, kth, ra, j, cur, d0, d1, st);
+            else if (k >= k0 && k + 4 <= k1 && k + 4 <= kth) rs_group<L, 0, ACC>(lat, desc, tbl, bins, prm, k, k0, k1, kth, ra, j, cur, d0, d1, st);
+            else rs_group<L, 2, ACC>(lat, desc, tbl, bins, prm, k, k0, k1, kth, ra, j, cur, d0, d1, st);
         }
     }
     if (active) {
@@ -217,9 +263,9 @@ __global__ void random_site_kernel(const RandomSiteParams prm) {
         }
 }
 
-template <int L>
+template <int L, int ACC>
 __host__ __device__ constexpr size_t random_site_smem_bytes(int tpb) {
-    return RandomSite<L>::smem_bytes(tpb);
+    return RandomSite<L, ACC>::smem_bytes(tpb);
 }
 
 }  // namespace muca

@@ -170,6 +170,29 @@ def test_gpu_random_site_matches_oracle(L, W, offset, therm, updates):
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("L,W,offset,therm,updates", [(8, 131, 0, 50, 3000), (16, 300, 7, 101, 5000), (32, 200, 1000, 333, 20001),
+                                                      (64, 150, 3, 10, 9000), (128, 40, 0, 7, 6000)])
+def test_gpu_random_site_fp32_acceptance_matches_oracle(L, W, offset, therm, updates):
+    # MUCA_OPT_ACCEPTANCE = EXPF32 (R23): same chains as the oracle's fp32 variant, bit for bit
+    from paper_1707_00919_b200 import binding as B
+    g, o = mb.Muca(L, W, 170700919, walker_offset=offset), mo.Oracle(L, W, 170700919, walker_offset=offset)
+    try:
+        g.set_option(B.MUCA_OPT_ACCEPTANCE, B.MUCA_ACCEPT_EXPF32)
+        for it in range(4):
+            Hg = g.run_iteration_random_site(therm, updates)
+            Ho = o.run_iteration_random_site_expf(therm, updates, n_threads=mo.max_threads())
+            assert int(Hg.sum()) == W * updates and np.array_equal(Hg, Ho), f"it{it}"
+            g.update_weights(); o.update_weights()
+        assert np.array_equal(g.get_energies(), o.get_energies())
+        assert np.array_equal(g.get_spins(), o.get_spins())
+        # back to thresholds on the same context
+        g.set_option(B.MUCA_OPT_ACCEPTANCE, B.MUCA_ACCEPT_THRESHOLD)
+        assert np.array_equal(g.run_iteration_random_site(3, 500), o.run_iteration_random_site(3, 500, n_threads=mo.max_threads()))
+    finally:
+        g.close(); o.close()
+
+
+@pytest.mark.gpu
 def test_gpu_random_site_zero_updates_and_errors():
     g = mb.Muca(16, 33, 1)
     H = g.run_iteration_random_site(0, 0)
