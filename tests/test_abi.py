@@ -38,6 +38,9 @@ def test_host_only_entry_points():
     w, p = ctypes.c_int(), ctypes.c_int()
     assert lib.muca_suggest_walkers(12, ctypes.byref(w), ctypes.byref(p)) == -1
     assert lib.muca_suggest_walkers(32, None, ctypes.byref(p)) == -1
+    import torch
+    if not torch.cuda.is_available():                            # no device: MUCA_ECUDA, never a made-up number
+        assert lib.muca_suggest_walkers(32, ctypes.byref(w), ctypes.byref(p)) == -2
     # bad arguments are rejected before any CUDA call
     h = ctypes.c_void_p()
     assert lib.muca_create(ctypes.byref(h), 7, 32, 1) == -1 and not h
