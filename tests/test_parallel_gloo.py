@@ -83,3 +83,45 @@ def test_two_ranks_reproduce_the_single_process_run(tmp_path):
     assert np.array_equal(r0["logw"], ref.get_log_weights()) and np.array_equal(r1["logw"], r0["logw"])
     assert np.array_equal(np.concatenate([r0["E"], r1["E"]]), ref.get_energies())
     assert np.array_equal(np.concatenate([r0["spins"], r1["spins"]]), ref.get_spins())
+
+
+# ------------------------------------------------------------------------------------------------ the same with the CUDA library
+def _gpu_worker(rank, world, port, out_dir):
+    for p in (ROOT, os.path.join(ROOT, "oracle"), os.path.join(ROOT, "tests")):
+        if p not in sys.path:
+            sys.path.insert(0, p)
+    import torch
+    import torch.distributed as dist
+    torch.cuda.set_device(rank % torch.cuda.device_count())     # one process per GPU where there are several
+    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world)
+    try:
+        sm = ShardedMuca(32, 301, 170700919)                    # default engine: the CUDA library binding
+        Hs = []
+        for _ in range(3):
+            Hs.append(sm.run_iteration(2, 10))
+            sm.update_weights()
+        np.savez(os.path.join(out_dir, f"r{rank}.npz"), H=np.stack(Hs), logw=sm.get_log_weights(),
+                 E=sm.get_energies(), spins=sm.get_spins(), offset=sm.offset, count=sm.count)
+        sm.close()
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.gpu
+def test_two_ranks_with_the_cuda_library_reproduce_the_oracle(tmp_path):
+    # ShardedMuca with its default engine (libmuca_b200 through the binding) in two processes -- on two GPUs where the box
+    # has them, otherwise both on cuda:0 --, histogram sum over gloo: global walker ids make the chains independent of
+    # the split (R16), so the result is the single-process oracle's
+    port = 31500 + (os.getpid() % 2000)
+    mp.spawn(_gpu_worker, args=(2, port, str(tmp_path)), nprocs=2, join=True)
+    r0, r1 = np.load(tmp_path / "r0.npz"), np.load(tmp_path / "r1.npz")
+    ref = mo.Oracle(32, 301, 170700919)
+    Hs = []
+    for _ in range(3):
+        Hs.append(ref.run_iteration(2, 10, n_threads=mo.max_threads()))
+        ref.update_weights()
+    assert (int(r0["offset"]), int(r0["count"]), int(r1["offset"]), int(r1["count"])) == (0, 151, 151, 150)
+    assert np.array_equal(r0["H"], np.stack(Hs)) and np.array_equal(r1["H"], r0["H"])
+    assert np.max(np.abs(r0["logw"] - ref.get_log_weights())) <= 1e-12 and np.array_equal(r1["logw"], r0["logw"])
+    assert np.array_equal(np.concatenate([r0["E"], r1["E"]]), ref.get_energies())
+    assert np.array_equal(np.concatenate([r0["spins"], r1["spins"]]), ref.get_spins())
