@@ -263,6 +263,37 @@ const char* muca_last_error(const muca_ctx* ctx);
  * ctr: host uint32[4n], key: host uint32[2n], out: host uint32[4n]. */
 int muca_debug_philox(const uint32_t* ctr, const uint32_t* key, uint32_t* out, int n);
 
+/* The same test hook for callers that are not allowed to allocate device memory.
+ *
+ * Who that is: muca_debug_philox() above stages its rows in three buffers it cudaMalloc's and cudaFree's on every call.
+ * That is fine for a stand-alone test program, but not for a host process in which someone else owns the GPU's memory --
+ * a PyTorch (or similar) caching allocator that has already taken most of the HBM, or a job that runs with a fixed
+ * memory partition: there a raw cudaMalloc can fail although the framework still has plenty of room, and both cudaMalloc
+ * and cudaFree stall every stream of the device while they run, a running muca_run_iteration included.  Such a caller
+ * (a start-up self-test of the device generator inside a long simulation, say) uses this entry point instead.
+ *
+ * What it does: the same kernel on the same rows, with the staging area in a fixed array that is part of the library
+ * image: MUCA_PHILOX_STATIC_MAX rows of (ctr, key, out) = 160 KiB of device memory, held by every GPU on which the
+ * library has been used, from the moment the CUDA runtime loads the library's device code there until the process
+ * exits.  The function calls neither cudaMalloc / cudaFree nor any other allocating routine.
+ *
+ * ctr: host uint32[4n], key: host uint32[2n], out: host uint32[4n], all caller-owned; runs on the CURRENT device, legacy
+ * default stream, and returns after `out` has been filled.
+ *   n < 1 or a NULL pointer    -> MUCA_EINVAL;
+ *   n > MUCA_PHILOX_STATIC_MAX -> MUCA_ENOMEM: the fixed array cannot hold the rows; nothing is copied or launched and
+ *                                 `out` is untouched (split the rows over several calls, or use muca_debug_philox);
+ *   a CUDA failure             -> MUCA_ECUDA.
+ * First call on a device: it looks up where that device keeps the array (one cudaGetSymbolAddress with that device
+ * current; the answer is remembered per device).  Make that first call at set-up, before any stream capture begins.
+ * Shared state: all calls on one device use the same array, and it still holds the previous call's rows afterwards.
+ * Nothing in it has to be zero at the start -- every word the kernel reads was written by this call's own copy-in, and
+ * only the first n output rows, all of them written by this call's kernel, are copied out -- so stale rows never leak
+ * into a result.  But two calls whose GPU work overlaps would overwrite each other's rows: the function therefore
+ * holds a lock from copy-in to copy-out, which keeps calls made through this one loaded copy of the library apart.
+ * Any other route to running two of them at once on one GPU is a data race. */
+#define MUCA_PHILOX_STATIC_MAX 4096
+int muca_debug_philox_static(const uint32_t* ctr, const uint32_t* key, uint32_t* out, int n);
+
 /* Library version string. */
 const char* muca_version(void);
 

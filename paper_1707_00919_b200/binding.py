@@ -29,7 +29,9 @@ EXPORTS = (
     "muca_unpack_spins_device", "muca_get_thresholds", "muca_get_iteration", "muca_set_iteration",
     "muca_last_sweep_ms", "muca_last_error", "muca_debug_philox", "muca_version",
     "muca_flatness", "muca_schedule", "muca_converge", "muca_production", "muca_run_iteration_random_site", "muca_window_stats",
+    "muca_debug_philox_static",
 )
+MUCA_PHILOX_STATIC_MAX = 4096   # include/muca.h: rows the library's fixed staging array holds
 
 
 class Flatness(C.Structure):
@@ -99,6 +101,7 @@ def lib():
     L.muca_last_error.argtypes = [vp]
     L.muca_last_error.restype = C.c_char_p
     L.muca_debug_philox.argtypes = [u32p, u32p, u32p, C.c_int]
+    L.muca_debug_philox_static.argtypes = [u32p, u32p, u32p, C.c_int]
     L.muca_version.restype = C.c_char_p
     L.muca_flatness.argtypes = [u64p, C.c_int, C.c_int, C.POINTER(Flatness)]
     L.muca_schedule.argtypes = [C.c_int, C.c_int, C.c_int, f64p, C.POINTER(C.c_int), C.POINTER(C.c_int),
@@ -137,6 +140,29 @@ def debug_philox(ctr, key) -> np.ndarray:
     rc = lib().muca_debug_philox(_p(c, C.c_uint32), _p(k, C.c_uint32), _p(out, C.c_uint32), c.shape[0])
     if rc != MUCA_OK:
         raise MucaError(f"muca_debug_philox failed rc={rc}")
+    return out
+
+
+def debug_philox_static(ctr, key) -> np.ndarray:
+    """muca_debug_philox_static: what debug_philox computes, for a caller that must not allocate device memory.
+
+    debug_philox makes the library cudaMalloc and cudaFree its staging buffers on every call.  Inside a process whose
+    GPU memory belongs to someone else (torch's caching allocator holding most of the HBM, a fixed memory partition)
+    that allocation can fail, and it stalls all streams of the device while it runs.  This variant stages the rows in a
+    fixed 160 KiB array inside the library instead and allocates nothing; in exchange it takes at most
+    MUCA_PHILOX_STATIC_MAX rows per call, and calls share that array (one at a time; the library holds a lock).  The
+    first call on a device also looks the array's address up: make it at set-up, before any stream capture."""
+    c = np.ascontiguousarray(ctr, dtype=np.uint32).reshape(-1, 4)
+    k = np.ascontiguousarray(key, dtype=np.uint32).reshape(-1, 2)
+    if c.shape[0] != k.shape[0]:
+        raise MucaError(f"muca_debug_philox_static: {c.shape[0]} counter rows but {k.shape[0]} key rows")
+    out = np.empty_like(c)
+    rc = lib().muca_debug_philox_static(_p(c, C.c_uint32), _p(k, C.c_uint32), _p(out, C.c_uint32), c.shape[0])
+    if rc == -4:
+        raise MucaError(f"muca_debug_philox_static: {c.shape[0]} rows do not fit the library's fixed staging array "
+                        f"(at most MUCA_PHILOX_STATIC_MAX = {MUCA_PHILOX_STATIC_MAX} per call); nothing was computed")
+    if rc != MUCA_OK:
+        raise MucaError(f"muca_debug_philox_static failed rc={rc}")
     return out
 
 

@@ -1051,3 +1051,46 @@ int muca_debug_philox(const uint32_t* ctr, const uint32_t* key, uint32_t* out, i
 }
 
 }  // extern "C"
+
+// ---- muca_debug_philox_static: the Philox test hook for callers that must not allocate (include/muca.h) -----------------
+// The staging rows live in a fixed device array that belongs to the library image: MUCA_PHILOX_STATIC_MAX rows of
+// ctr (16 B), key (8 B) and out (16 B), i.e. 160 KiB on every GPU that loads this module, until the process exits.
+// On the host side the NAME of the array is only a handle for the runtime, not an address a kernel could use: the device
+// address is asked for once per device with cudaGetSymbolAddress (that device current) and it is this pointer that the
+// kernel and the copies get.
+static __device__ __align__(256) unsigned char philox_static_scratch[(size_t)MUCA_PHILOX_STATIC_MAX * 40];
+
+namespace {
+constexpr size_t PHILOX_STATIC_KEY_OFF = (size_t)MUCA_PHILOX_STATIC_MAX * 16;   // ctr rows first, then key rows,
+constexpr size_t PHILOX_STATIC_OUT_OFF = (size_t)MUCA_PHILOX_STATIC_MAX * 24;   // then out rows (both offsets 256-aligned)
+constexpr int PHILOX_STATIC_DEVICES = 64;                                       // device ordinals with a remembered address
+std::mutex philox_static_mutex;                                                 // one call at a time: they share the array
+unsigned char* philox_static_addr[PHILOX_STATIC_DEVICES] = {};                  // device address of the array, per device
+}  // namespace
+
+extern "C" int muca_debug_philox_static(const uint32_t* ctr, const uint32_t* key, uint32_t* out, int n) {
+    if (!ctr || !key || !out || n < 1) return MUCA_EINVAL;
+    if (n > MUCA_PHILOX_STATIC_MAX) return MUCA_ENOMEM;   // more rows than the fixed array holds: refused before any CUDA call
+    std::lock_guard<std::mutex> lock(philox_static_mutex);
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0) return MUCA_ECUDA;
+    unsigned char* base = dev < PHILOX_STATIC_DEVICES ? philox_static_addr[dev] : nullptr;
+    if (!base) {   // set-up, once per device, with that device current
+        void* p = nullptr;
+        if (cudaGetSymbolAddress(&p, philox_static_scratch) != cudaSuccess || !p) return MUCA_ECUDA;
+        base = static_cast<unsigned char*>(p);
+        if (dev < PHILOX_STATIC_DEVICES) philox_static_addr[dev] = base;
+    }
+    uint32_t* const d_c = reinterpret_cast<uint32_t*>(base);
+    uint32_t* const d_k = reinterpret_cast<uint32_t*>(base + PHILOX_STATIC_KEY_OFF);
+    uint32_t* const d_o = reinterpret_cast<uint32_t*>(base + PHILOX_STATIC_OUT_OFF);
+    // Whatever the previous call left in the array is overwritten (rows 0 .. n-1 of ctr and key) or never read (the
+    // rest): nothing has to be cleared.  The copies are blocking, so the call has left the GPU when the lock is dropped.
+    if (cudaMemcpy(d_c, ctr, 16 * (size_t)n, cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(d_k, key, 8 * (size_t)n, cudaMemcpyHostToDevice) != cudaSuccess)
+        return MUCA_ECUDA;
+    philox_debug_kernel<<<(n + 127) / 128, 128>>>(d_c, d_k, d_o, n);
+    if (cudaGetLastError() != cudaSuccess || cudaMemcpy(out, d_o, 16 * (size_t)n, cudaMemcpyDeviceToHost) != cudaSuccess)
+        return MUCA_ECUDA;
+    return MUCA_OK;
+}
