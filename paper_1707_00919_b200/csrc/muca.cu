@@ -597,11 +597,14 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
     };
     // Walkers spread over more table rows than shared memory holds (L = 128 once the weights have spread them: the regime of
     // every production run): the iteration is cut into launches of a few sweeps.  Before each one the walkers are sorted by
-    // energy on the host (8192 energies: a D2H copy and a sort, ~0.3 ms against milliseconds of sweeps), every block is
+    // energy on the host (8192 energies: a D2H copy and a counting sort, ~30 us against milliseconds of sweeps), every block is
     // handed neighbours in energy and a window of its own around them, and spins, energies and histogram are copied aside;
     // a launch that a walker left through a sentinel is undone and repeated with the plain kernel.  The number of sweeps per
     // launch follows from the rows left between a block's walkers and its sentinels: a sweep moves a walker by about
-    // sqrt(3 N / 4) slots (N attempts, every second one accepted, mean squared step 1.5), and 6 sigma must fit.
+    // sqrt(3 N / 4) slots (N attempts, every second one accepted, mean squared step 1.5), and 6 sigma must fit.  That rule
+    // alone decides whether a launch gets windows: win_margin, the back-off of the single-window path below, plays no part
+    // here (it is only ever lowered by clean single-window iterations, which a spread population no longer has -- a margin
+    // grown to thousands of rows would otherwise keep every later iteration on the plain kernel for good).
     auto run_sorted = [&]() -> int {
         const int W = ctx->W, tpb = plan.tpb, n_blocks = (W + tpb - 1) / tpb, cap = win.n_rows;
         const size_t spin_bytes = (size_t)W * (ctx->N / 8);
@@ -638,7 +641,7 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
             const uint64_t meas_begin = s > (uint64_t)therm_sweeps ? s : (uint64_t)therm_sweeps;
             if (e > meas_begin + max_meas) e = meas_begin + max_meas;
             if (ctx->opt_max_sweeps > 0 && e > s + (uint64_t)ctx->opt_max_sweeps) e = s + (uint64_t)ctx->opt_max_sweeps;
-            const double k = room > ctx->win_margin ? (double)room / (6.0 * sigma1) : 0.0;
+            const double k = room > 0 ? (double)room / (6.0 * sigma1) : 0.0;
             uint64_t chunk = (uint64_t)(k * k);
             if (chunk > 64) chunk = 64;
             prm.sweep_begin = (uint32_t)s;
