@@ -255,38 +255,54 @@ def test_windowed_table_and_fallback(L, W, rows, iters, therm, sweeps, expect_fa
 
 # Walkers spread over more table rows than the window holds (L = 128 in every production run): the library sorts the
 # walkers by energy, gives every block a window of its own and cuts the iteration into launches of a few sweeps
-# (muca.cu run_sorted).  Here: L = 32 with a forced 600-row window and exact flat-histogram weights, L = 64 with 1500 rows
-# and omega = 0 (walkers leave their windows: launches are undone and repeated), walkers started all over the energy range.
-@pytest.mark.parametrize("L,W,rows,sweeps", [(32, 200, 600, 8), (64, 150, 1500, 6)])
-def test_sorted_windows_for_widely_spread_walkers(L, W, rows, sweeps):
+# (muca.cu run_sorted).  Walkers are started all over the energy range.  Cases:
+#   L = 32, forced 600-row window, exact flat-histogram weights (every walker diffuses slowly from where it starts);
+#   L = 64, forced 1500 rows, omega = 0 at the start, Eq. (4) updates;
+#   L = 128 with the window the library itself picks (~5500 of the 16385 rows: the shape production runs take), omega = 0
+#     at the start, Eq. (4) updates;
+#   "quench", L = 64 and L = 128: omega = -E (a canonical ensemble far below T_c) pulls the disordered walkers down by
+#     hundreds of slots per sweep, far beyond the 6 sigma of diffusion the launches are sized for: walkers DO leave their
+#     windows, so launches are undone from the snapshot and repeated with the plain kernel (undone > 0 is asserted).
+@pytest.mark.parametrize("L,W,rows,sweeps,weights,expect_undone", [
+    (32, 200, 600, 8, "exact", False), (64, 150, 1500, 6, "zero", False), (128, 200, 0, 6, "zero", False),
+    (64, 150, 1500, 6, "quench", True), (128, 200, 0, 4, "quench", True),
+])
+def test_sorted_windows_for_widely_spread_walkers(L, W, rows, sweeps, weights, expect_undone):
     import os
     N = L * L
     rng = np.random.default_rng(5)
     p = np.linspace(0.0, 0.5, W)[:, None]                       # walker k: a fraction p_k of its spins down -> E from -2N up to ~0
     spins = np.where(rng.random((W, N)) < p, -1, 1).astype(np.int8)
-    if L == 32:                                                 # every second walker times a checkerboard: E -> -E, up to +2N
+    if L != 64:                                                 # every second walker times a checkerboard: E -> -E, up to +2N
         yy, xx = np.divmod(np.arange(N), L)
         spins[1::2] *= np.where((xx + yy) % 2 == 0, 1, -1).astype(np.int8)[None, :]
     g, o = mb.Muca(L, W, PRIMARY_SEED, walker_offset=9), mo.Oracle(L, W, PRIMARY_SEED, walker_offset=9)
     try:
         g.set_spins(spins); o.set_spins(spins)
-        if L == 32:                                             # omega = -ln g: every walker diffuses slowly from where it starts
-            with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "ising_dos_L32.txt")) as f:
+        if weights == "exact":                                  # omega = -ln g
+            with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", f"ising_dos_L{L}.txt")) as f:
                 gE = [int(x) for x in f if not x.startswith("#")]
             import mpmath as mp
             w = np.array([-float(mp.log(v)) if v > 0 else 0.0 for v in gE])
             g.set_log_weights(w); o.set_log_weights(w)
+        if weights == "quench":                                 # omega(E) = -beta E, beta = 1
+            w = -1.0 * (-2.0 * N + 4.0 * np.arange(N + 1))
+            g.set_log_weights(w); o.set_log_weights(w)
         g.set_option(B.MUCA_OPT_KERNEL, B.MUCA_KERNEL_STREAMED_PAIRS)
-        g.set_option(B.MUCA_OPT_TABLE_WINDOW_ROWS, rows)
+        if rows:
+            g.set_option(B.MUCA_OPT_TABLE_WINDOW_ROWS, rows)
         E0 = g.get_energies()
-        assert (E0.max() - E0.min()) // 4 > rows                # one window cannot hold them
+        assert (E0.max() - E0.min()) // 4 > (rows if rows else 6000)   # one window cannot hold them (L = 128: < 5600 rows fit)
         for it in range(3):
             Hg, Ho = g.run_iteration(2, sweeps), o.run_iteration(2, sweeps, n_threads=mo.max_threads())
             assert np.array_equal(Hg, Ho), f"it{it}: H differs in slots {np.nonzero(Hg != Ho)[0][:8]}"
             compare_state(g, o, f"it{it}")
-            g.update_weights(); o.update_weights()
+            if weights != "quench":
+                g.update_weights(); o.update_weights()
         windowed, undone = g.window_stats()
         assert windowed > 0, (windowed, undone)                 # launches with per-block windows did run
+        if expect_undone:
+            assert undone > 0, (windowed, undone)               # ... and some were undone and repeated
     finally:
         g.close(); o.close()
 
@@ -376,10 +392,12 @@ def test_suggested_walker_count_loads_the_device_evenly():
     # SURVEY 8(f)4 / PAPER.md:179, :201: the suggested W is the first optimum of the time per flip -- not slower per flip
     # than one warp per SM less (idle lanes) or one warp per SM more (a second, nearly empty round of blocks)
     import torch
+    n_sm = torch.cuda.get_device_properties(0).multi_processor_count
+    for Lx, px in ((8, 4), (16, 4), (32, 4), (64, 8), (128, 4)):   # include/muca.h: pairs_per_sm of the default kernel per L
+        Wx, pairs = mb.suggest_walkers(Lx)
+        assert pairs == px and Wx == n_sm * px * 32, (Lx, Wx, pairs)
     L = 32
     W, pairs = mb.suggest_walkers(L)
-    n_sm = torch.cuda.get_device_properties(0).multi_processor_count
-    assert W == n_sm * pairs * 32 and pairs == 4
 
     def ns_per_flip(Wx):
         g = mb.Muca(L, Wx, PRIMARY_SEED)
@@ -392,8 +410,10 @@ def test_suggested_walker_count_loads_the_device_evenly():
         finally:
             g.close()
 
+    # a timing on whatever GPU the suite runs on: 10 % of slack (measured: one warp per SM more costs a second round of
+    # blocks, +86 % per flip; one less leaves the time unchanged and wastes 25 % of the lanes, +32 % per flip: profiles/r02_flips_over_W_L32.txt)
     t_opt, t_less, t_more = ns_per_flip(W), ns_per_flip(W - 32 * n_sm), ns_per_flip(W + 32 * n_sm)
-    assert t_opt <= 1.02 * min(t_less, t_more), (t_opt, t_less, t_more)
+    assert t_opt <= 1.10 * min(t_less, t_more), (t_opt, t_less, t_more)
 
 
 def test_context_on_an_explicit_device():
