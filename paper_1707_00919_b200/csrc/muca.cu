@@ -574,8 +574,8 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
     prm.check = ctx->d_flag + 3; prm.fault = 0u;
 #ifdef MUCA_CHECKED
     if (const char* f = getenv("MUCA_CHECKED_FAULT")) prm.fault = (uint32_t)atoi(f);   // tests: make the self-check fire
-    CU(cudaMemsetAsync(ctx->d_flag + 3, 0, sizeof(int), ctx->stream));
 #endif
+    CU(cudaMemsetAsync(ctx->d_flag + 3, 0, sizeof(int), ctx->stream));
     int launches = windowed_plan ? 1 : 0;   // the slot-range kernel
     auto run_sweeps = [&](const Plan& pl) -> int {
         uint64_t max_meas = 0xFFFFFFFFull / ((uint64_t)pl.tpb * (uint64_t)ctx->N);
@@ -700,10 +700,12 @@ int muca_run_iteration(muca_ctx* ctx, int therm_sweeps, int sweeps, uint64_t* H_
     }
     CU(cudaEventRecord(ctx->ev1, ctx->stream));
     CU(cudaMemcpyAsync(ctx->h_H, ctx->d_H, (size_t)ctx->n_bins * 8, cudaMemcpyDeviceToHost, ctx->stream));
-#ifdef MUCA_CHECKED
     CU(cudaMemcpyAsync(ctx->h_flag + 3, ctx->d_flag + 3, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
-#endif
     CU(cudaStreamSynchronize(ctx->stream));
+    if (ctx->h_flag[3] & CHK_SMEM_BASE)   // muca_device.cuh smem_base_ok(): the paired kernels refused to run
+        return fail(ctx, MUCA_ECUDA, "sweep kernel refused to run: on this device / driver the dynamic shared memory does not start at "
+                    "the offset the kernel's table addressing was built for; the iteration was not completed (MUCA_OPT_KERNEL = "
+                    "MUCA_KERNEL_STREAMED does not depend on it, L >= 32)");
 #ifdef MUCA_CHECKED
     if (ctx->h_flag[3])
         return fail(ctx, MUCA_ECUDA, "checked build: self-check failed, mask 0x%x (1 = state is not a table row, 2 = deviates read before "

@@ -181,7 +181,7 @@ struct SweepParams {
     uint32_t sweep_begin;       // first sweep index of this launch (ctr.y)
     uint32_t sweep_end;         // one past the last
     uint32_t therm;             // sweeps with index < therm are not recorded
-    int* check;                 // MUCA_CHECKED build: device word the violations are OR-ed into
+    int* check;                 // device word the violations are OR-ed into (CHK_SMEM_BASE in every build, the rest MUCA_CHECKED)
     uint32_t fault;             // MUCA_CHECKED build, tests: 1 + the hand-over that pair 0 of block 0 tags wrongly; 0 = none
 };
 
@@ -198,7 +198,7 @@ struct SweepParams {
 // A violation sets a bit in a device word; muca_run_iteration then fails with MUCA_ECUDA.  In the normal build all of
 // this compiles to nothing.
 // ------------------------------------------------------------------------------------------------
-enum { CHK_STATE = 1, CHK_RING_EARLY = 2, CHK_RING_LATE = 4 };
+enum { CHK_STATE = 1, CHK_RING_EARLY = 2, CHK_RING_LATE = 4, CHK_SMEM_BASE = 8 };
 struct RingCheck {
 #ifdef MUCA_CHECKED
     uint32_t ctr = 0;                     // hand-overs so far (deviate warp: published, walker warp: fetched)
@@ -229,6 +229,21 @@ __device__ __forceinline__ void state_check(RingCheck& rc, const bool ok) {
 #ifdef MUCA_CHECKED
     if (!ok) atomicOr(rc.flag, CHK_STATE);
 #endif
+}
+
+// Checked in EVERY build: the site macros of the paired kernels address the delta table by an immediate, so the dynamic
+// shared memory must start at the offset they were written for (the driver's reserved area, no static __shared__ in
+// front).  Where it does not, the block sets CHK_SMEM_BASE and returns before touching anything, and muca_run_iteration
+// fails with MUCA_ECUDA -- an ordinary error the caller can handle.  (A __trap() here would leave a sticky error behind
+// that takes the caller's whole CUDA context down, torch's included.)  The condition is the same for every thread of
+// the launch.  MUCA_CHECKED build, tests: prm.fault = 0xFFFFFFFF pretends a mismatch.
+__device__ __forceinline__ bool smem_base_ok(const SweepParams& prm, const uint32_t base, const uint32_t expected) {
+    bool ok = base == expected;
+#ifdef MUCA_CHECKED
+    if (prm.fault == 0xFFFFFFFFu) ok = false;
+#endif
+    if (!ok && threadIdx.x == 0) atomicOr(prm.check, CHK_SMEM_BASE);
+    return ok;
 }
 
 template <int L>

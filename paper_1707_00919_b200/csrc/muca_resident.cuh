@@ -405,7 +405,7 @@ __global__ void __launch_bounds__(64 * V6<L>::MAX_WARPS, 1) sweep_kernel_v6(cons
     char* const sm = reinterpret_cast<char*>(smem);
     const int tid = threadIdx.x, nthr = blockDim.x, nw = nthr >> 6;
     const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(smem);
-    if (sbase != V::SBASE) __trap();   // the site macro addresses the delta table by an immediate
+    if (!smem_base_ok(prm, sbase, V::SBASE)) return;   // the site macro addresses the delta table by an immediate
 
     // ---- table: row j = t[8] | bin; delta table behind the rows
     for (int idx = tid; idx < BINS * 8; idx += nthr) {

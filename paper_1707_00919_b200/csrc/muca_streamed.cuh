@@ -175,7 +175,7 @@ sweep_kernel_s6(const SweepParams prm, const int j_lo_all, const int n_rows, con
     const int j_lo = blk_j_lo ? blk_j_lo[blockIdx.x] : j_lo_all;
     const int sent_lo = blk_j_lo ? (j_lo > 0 ? 2 : 0) : sent_lo_all;
     const int sent_hi = blk_j_lo ? (j_lo + n_rows < N + 1 ? 2 : 0) : sent_hi_all;
-    if ((uint32_t)__cvta_generic_to_shared(smem) != S6_SBASE) __trap();   // the site macro addresses the delta table by an immediate
+    if (!smem_base_ok(prm, (uint32_t)__cvta_generic_to_shared(smem), S6_SBASE)) return;   // the site macro addresses the delta table by an immediate
     uint4* const ring = reinterpret_cast<uint4*>(sm + S6_RING_OFF) + slot;
     uint4* const scratch = reinterpret_cast<uint4*>(sm + S6_SCRATCH_OFF) + pair * 8;
     char* const win = sm + S6_RING_OFF + s6_ring_bytes(npairs);
