@@ -42,6 +42,14 @@
 extern "C" {
 #endif
 
+/* Version of THIS interface: the numeric values of the enums below and the signatures of the entry points.  It is
+ * raised whenever a value is renumbered or retired or a signature changes (history: 1 = round-1 kernels, values 3..6 of
+ * MUCA_OPT_KERNEL in use; 2 = STREAMED_PAIRS renumbered from 6 to 3, values 4..6 retired; 3 = muca_abi_version,
+ * muca_debug_philox_static).  A caller that passes raw integers compares muca_abi_version() of the library it loaded
+ * with the MUCA_ABI_VERSION it was written against and refuses to run on a mismatch (the Python binding does). */
+#define MUCA_ABI_VERSION 3
+int muca_abi_version(void);
+
 typedef struct muca_ctx muca_ctx;
 
 typedef enum muca_status {
@@ -78,16 +86,16 @@ enum {
                                      schedule rounded up to whole sweeps, R18) or MUCA_SCHEME_RANDOM_SITE (the paper's
                                      own scheme and units: N_therm = 30 w and N_updates attempted flips per walker;
                                      muca_production then runs therm_sweeps * N and sweeps * N updates per call) */
-    MUCA_OPT_ACCEPTANCE = 8,      /* muca_run_iteration_random_site only: MUCA_ACCEPT_THRESHOLD (default: integer thresholds from
+    MUCA_OPT_TABLE_WINDOW_ROWS = 6, /* STREAMED_PAIRS kernel: rows of the threshold-table window held in shared memory;
+                                     0 = as many as fit.  A value below L*L+1 forces a window (testing) */
+    MUCA_OPT_ROLE_MAP = 7,        /* resident kernel with 4 warp pairs per block: 0 = walker warps share schedulers with
+                                     walker warps, 1 = every scheduler runs one walker and one deviate warp (A/B knob) */
+    MUCA_OPT_ACCEPTANCE = 8       /* muca_run_iteration_random_site only: MUCA_ACCEPT_THRESHOLD (default: integer thresholds from
                                      double omega, R6/R7) or MUCA_ACCEPT_EXPF32, the paper's single-precision form (
                                      DESIGN.md R23): omega rounded to fp32, a proposal j -> j' is accepted iff the difference
                                      D = omega_f[j'] - omega_f[j] >= 0 or U < exp32(D), U the Philox word mapped to (0, 1] as
                                      cuRAND's curand_uniform maps it, exp32 a fixed sequence of fp32 operations (identical on
                                      CPU and GPU, which is what the paper asks of its own code) */
-    MUCA_OPT_ROLE_MAP = 7,        /* resident kernel with 4 warp pairs per block: 0 = walker warps share schedulers with
-                                     walker warps, 1 = every scheduler runs one walker and one deviate warp (A/B knob) */
-    MUCA_OPT_TABLE_WINDOW_ROWS = 6 /* STREAMED_PAIRS kernel: rows of the threshold-table window held in shared memory;
-                                     0 = as many as fit.  A value below L*L+1 forces a window (testing) */
 };
 enum { MUCA_SCHEME_TYPEWRITER = 0, MUCA_SCHEME_RANDOM_SITE = 1 };
 enum { MUCA_ACCEPT_THRESHOLD = 0, MUCA_ACCEPT_EXPF32 = 1 };

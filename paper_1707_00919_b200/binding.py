@@ -29,8 +29,9 @@ EXPORTS = (
     "muca_unpack_spins_device", "muca_get_thresholds", "muca_get_iteration", "muca_set_iteration",
     "muca_last_sweep_ms", "muca_last_error", "muca_debug_philox", "muca_version",
     "muca_flatness", "muca_schedule", "muca_converge", "muca_production", "muca_run_iteration_random_site", "muca_window_stats",
-    "muca_debug_philox_static",
+    "muca_debug_philox_static", "muca_abi_version",
 )
+MUCA_ABI_VERSION = 3            # include/muca.h: the enum values and signatures this file was written against
 MUCA_PHILOX_STATIC_MAX = 4096   # include/muca.h: rows the library's fixed staging array holds
 
 
@@ -74,6 +75,12 @@ def lib():
             raise MucaError(f"{os.path.basename(lib_path())} is not built and cannot be built here: {e}") from e
         path = lib_path()
     L = C.CDLL(path)
+    # The constants at the top of this file are raw integers: a library with another numbering (an older build found on
+    # the path) would silently run a different kernel or option.  Refuse it instead.
+    have = L.muca_abi_version() if hasattr(L, "muca_abi_version") else None
+    if have != MUCA_ABI_VERSION:
+        raise MucaError(f"{os.path.basename(path)} has ABI version {have}, this binding was written against {MUCA_ABI_VERSION} "
+                        f"(include/muca.h MUCA_ABI_VERSION): rebuild the library (python -m paper_1707_00919_b200.build --force)")
     vp, u32p, u64p = C.c_void_p, C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)
     f64p, i8p, i32p = C.POINTER(C.c_double), C.POINTER(C.c_int8), C.POINTER(C.c_int32)
     L.muca_suggest_walkers.argtypes = [C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int)]

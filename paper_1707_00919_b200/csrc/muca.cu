@@ -393,10 +393,12 @@ int launch_random_site(muca_ctx* ctx, const RandomSiteParams& prm, int tpb) {
 extern "C" {
 
 #ifdef MUCA_CHECKED
-const char* muca_version(void) { return "muca_b200 0.2 (sm_100a) +checked"; }
+const char* muca_version(void) { return "muca_b200 0.3 (sm_100a) +checked"; }
 #else
-const char* muca_version(void) { return "muca_b200 0.2 (sm_100a)"; }
+const char* muca_version(void) { return "muca_b200 0.3 (sm_100a)"; }
 #endif
+
+int muca_abi_version(void) { return MUCA_ABI_VERSION; }
 
 int muca_suggest_walkers(int L, int* n_walkers_out, int* pairs_per_sm_out) {
     if (!valid_L(L) || !n_walkers_out || !pairs_per_sm_out) return MUCA_EINVAL;
