@@ -449,38 +449,61 @@ def test_error_paths():
 
 def test_randomized_configurations():
     # seeded random mix of lattice sizes, walker counts (ragged warps), global offsets, kernel variants, launch splits,
-    # table windows, walkers per warp, both update schemes and optional weight updates: every combination must give the
-    # oracle's chains bit for bit (3000 cases of this generator were run once during development)
+    # forced table windows, walkers per warp, walkers started all over the energy range (the sorted per-block windows),
+    # smooth non-zero weights, both update schemes, both acceptance forms of the random-site scheme and optional weight
+    # updates: every combination must give the oracle's chains bit for bit.  (The same generator ran 208 450 trials as a
+    # soak during round 2 without a mismatch: profiles/r02_soak.txt.)
     import random
-    rng = random.Random(20260411)
-    for trial in range(80):
-        L = rng.choice([8, 16, 32, 32, 64, 128])
-        W = rng.choice([1, 3, 31, 32, 33, 64, 97, 130, 257])
+    rng = random.Random(20261106)
+    stats = {"windowed": 0, "undone": 0, "expf": 0, "spread": 0, "random_site": 0}
+    for trial in range(120):
+        L = rng.choice([8, 16, 32, 32, 64, 64, 128])
+        W = rng.choice([1, 3, 31, 32, 33, 64, 97, 130, 257, 300])
         if L == 128:
             W = min(W, 97)
         seed, off = rng.getrandbits(64), rng.choice([0, 0, 5, 1000, 2 ** 31])
-        kernel = rng.choice({8: [0, 1, 3], 16: [0, 1, 2, 3], 32: [0, 1, 2, 3, 3], 64: [0, 1, 2, 3, 3], 128: [0, 1, 2, 3, 3]}[L])
+        kernel = rng.choice([B.MUCA_KERNEL_AUTO, B.MUCA_KERNEL_RESIDENT, B.MUCA_KERNEL_STREAMED, B.MUCA_KERNEL_STREAMED_PAIRS,
+                             B.MUCA_KERNEL_STREAMED_PAIRS])
         g, o = mb.Muca(L, W, seed, walker_offset=off), mo.Oracle(L, W, seed, walker_offset=off)
         tag = [trial, L, W, kernel]
         try:
             g.set_option(B.MUCA_OPT_KERNEL, kernel)
+            if rng.random() < 0.4:                                   # walkers all over the energy range, -2N .. +2N
+                N = L * L
+                nr = np.random.default_rng(rng.getrandbits(32))
+                p = np.linspace(0.0, 0.5, W)[:, None]
+                spins = np.where(nr.random((W, N)) < p, -1, 1).astype(np.int8)
+                yy, xx = np.divmod(np.arange(N), L)
+                spins[1::2] *= np.where((xx + yy) % 2 == 0, 1, -1).astype(np.int8)[None, :]
+                g.set_spins(spins); o.set_spins(spins); tag.append("spread"); stats["spread"] += 1
+                if rng.random() < 0.5:
+                    w = -0.002 * (np.arange(N + 1) - N / 2.0) ** 2 * (64.0 / N)   # smooth weights, maximum in the middle
+                    g.set_log_weights(w); o.set_log_weights(w); tag.append("weights")
             if rng.random() < 0.3:
                 g.set_option(B.MUCA_OPT_MAX_SWEEPS_PER_LAUNCH, rng.choice([1, 2, 3])); tag.append("split")
-            if L >= 32 and kernel in (0, 3) and rng.random() < 0.5:
-                rows = rng.choice([40, 60, 100, 300, 1000]); g.set_option(B.MUCA_OPT_TABLE_WINDOW_ROWS, rows); tag.append(("window", rows))
-            if L <= 32 and kernel in (0, 1) and rng.random() < 0.5:
+            if L >= 32 and kernel in (B.MUCA_KERNEL_AUTO, B.MUCA_KERNEL_STREAMED_PAIRS) and rng.random() < 0.6:
+                rows = rng.choice([40, 60, 100, 300, 600, 1000, 2000]); g.set_option(B.MUCA_OPT_TABLE_WINDOW_ROWS, rows); tag.append(("window", rows))
+            if L <= 32 and kernel in (B.MUCA_KERNEL_AUTO, B.MUCA_KERNEL_RESIDENT) and rng.random() < 0.5:
                 wpw = rng.choice([1, 7, 16, 28, 32]); g.set_option(B.MUCA_OPT_WALKERS_PER_WARP, wpw); tag.append(("wpw", wpw))
+            expf = rng.random() < 0.5                                # the paper's fp32 acceptance (random-site scheme only, R23)
+            if expf:
+                g.set_option(B.MUCA_OPT_ACCEPTANCE, B.MUCA_ACCEPT_EXPF32); tag.append("expf32")
             for it in range(rng.choice([1, 2, 4])):
-                if rng.random() < 0.2:
-                    u0, u1 = rng.choice([0, 17, 100]), rng.choice([0, 1, 999, 4001])
-                    Hg, Ho = g.run_iteration_random_site(u0, u1), o.run_iteration_random_site(u0, u1, n_threads=mo.max_threads())
+                if rng.random() < 0.3:
+                    u0, u1 = rng.choice([0, 17, 100, 255, 256, 257]), rng.choice([0, 1, 999, 4001, 1024, 1023])
+                    Hg = g.run_iteration_random_site(u0, u1)
+                    Ho = (o.run_iteration_random_site_expf if expf else o.run_iteration_random_site)(u0, u1, n_threads=mo.max_threads())
+                    stats["random_site"] += 1; stats["expf"] += int(expf)
                 else:
-                    th, sw = rng.choice([0, 1, 3]), rng.choice([0, 1, 2, 5, 9] if L < 128 else [0, 1, 2])
+                    th, sw = rng.choice([0, 1, 3]), rng.choice([0, 1, 2, 5, 9] if L < 128 else [0, 1, 2, 3])
                     Hg, Ho = g.run_iteration(th, sw), o.run_iteration(th, sw, n_threads=mo.max_threads())
                 assert np.array_equal(Hg, Ho), (tag, it)
                 if rng.random() < 0.7:
                     g.update_weights(); o.update_weights()
             compare_state(g, o, str(tag))
-            assert np.max(np.abs(g.get_log_weights() - o.get_log_weights())) <= LOGW_TOL
+            assert np.max(np.abs(g.get_log_weights() - o.get_log_weights())) <= LOGW_TOL, tag
+            a, b = g.window_stats(); stats["windowed"] += a; stats["undone"] += b
         finally:
             g.close(); o.close()
+    # the mix did reach the paths it is there for
+    assert stats["spread"] >= 30 and stats["windowed"] >= 10 and stats["expf"] >= 10 and stats["random_site"] > stats["expf"], stats
