@@ -35,16 +35,23 @@ UNIT = "flips/s"
 ALU_OPS_PER_FLIP = 11.7             # binding pipe: ALU, 16 lanes per scheduler per clock (profiles/r01_ubench_pipes.txt)
 OPS_PER_FLIP = 20.0                 # all thread-instructions (issue slots: 32 lanes per scheduler per clock)
 SCHED_PER_SM, ALU_LANES, ISSUE_LANES = 4, 16, 32
-# Counters of ONE sweep-kernel launch per workload, copied from the ncu --set full captures under profiles/ by hand into
-# this file (dram__bytes_read.sum + dram__bytes_write.sum, pipe and issue utilisation; profiles/README.md names the
-# captures): read at run time, nothing is measured under the profiler here.
-NCU_SUMMARY = os.path.join(ROOT, "profiles", "r02_ncu_summary.json")
+# Counters of ONE sweep-kernel launch per workload, copied by hand from the ncu --set full captures under profiles/ into
+# that JSON file (dram__bytes_read.sum + dram__bytes_write.sum, pipe and issue utilisation; profiles/README.md names the
+# captures): read at run time, nothing is measured under the profiler here.  The file records the commit and the sha256
+# of csrc/ (paper_1707_00919_b200.build.csrc_sha256) it was captured from; when the sources have changed since, the
+# entry is still printed, with "stale": true beside it.
+NCU_SUMMARY = os.path.join(ROOT, "profiles", "r03_ncu_summary.json")
 
 
 def ncu_summary(workload):
     try:
         with open(NCU_SUMMARY) as f:
-            return json.load(f).get(workload)
+            doc = json.load(f)
+        entry = doc.get(workload)
+        if entry is None:
+            return None
+        from paper_1707_00919_b200 import build as lib_build
+        return dict(entry, stale=(entry.get("captured_from") or {}).get("csrc_sha256") != lib_build.csrc_sha256())
     except Exception:
         return None
 
@@ -58,6 +65,7 @@ def parse():
     ap.add_argument("--config", default="L32_w16384")
     ap.add_argument("--ref-walkers", type=int, default=128, help="walker sample of the reference / cpu_baseline legs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the untimed legs on configs 4 and 5")
     return ap.parse_args()
 
 
@@ -158,6 +166,74 @@ class ClockSampler:
                 "how": "NVML from the main thread after every iteration of the timed steps"}
 
 
+# ------------------------------------------------------------------------------------------------ the other configs
+def other_configs(mb, cfg_main, peak, f_max_hz, device_index):
+    """north_star: "throughput is reported on each config".  The headline legs time ONE workload; here, after them and
+    outside their timed regions, the two other large configs run two jobs each, and L = 128 once more in the regime of a
+    production run (walkers spread over the whole energy range -> sorted per-block table windows).
+    Sweep kernels only: the library's own CUDA events around the launches of every iteration (muca_last_sweep_ms)."""
+    from paper_1707_00919_b200.workloads import by_name, onsager_log_dos
+    res = {}
+
+    def entry(c, W, flips, ms, launches, sampler, what, extra=None):
+        fps = flips / (ms * 1e-3)
+        e = {"value": fps, "unit": UNIT, "c_flip_cycles": W * f_max_hz / fps, "frac": fps * ALU_OPS_PER_FLIP / 1e12 / peak,
+             "sweep_ms": ms, "launches": launches, "clocks": sampler.result(), "what": what}
+        e.update(extra or {})
+        return e
+
+    for name in ("L64_w32768", "L128_w8192"):
+        if name == cfg_main.name:
+            continue
+        c = by_name(name)
+        sampler = ClockSampler(device_index)
+        ms = 0.0; launches = 0; steps = 2
+        for _ in range(steps):
+            g = mb.Muca(c.L, c.n_walkers, c.seed)
+            for _ in range(c.iterations):
+                g.run_iteration(c.therm_sweeps, c.sweeps)
+                m, k = g.last_sweep_ms()
+                ms += m; launches += k
+                sampler.sample()
+                g.update_weights()
+            g.close()
+        res[name] = entry(c, c.n_walkers, steps * mb.total_flips(c), ms, launches, sampler,
+                          f"{steps} jobs of {c.iterations} x ({c.therm_sweeps}+{c.sweeps}) sweeps, sweep kernels only")
+    # L = 128, walkers spread from -2N to +2N (walker k: a fraction k/2W of its spins down, every second walker times a
+    # checkerboard), weights omega(E) = -N s(E/N) from the infinite-lattice entropy (workloads.onsager_log_dos: no exact
+    # g(E) exists in the tree for L = 128), close enough to flat-histogram weights to keep them spread: 3 x (20 + 50) sweeps
+    c = by_name("L128_w8192")
+    W, N, L = c.n_walkers, c.N, c.L
+    rng = np.random.default_rng(c.seed)
+    spins = np.empty((W, N), dtype=np.int8)
+    pk = np.linspace(0.0, 0.5, W, dtype=np.float32)
+    for a in range(0, W, 1024):
+        spins[a:a + 1024] = np.where(rng.random((min(1024, W - a), N), dtype=np.float32) < pk[a:a + 1024, None], -1, 1)
+    yy, xx = np.divmod(np.arange(N), L)
+    spins[1::2] *= np.where((xx + yy) % 2 == 0, 1, -1).astype(np.int8)[None, :]
+    g = mb.Muca(L, W, c.seed)
+    g.set_spins(spins)
+    g.set_log_weights(-onsager_log_dos(L))
+    sampler = ClockSampler(device_index)
+    ms = 0.0; launches = 0
+    g.run_iteration(c.therm_sweeps, c.sweeps)                                  # untimed first call
+    for _ in range(3):
+        g.run_iteration(c.therm_sweeps, c.sweeps)
+        m, k = g.last_sweep_ms()
+        ms += m; launches += k
+        sampler.sample()
+    E = g.get_energies()
+    windowed, undone = g.window_stats()
+    g.close()
+    res["L128_w8192_spread"] = entry(c, W, 3 * W * N * (c.therm_sweeps + c.sweeps), ms, launches, sampler,
+                                     "walkers spread over the whole energy range, fixed weights -N s_Onsager(E/N), 3 x "
+                                     f"({c.therm_sweeps}+{c.sweeps}) sweeps: sorted per-block table windows; the time "
+                                     "includes the host's sorting and the snapshots between the launches",
+                                     {"slots_spanned": int((E.max() - E.min()) // 4), "windowed_iterations": windowed,
+                                      "undone_launches": undone})
+    return res
+
+
 # ------------------------------------------------------------------------------------------------ our arm
 def run_ours(args, cfg):
     import torch
@@ -183,27 +259,26 @@ def run_ours(args, cfg):
     h_spins_t = torch.empty((W, cfg.L, cfg.L), dtype=torch.int8).pin_memory()
     h_spins = h_spins_t.numpy()
     l2_flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    Hbuf = torch.zeros(cfg.n_bins, dtype=torch.int64, device=dev)
 
     stats = {"sweep_ms": 0.0, "sweep_launches": 0, "launches": 0}
     sampler = ClockSampler(local)
 
     def job(e2e: bool, record: bool):
-        g = mb.Muca(cfg.L, W, cfg.seed, walker_offset=offset)                  # a0 (init kernel)
+        # ShardedMuca (paper_1707_00919_b200/parallel.py) is the N > 1 path the tests cover (tests/test_parallel_gloo.py):
+        # contiguous walker ranges with global ids, one all-reduce of H per iteration -- the method's one exchange,
+        # PAPER.md:87 --, the same Eq. (4) on every rank.  At N = 1 it is the plain context plus a copy of H.
+        sm = mb.ShardedMuca(cfg.L, world * W, cfg.seed)                        # a0 (init kernel)
+        g = sm.engine
+        assert (sm.offset, sm.count) == (offset, W)
         n_launch = 1
         for _ in range(cfg.iterations):
-            H = g.run_iteration(cfg.therm_sweeps, cfg.sweeps)                  # a1-a4 (+ H2D table, D2H H)
+            sm.run_iteration(cfg.therm_sweeps, cfg.sweeps)                     # a1-a4 (+ H2D table, D2H H), all-reduce(H)
             ms, k = g.last_sweep_ms()
             n_launch += k
             if record:
                 stats["sweep_ms"] += ms; stats["sweep_launches"] += k
                 sampler.sample()                                               # clocks line of the contract (see ClockSampler)
-            if world > 1:                                                      # the one exchange of the method
-                Hbuf.copy_(torch.from_numpy(H.astype(np.int64)))
-                dist.all_reduce(Hbuf)
-                g.update_weights_with(Hbuf.cpu().numpy().astype(np.uint64))    # a5
-            else:
-                g.update_weights()                                             # a5
+            sm.update_weights()                                                # a5
         if e2e:
             g.get_energies(h_E)
             g.get_spins(h_spins)                                               # a6: unpack kernel + D2H
@@ -212,7 +287,7 @@ def run_ours(args, cfg):
         n_launch += 1
         if record:
             stats["launches"] += n_launch
-        g.close()
+        sm.close()
 
     def timed(e2e: bool, steps: int, record: bool):
         total_ms = 0.0
@@ -279,7 +354,7 @@ def run_ours(args, cfg):
         "kernel": kernel, "kernel_flips_per_s": kern_flips_s,
         "ops_per_flip": ALU_OPS_PER_FLIP, "avg_launch_ms": avg_launch_s * 1e3, "kernel_share_of_step": stats["sweep_ms"] / ms_dev,
         "c_flip_cycles": W * f_max_hz / kern_flips_s,
-        "peak_source": f"148 SM x 4 schedulers x 16 ALU lanes x sm_max_mhz ({pk_kind} MEASURED_PEAKS.json clock); "
+        "peak_source": f"{SM_COUNT} SM x {SCHED_PER_SM} schedulers x {ALU_LANES} ALU lanes x sm_max_mhz ({pk_kind} MEASURED_PEAKS.json clock); "
                        "11.7 ALU-only instructions per attempted flip (DESIGN.md 6.2)",
         "issue": {"achieved": kern_flips_s * OPS_PER_FLIP / 1e12, "peak": issue_peak, "unit": "T thread-instructions/s",
                   "frac": kern_flips_s * OPS_PER_FLIP / 1e12 / issue_peak, "ops_per_flip": OPS_PER_FLIP},
@@ -322,6 +397,8 @@ def run_ours(args, cfg):
         out["frozen_weights"] = {"value": float(np.median(fz)), "unit": UNIT,
                                  "what": f"sweep kernel only, 3 x {cfg.sweeps} measured sweeps after the {cfg.iterations} "
                                          "configured iterations, weights not updated (outside the timed region)"}
+    if world == 1 and not args.no_other_configs:
+        out["other_configs"] = other_configs(mb, cfg, peak, f_max_hz, local)
     if world == 1 and not args.no_cpu_baseline:
         import muca_oracle as mo
         cores = mo.max_threads()

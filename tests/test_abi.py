@@ -63,3 +63,22 @@ def test_product_does_not_import_the_oracle():
                 src = open(os.path.join(dirpath, f)).read()
                 assert "muca_oracle" not in src and "oracle/" not in src.replace("shares nothing with oracle/", "").replace(
                     "Shares nothing with oracle/", "").replace("imported by neither oracle/", ""), f
+
+
+def test_onsager_stand_in_is_close_to_the_exact_density_of_states():
+    # workloads.onsager_log_dos (bench.py's weights for spread walkers at L = 128, where the tree has no exact g(E)):
+    # against the exact finite-lattice g(E) of tests/golden/ it must be flat-histogram quality, i.e. off by a few units
+    # of ln g over hundreds of units of range, symmetric in E, and largest in the middle
+    import math
+    import numpy as np
+    from paper_1707_00919_b200.workloads import onsager_log_dos
+    for L in (16, 32):
+        with open(os.path.join(ROOT, "tests", "golden", f"ising_dos_L{L}.txt")) as f:
+            g = [int(x) for x in f if not x.startswith("#")]
+        approx = onsager_log_dos(L)
+        exact = np.array([math.log(v) if v > 0 else np.nan for v in g])
+        d = exact - approx
+        assert approx.shape == (L * L + 1,) and np.all(np.isfinite(approx))
+        assert np.nanmax(np.abs(d)) < 4.5, (L, np.nanmin(d), np.nanmax(d))
+        assert np.allclose(approx, approx[::-1]) and np.argmax(approx) == L * L // 2
+        assert abs(approx[L * L // 2] - L * L * math.log(2.0)) < 1e-3 and abs(approx[0]) < 1e-3

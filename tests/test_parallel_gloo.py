@@ -86,14 +86,14 @@ def test_two_ranks_reproduce_the_single_process_run(tmp_path):
 
 
 # ------------------------------------------------------------------------------------------------ the same with the CUDA library
-def _gpu_worker(rank, world, port, out_dir):
+def _gpu_worker(rank, world, port, out_dir, backend="gloo"):
     for p in (ROOT, os.path.join(ROOT, "oracle"), os.path.join(ROOT, "tests")):
         if p not in sys.path:
             sys.path.insert(0, p)
     import torch
     import torch.distributed as dist
     torch.cuda.set_device(rank % torch.cuda.device_count())     # one process per GPU where there are several
-    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world)
+    dist.init_process_group(backend, init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world)
     try:
         sm = ShardedMuca(32, 301, 170700919)                    # default engine: the CUDA library binding
         Hs = []
@@ -108,12 +108,18 @@ def _gpu_worker(rank, world, port, out_dir):
 
 
 @pytest.mark.gpu
-def test_two_ranks_with_the_cuda_library_reproduce_the_oracle(tmp_path):
+@pytest.mark.parametrize("backend", ["gloo", "nccl"])
+def test_two_ranks_with_the_cuda_library_reproduce_the_oracle(tmp_path, backend):
     # ShardedMuca with its default engine (libmuca_b200 through the binding) in two processes -- on two GPUs where the box
     # has them, otherwise both on cuda:0 --, histogram sum over gloo: global walker ids make the chains independent of
-    # the split (R16), so the result is the single-process oracle's
-    port = 31500 + (os.getpid() % 2000)
-    mp.spawn(_gpu_worker, args=(2, port, str(tmp_path)), nprocs=2, join=True)
+    # the split (R16), so the result is the single-process oracle's.  This is the path bench.py takes for --gpus N > 1.
+    # The nccl variant (the all-reduce on device tensors, as bench.py runs it under torchrun) needs a GPU per rank: NCCL
+    # refuses two ranks on one device, so on a one-GPU box it is skipped and only the gloo variant runs.
+    import torch
+    if backend == "nccl" and torch.cuda.device_count() < 2:
+        pytest.skip("NCCL needs one GPU per rank; this box has one")
+    port = 31500 + (os.getpid() % 2000) + (0 if backend == "gloo" else 2000)
+    mp.spawn(_gpu_worker, args=(2, port, str(tmp_path), backend), nprocs=2, join=True)
     r0, r1 = np.load(tmp_path / "r0.npz"), np.load(tmp_path / "r1.npz")
     ref = mo.Oracle(32, 301, 170700919)
     Hs = []
